@@ -1,0 +1,279 @@
+"""ctypes binding and step composition for the CPU fp64 ORACLE (oracle/sp_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It imports nothing from the CUDA
+package and never receives a value the CUDA path produced.
+
+All tensors are numpy arrays; bf16 tensors are uint16 bit patterns.  Step names O1..O7 and the
+PAPER.md citations are in sp_oracle.c's header.  This file only marshals arguments and chains the
+steps in the paper's order (Alg.1 steps 2-5; Alg.2 steps 2,4,5).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sp_oracle.c")
+_LIB = os.path.join(_HERE, "libsp_oracle.so")
+
+MODE_ORACLE = 0
+MODE_INDEXER = 1
+
+
+def build(force: bool = False) -> str:
+    """Compile sp_oracle.c with gcc (fp64, OpenMP, no fast-math, no FMA contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("batch", C.c_int32), ("L", C.c_int32), ("cu_seqlens", C.POINTER(C.c_int32)),
+        ("Hq", C.c_int32), ("Hkv", C.c_int32), ("d", C.c_int32), ("k", C.c_int32),
+        ("b_sel", C.c_int32), ("hidden", C.c_int32), ("d_idx", C.c_int32),
+        ("scale", C.c_double), ("idx_scale", C.c_double),
+        ("local_window", C.c_int32), ("local_bias", C.c_double),
+    ]
+
+
+@dataclass
+class Problem:
+    """The paper's problem statement for one layer."""
+    L: int
+    Hq: int
+    Hkv: int
+    d: int
+    k: int
+    b_sel: int = 1
+    hidden: int = 0
+    d_idx: int = 0
+    scale: Optional[float] = None        # None -> 1/sqrt(d)
+    idx_scale: Optional[float] = None    # None -> 1/sqrt(d_idx)
+    local_window: int = 0
+    local_bias: float = 0.0
+    cu_seqlens: Optional[Sequence[int]] = None
+
+    def c_params(self):
+        cu = None
+        batch = 1
+        keep = None
+        if self.cu_seqlens is not None:
+            keep = np.ascontiguousarray(np.asarray(self.cu_seqlens, dtype=np.int32))
+            cu = keep.ctypes.data_as(C.POINTER(C.c_int32))
+            batch = len(keep) - 1
+        p = _Params(
+            batch, self.L, cu, self.Hq, self.Hkv, self.d, self.k, self.b_sel, self.hidden, self.d_idx,
+            self.scale if self.scale is not None else 1.0 / math.sqrt(self.d),
+            self.idx_scale if self.idx_scale is not None else (1.0 / math.sqrt(self.d_idx) if self.d_idx else 0.0),
+            self.local_window, self.local_bias,
+        )
+        p._keep = keep
+        return p
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_num_rows.restype = C.c_int32
+        _lib.orc_row_info.restype = C.c_int32
+        _lib.orc_row_of_pos.restype = C.c_int32
+        _lib.orc_max_threads.restype = C.c_int32
+    return _lib
+
+
+def _u16(a):
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.uint16, a.dtype
+    return a
+
+
+def _i32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def _ptr(a, ty):
+    return a.ctypes.data_as(C.POINTER(ty))
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+def f64_to_bf16(x) -> np.ndarray:
+    x = np.ascontiguousarray(np.asarray(x, dtype=np.float64))
+    out = np.empty(x.shape, dtype=np.uint16)
+    lib().orc_f64_to_bf16(_ptr(x, C.c_double), C.c_int64(x.size), _ptr(out, C.c_uint16))
+    return out
+
+
+def bf16_to_f64(b) -> np.ndarray:
+    b = np.ascontiguousarray(b, dtype=np.uint16)
+    return (b.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def num_rows(pb: Problem) -> int:
+    p = pb.c_params()
+    return int(lib().orc_num_rows(C.byref(p)))
+
+
+def row_info(pb: Problem, row: int):
+    """(seq_start, first local position, last local position) of a support row (A8)."""
+    p = pb.c_params()
+    a, b, c = C.c_int32(), C.c_int32(), C.c_int32()
+    rc = lib().orc_row_info(C.byref(p), C.c_int32(row), C.byref(a), C.byref(b), C.byref(c))
+    if rc != 0:
+        raise IndexError(row)
+    return a.value, b.value, c.value
+
+
+def row_of_pos(pb: Problem, pos: int) -> int:
+    p = pb.c_params()
+    return int(lib().orc_row_of_pos(C.byref(p), C.c_int32(pos)))
+
+
+def project(pb: Problem, X, W, rows=None) -> np.ndarray:
+    """O3' projection: bf16_rne(X[rows] @ W) with an fp64 sum (A14)."""
+    X, W = _u16(X), _u16(W)
+    rows = _i32(np.arange(X.shape[0]) if rows is None else rows)
+    out = np.empty((len(rows), pb.d_idx), dtype=np.uint16)
+    lib().orc_project(_ptr(X, C.c_uint16), _ptr(W, C.c_uint16), C.c_int32(pb.hidden), C.c_int32(pb.d_idx),
+                      _ptr(rows, C.c_int32), C.c_int32(len(rows)), _ptr(out, C.c_uint16))
+    return out
+
+
+def query_scores(pb: Problem, mode: int, A, B, pos, ld: Optional[int] = None) -> np.ndarray:
+    """Per-query score rows: mass P_t (mode ORACLE; A=Q, B=K) or indexer logits
+    (mode INDEXER; A=q_idx, B=k_idx).  Returns [len(pos), ld] fp64, -inf beyond t."""
+    A, B = _u16(A), _u16(B)
+    pos = _i32(pos)
+    ld = int(ld or pb.L)
+    out = np.empty((len(pos), ld), dtype=np.float64)
+    p = pb.c_params()
+    lib().orc_query_scores(C.byref(p), C.c_int32(mode), _ptr(A, C.c_uint16), _ptr(B, C.c_uint16),
+                           _ptr(pos, C.c_int32), C.c_int32(len(pos)), _ptr(out, C.c_double), C.c_int64(ld))
+    return out
+
+
+def support_scores(pb: Problem, mode: int, A, B, rows, ld: Optional[int] = None):
+    """O4: support-row scores R. Returns (R [len(rows), ld] fp64, n_valid int32)."""
+    A, B = _u16(A), _u16(B)
+    rows = _i32(rows)
+    ld = int(ld or pb.L)
+    out = np.empty((len(rows), ld), dtype=np.float64)
+    nv = np.empty(len(rows), dtype=np.int32)
+    p = pb.c_params()
+    lib().orc_support_scores(C.byref(p), C.c_int32(mode), _ptr(A, C.c_uint16), _ptr(B, C.c_uint16),
+                             _ptr(rows, C.c_int32), C.c_int32(len(rows)), _ptr(out, C.c_double),
+                             C.c_int64(ld), _ptr(nv, C.c_int32))
+    return out, nv
+
+
+def topk(scores, n_valid, k: int, seq_start=None):
+    """O5: per row the first min(k,n) of (score desc, index asc), ascending, -1 padded."""
+    scores = np.ascontiguousarray(np.asarray(scores, dtype=np.float64))
+    if scores.ndim == 1:
+        scores = scores[None, :]
+    n_valid = _i32(n_valid)
+    nrows, ld = scores.shape
+    idx = np.empty((nrows, k), dtype=np.int32)
+    cnt = np.empty(nrows, dtype=np.int32)
+    ss = _i32(seq_start) if seq_start is not None else None
+    lib().orc_topk(_ptr(scores, C.c_double), C.c_int64(ld), _ptr(n_valid, C.c_int32),
+                   _ptr(ss, C.c_int32) if ss is not None else None,
+                   C.c_int32(nrows), C.c_int32(k), _ptr(idx, C.c_int32), _ptr(cnt, C.c_int32))
+    return idx, cnt
+
+
+def sparse_attn(pb: Problem, Q, K, V, pos, sup, want_lse: bool = False):
+    """O6: attention recomputed on the support. sup: [len(pos), k] packed idx."""
+    Q, K, V = _u16(Q), _u16(K), _u16(V)
+    pos = _i32(pos)
+    sup = _i32(sup)
+    assert sup.shape == (len(pos), pb.k), (sup.shape, len(pos), pb.k)
+    o = np.empty((len(pos), pb.Hq, pb.d), dtype=np.float64)
+    lse = np.empty((len(pos), pb.Hq), dtype=np.float64)
+    p = pb.c_params()
+    lib().orc_sparse_attn(C.byref(p), _ptr(Q, C.c_uint16), _ptr(K, C.c_uint16), _ptr(V, C.c_uint16),
+                          _ptr(pos, C.c_int32), C.c_int32(len(pos)), _ptr(sup, C.c_int32),
+                          _ptr(o, C.c_double), _ptr(lse, C.c_double))
+    return (o, lse) if want_lse else o
+
+
+def dense_attn(pb: Problem, Q, K, V, pos, want_lse: bool = False):
+    """O7: dense causal GQA attention by brute force."""
+    Q, K, V = _u16(Q), _u16(K), _u16(V)
+    pos = _i32(pos)
+    o = np.empty((len(pos), pb.Hq, pb.d), dtype=np.float64)
+    lse = np.empty((len(pos), pb.Hq), dtype=np.float64)
+    p = pb.c_params()
+    lib().orc_dense_attn(C.byref(p), _ptr(Q, C.c_uint16), _ptr(K, C.c_uint16), _ptr(V, C.c_uint16),
+                         _ptr(pos, C.c_int32), C.c_int32(len(pos)), _ptr(o, C.c_double), _ptr(lse, C.c_double))
+    return (o, lse) if want_lse else o
+
+
+# ---------------------------------------------------------------------------------------------
+# Composition in the paper's order
+# ---------------------------------------------------------------------------------------------
+
+@dataclass
+class LayerResult:
+    rows: np.ndarray        # support rows evaluated
+    scores: np.ndarray      # R [len(rows), ld] fp64
+    n_valid: np.ndarray     # [len(rows)]
+    idx: np.ndarray         # [len(rows), k] packed positions, ascending, -1 padded
+    cnt: np.ndarray         # [len(rows)]
+    pos: np.ndarray         # query positions whose outputs were computed
+    out: np.ndarray         # [len(pos), Hq, d] fp64
+    q_idx: Optional[np.ndarray] = None
+    k_idx: Optional[np.ndarray] = None
+
+
+def select_support(pb: Problem, mode: int, A, B, rows):
+    """Alg.1 steps 2-4 / Alg.2 steps 4-5 (first half): scores -> causal top-k for the given rows."""
+    rows = _i32(rows)
+    R, nv = support_scores(pb, mode, A, B, rows)
+    starts = np.array([row_info(pb, int(r))[0] for r in rows], dtype=np.int32)
+    idx, cnt = topk(R, nv, pb.k, starts)
+    return R, nv, idx, cnt
+
+
+def prefill_layer(pb: Problem, mode: int, Q, K, V, X=None, Wqi=None, Wki=None,
+                  rows=None, pos=None, q_idx=None, k_idx=None) -> LayerResult:
+    """One patched layer on a subset of support rows (all when rows is None).
+
+    ORACLE mode: Alg.1 steps 2-5. INDEXER mode: Alg.2 steps 2,4,5.
+    `pos` (query positions whose output is computed) defaults to every query of the chosen rows.
+    """
+    rows = _i32(np.arange(num_rows(pb)) if rows is None else rows)
+    if mode == MODE_INDEXER:
+        if q_idx is None:
+            q_idx = project(pb, X, Wqi)
+        if k_idx is None:
+            k_idx = project(pb, X, Wki)
+        A, B = q_idx, k_idx
+    else:
+        A, B = Q, K
+    R, nv, idx, cnt = select_support(pb, mode, A, B, rows)
+    if pos is None:
+        pos = []
+        for r in rows:
+            s0, t0, t1 = row_info(pb, int(r))
+            pos.extend(range(s0 + t0, s0 + t1 + 1))
+    pos = _i32(pos)
+    row_index = {int(r): i for i, r in enumerate(rows)}
+    sup = np.stack([idx[row_index[row_of_pos(pb, int(t))]] for t in pos]) if len(pos) else np.empty((0, pb.k), np.int32)
+    out = sparse_attn(pb, Q, K, V, pos, sup)
+    return LayerResult(rows, R, nv, idx, cnt, pos, out, q_idx, k_idx)

@@ -1,0 +1,398 @@
+"""Pins for the CPU oracle (oracle/sp_oracle.c) against things OTHER than itself: values the paper
+prints, closed forms, invariants, library routines and a numpy brute force on tiny inputs.
+Each pin is chosen so that a plausible slip (dropped term, wrong sign/index, transposed operand,
+off-by-one in the causal bound, wrong head mean) fails at least one of them.  All CPU, no GPU."""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import bruteforce as bf
+from oracle import oracle as orc
+from paper_2606_07703_b200 import inputs as gen
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def rand_bf16(seed, shape, sigma=1.0):
+    rng = np.random.Generator(np.random.Philox(seed))
+    return gen.f32_to_bf16((rng.standard_normal(shape) * sigma).astype(np.float32))
+
+
+def small_problem(L=48, Hq=4, Hkv=2, d=8, k=6, b=1, seed=1, **kw):
+    pb = orc.Problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=b, **kw)
+    Q = rand_bf16(seed, (L, Hq, d))
+    K = rand_bf16(seed + 1, (L, Hkv, d))
+    V = rand_bf16(seed + 2, (L, Hkv, d))
+    return pb, Q, K, V
+
+
+# ---------------------------------------------------------------- bf16 rounding (A14)
+
+def test_bf16_rne_known_cases():
+    x = np.array([1.0, 1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8, 1.0 + 2.0 ** -8 + 2.0 ** -40,
+                  -1.0 - 2.0 ** -8, 0.0, 3.140625, 2.0 ** -130, 1e39])
+    want = np.array([1.0, 1.0, 1.015625, 1.0078125, -1.0, 0.0, 3.140625, 2.0 ** -130, np.inf])
+    got = orc.bf16_to_f64(orc.f64_to_bf16(x))
+    assert np.array_equal(got, want), (got, want)
+
+
+def test_bf16_roundtrip_all_finite_patterns():
+    b = np.arange(0, 0x7F80, dtype=np.uint16)  # all non-negative finite bf16
+    assert np.array_equal(orc.f64_to_bf16(orc.bf16_to_f64(b)), b)
+    # midpoint between consecutive values goes to the even pattern
+    v = orc.bf16_to_f64(b)
+    mid = (v[:-1] + v[1:]) / 2
+    r = orc.f64_to_bf16(mid)
+    even = np.where(b[:-1] % 2 == 0, b[:-1], b[1:])
+    assert np.array_equal(r, even)
+
+
+# ---------------------------------------------------------------- P3: the paper's own numbers
+
+def kept_pairs(S, k):
+    return k * S - k * (k - 1) // 2
+
+
+def test_paper_printed_sparsities():
+    n = 0
+    for line in open(os.path.join(HERE, "golden", "paper_sparsity.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        S, k, printed, dec = line.split()[:4]
+        S, k, dec = int(S), int(k), int(dec)
+        sparsity = 100.0 * (1.0 - kept_pairs(S, k) / (S * (S + 1) / 2))
+        assert round(sparsity, dec) == float(printed), (S, k, sparsity, printed)
+        n += 1
+    assert n == 5
+
+
+@pytest.mark.parametrize("L,k", [(40, 7), (33, 33), (20, 64), (64, 1)])
+def test_per_query_counts_match_paper_accounting(L, k):
+    """Sum over per-query rows of cnt == k*L - k(k-1)/2 under readings A1/A3."""
+    R = np.random.default_rng(0).standard_normal((L, L))
+    nv = np.arange(1, L + 1)
+    idx, cnt = orc.topk(R, nv, k)
+    kk = min(k, L)
+    assert int(cnt.sum()) == kept_pairs(L, kk)
+    assert int((idx >= 0).sum()) == kept_pairs(L, kk)
+    assert np.array_equal(cnt, np.minimum(k, nv))
+
+
+def test_config1_pair_count():
+    assert kept_pairs(1024, 256) == 229504 and 1024 * 1025 // 2 == 524800
+
+
+# ---------------------------------------------------------------- P7: hand-worked case
+
+def test_handworked_L4():
+    """L=4, Hq=2, Hkv=1, d=1.  q[t,0]=1, q[t,1]=0, k_s = s, scale = ln 2, v_s = s.
+    Head 0 has logits s*ln2 -> weights 2^s; head 1 is uniform.  From PAPER.md:94, :123:
+      P_1 = ((1/3+1/2)/2, (2/3+1/2)/2) = (5/12, 7/12)
+      P_2 = ((1/7+1/3)/2, (2/7+1/3)/2, (4/7+1/3)/2) = (5/21, 13/42, 19/42)
+      P_3 = ((1/15+1/4)/2, (2/15+1/4)/2, (4/15+1/4)/2, (8/15+1/4)/2) = (19,23,31,47)/120
+    Per-query k=2: S_1={0,1}, S_2={1,2}, S_3={2,3};
+      o[1]=(2/3,1/2), o[2]=(5/3,3/2), o[3]=(8/3,5/2), o[0]=(0,0).
+    Block b=2,k=2: block {2,3}: R=(5/21,13/42,19/42,47/120) -> S={2,3};
+      query 2 re-masks to {2} -> o[2]=(2,2); query 3 -> (8/3,5/2). Block {0,1}: S={0,1}."""
+    F = Fraction
+    one = gen.f32_to_bf16(np.array([1.0], np.float32))[0]
+    Q = np.zeros((4, 2, 1), np.uint16)
+    Q[:, 0, 0] = one
+    K = gen.f32_to_bf16(np.arange(4, dtype=np.float32)).reshape(4, 1, 1)
+    V = K.copy()
+    pb = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=2, b_sel=1, scale=math.log(2.0))
+    P = orc.query_scores(pb, orc.MODE_ORACLE, Q, K, np.arange(4))
+    want = [[F(1)], [F(5, 12), F(7, 12)], [F(5, 21), F(13, 42), F(19, 42)],
+            [F(19, 120), F(23, 120), F(31, 120), F(47, 120)]]
+    for t in range(4):
+        assert np.allclose(P[t, :t + 1], [float(x) for x in want[t]], rtol=0, atol=1e-15)
+        assert np.all(np.isneginf(P[t, t + 1:]))
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    assert res.idx.tolist() == [[0, -1], [0, 1], [1, 2], [2, 3]]
+    assert res.cnt.tolist() == [1, 2, 2, 2]
+    o = res.out[:, :, 0]
+    want_o = [[0, 0], [F(2, 3), F(1, 2)], [F(5, 3), F(3, 2)], [F(8, 3), F(5, 2)]]
+    assert np.allclose(o, np.array(want_o, dtype=float), rtol=0, atol=1e-14)
+    # block-shared
+    pbb = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=2, b_sel=2, scale=math.log(2.0))
+    R, nv = orc.support_scores(pbb, orc.MODE_ORACLE, Q, K, [0, 1])
+    assert nv.tolist() == [2, 4]
+    assert np.allclose(R[1], [5 / 21, 13 / 42, 19 / 42, 47 / 120], atol=1e-15)
+    assert np.allclose(R[0, :2], [1.0, 7 / 12], atol=1e-15) and np.all(np.isneginf(R[0, 2:]))
+    resb = orc.prefill_layer(pbb, orc.MODE_ORACLE, Q, K, V)
+    assert resb.idx.tolist() == [[0, 1], [2, 3]]
+    want_ob = [[0, 0], [F(2, 3), F(1, 2)], [2, 2], [F(8, 3), F(5, 2)]]
+    assert np.allclose(resb.out[:, :, 0], np.array(want_ob, dtype=float), rtol=0, atol=1e-14)
+    # k=1: the mass is increasing in s for both heads, so S_t={t} and o[t]=v_t=t
+    pb1 = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=1, b_sel=1, scale=math.log(2.0))
+    r1 = orc.prefill_layer(pb1, orc.MODE_ORACLE, Q, K, V)
+    assert r1.idx[:, 0].tolist() == [0, 1, 2, 3]
+    assert np.allclose(r1.out[:, :, 0], np.arange(4)[:, None], atol=1e-15)
+
+
+# ---------------------------------------------------------------- P1: mass invariants
+
+def test_mass_rows_sum_to_one_and_nonneg():
+    pb, Q, K, V = small_problem(L=96, Hq=8, Hkv=2, d=16)
+    P = orc.query_scores(pb, orc.MODE_ORACLE, Q, K, np.arange(pb.L))
+    for t in range(pb.L):
+        assert abs(P[t, :t + 1].sum() - 1.0) < 1e-12
+        assert (P[t, :t + 1] >= 0).all()
+        assert np.all(np.isneginf(P[t, t + 1:]))
+
+
+def test_mass_head_permutation_within_groups():
+    pb, Q, K, V = small_problem(L=40, Hq=8, Hkv=2, d=8)
+    P0 = orc.query_scores(pb, orc.MODE_ORACLE, Q, K, np.arange(pb.L))
+    perm = [3, 1, 0, 2, 5, 7, 6, 4]                          # stays inside each KV group of 4
+    P1 = orc.query_scores(pb, orc.MODE_ORACLE, Q[:, perm], K, np.arange(pb.L))
+    fin = np.isfinite(P0)
+    assert np.allclose(P0[fin], P1[fin], rtol=0, atol=1e-15)
+    # swapping whole groups together with their KV heads
+    gperm = [4, 5, 6, 7, 0, 1, 2, 3]
+    P2 = orc.query_scores(pb, orc.MODE_ORACLE, Q[:, gperm], K[:, [1, 0]], np.arange(pb.L))
+    assert np.allclose(P0[fin], P2[fin], rtol=0, atol=1e-15)
+
+
+def test_identical_heads_give_that_heads_softmax():
+    from scipy.special import softmax
+    L, d = 32, 8
+    q1 = rand_bf16(5, (L, 1, d))
+    K = rand_bf16(6, (L, 1, d))
+    Q = np.repeat(q1, 4, axis=1)
+    pb = orc.Problem(L=L, Hq=4, Hkv=1, d=d, k=4)
+    P = orc.query_scores(pb, orc.MODE_ORACLE, Q, K, np.arange(L))
+    z = (orc.bf16_to_f64(q1)[:, 0] @ orc.bf16_to_f64(K)[:, 0].T) / math.sqrt(d)
+    for t in range(L):
+        assert np.allclose(P[t, :t + 1], softmax(z[t, :t + 1]), rtol=1e-13, atol=0)
+
+
+def test_gqa_equals_mha_with_repeated_kv():
+    pb, Q, K, V = small_problem(L=40, Hq=8, Hkv=2, d=8, k=5)
+    pm = orc.Problem(L=40, Hq=8, Hkv=8, d=8, k=5)
+    Kr, Vr = np.repeat(K, 4, axis=1), np.repeat(V, 4, axis=1)
+    a = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    b = orc.prefill_layer(pm, orc.MODE_ORACLE, Q, Kr, Vr)
+    assert np.array_equal(a.idx, b.idx)
+    assert np.allclose(a.out, b.out, rtol=0, atol=1e-15)
+    # a WRONG group map (interleaved instead of contiguous, A5) must be visible on this input
+    Ki = np.tile(K, (1, 4, 1))
+    c = orc.query_scores(pm, orc.MODE_ORACLE, Q, Ki, np.arange(40))
+    fin = np.isfinite(a.scores)
+    assert np.abs(c[fin] - a.scores[fin]).max() > 1e-3
+
+
+# ---------------------------------------------------------------- P2 / P8: top-k
+
+@pytest.mark.parametrize("seed", range(4))
+def test_topk_matches_stable_argsort(seed):
+    rng = np.random.default_rng(seed)
+    rows, ld, k = 17, 70, 9
+    R = rng.standard_normal((rows, ld))
+    R = np.round(R * 4) / 4                                   # many exact ties
+    nv = rng.integers(1, ld + 1, size=rows)
+    idx, cnt = orc.topk(R, nv, k)
+    for r in range(rows):
+        n = int(nv[r])
+        want = np.sort(np.argsort(-R[r, :n], kind="stable")[:k])
+        got = idx[r][idx[r] >= 0]
+        assert np.array_equal(got, want)
+        assert cnt[r] == min(k, n) == len(got)
+        assert np.all(idx[r, cnt[r]:] == -1)
+        assert np.all(np.diff(got) > 0) and (len(got) == 0 or got[-1] < n)
+
+
+def test_topk_ties_go_to_lower_index():
+    R = np.zeros((1, 10))
+    idx, cnt = orc.topk(R, [10], 4)
+    assert idx[0].tolist() == [0, 1, 2, 3]
+    R[0, [7, 2]] = 1.0
+    R[0, [5, 9, 1]] = 0.5
+    idx, _ = orc.topk(R, [10], 3)
+    assert idx[0].tolist() == [1, 2, 7]                       # 2,7 (=1.0) then the lowest of the 0.5s
+    idx, _ = orc.topk(R, [10], 3, seq_start=[100])
+    assert idx[0].tolist() == [101, 102, 107]
+
+
+def test_duplicate_keys_resolve_to_lower_index():
+    pb, Q, K, V = small_problem(L=24, Hq=4, Hkv=2, d=8, k=3)
+    K[10] = K[4]
+    K[17] = K[4]
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V, rows=[23], pos=[23])
+    P = res.scores[0]
+    assert P[4] == P[10] == P[17]
+    sel = res.idx[0].tolist()
+    if 10 in sel:
+        assert 4 in sel
+    if 17 in sel:
+        assert 4 in sel and 10 in sel
+
+
+# ---------------------------------------------------------------- P6: closed forms
+
+def test_q_zero_closed_form():
+    L, Hq, Hkv, d, k = 20, 4, 2, 8, 5
+    Q = np.zeros((L, Hq, d), np.uint16)
+    K = rand_bf16(2, (L, Hkv, d))
+    V = rand_bf16(3, (L, Hkv, d))
+    pb = orc.Problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k)
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    v = orc.bf16_to_f64(V)
+    for t in range(L):
+        assert np.allclose(res.scores[t, :t + 1], 1.0 / (t + 1), rtol=1e-15)
+        m = min(k, t + 1)
+        assert res.idx[t, :m].tolist() == list(range(m))      # all ties -> lowest indices
+        for h in range(Hq):
+            assert np.allclose(res.out[t, h], v[:m, h // 2].mean(axis=0), rtol=0, atol=1e-15)
+
+
+def test_rank_one_logits_pick_topk_of_key_scalars():
+    """d=1 effective: all q positive -> every head's softmax is increasing in the key scalar, so the
+    support is the top-k of the key scalars over the prefix."""
+    L, k = 30, 4
+    Q = gen.f32_to_bf16(np.full((L, 2, 1), 1.5, np.float32))
+    ks = np.random.default_rng(3).permutation(L).astype(np.float32) / 8
+    K = gen.f32_to_bf16(ks).reshape(L, 1, 1)
+    pb = orc.Problem(L=L, Hq=2, Hkv=1, d=1, k=k)
+    R, nv, idx, cnt = orc.select_support(pb, orc.MODE_ORACLE, Q, K, np.arange(L))
+    for t in range(L):
+        want = np.sort(np.argsort(-ks[:t + 1], kind="stable")[:k])
+        assert idx[t][idx[t] >= 0].tolist() == want.tolist()
+
+
+# ---------------------------------------------------------------- P4: sparse == dense when k >= n; O7 vs SDPA
+
+def test_sparse_equals_dense_when_budget_covers_prefix():
+    pb, Q, K, V = small_problem(L=50, Hq=4, Hkv=2, d=8, k=50, local_window=5, local_bias=0.7)
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    o_d, lse_d = orc.dense_attn(pb, Q, K, V, np.arange(50), want_lse=True)
+    assert np.allclose(res.out, o_d, rtol=0, atol=1e-14)
+    sup = np.stack([res.idx[t] for t in range(50)])
+    _, lse_s = orc.sparse_attn(pb, Q, K, V, np.arange(50), sup, want_lse=True)
+    assert np.allclose(lse_s, lse_d, rtol=0, atol=1e-13)
+
+
+def test_dense_matches_torch_sdpa():
+    import torch
+    pb, Q, K, V = small_problem(L=37, Hq=6, Hkv=2, d=16, k=4)
+    o = orc.dense_attn(pb, Q, K, V, np.arange(37))
+    q = torch.from_numpy(orc.bf16_to_f64(Q)).permute(1, 0, 2)[None]
+    k = torch.from_numpy(np.repeat(orc.bf16_to_f64(K), 3, axis=1)).permute(1, 0, 2)[None]
+    v = torch.from_numpy(np.repeat(orc.bf16_to_f64(V), 3, axis=1)).permute(1, 0, 2)[None]
+    ref = torch.nn.functional.scaled_dot_product_attention(q, k, v, is_causal=True)[0].permute(1, 0, 2).numpy()
+    assert np.allclose(o, ref, rtol=0, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P5: block rule
+
+def test_block_rule_properties():
+    pb1, Q, K, V = small_problem(L=45, Hq=4, Hkv=2, d=8, k=6, b=1)
+    pbb = orc.Problem(L=45, Hq=4, Hkv=2, d=8, k=6, b_sel=8)
+    P, _ = orc.support_scores(pb1, orc.MODE_ORACLE, Q, K, np.arange(45))
+    P2 = orc.query_scores(pb1, orc.MODE_ORACLE, Q, K, np.arange(45))
+    assert np.array_equal(P, P2)                              # b_sel=1 block rule == per-query
+    assert orc.num_rows(pbb) == 6
+    R, nv = orc.support_scores(pbb, orc.MODE_ORACLE, Q, K, np.arange(6))
+    assert nv.tolist() == [8, 16, 24, 32, 40, 45]             # last block ragged (A8)
+    for j in range(6):
+        t0, t1 = j * 8, min(44, j * 8 + 7)
+        assert np.all(np.isneginf(R[j, t1 + 1:]))
+        for t in range(t0, t1 + 1):
+            assert np.all(R[j, :t + 1] >= P[t, :t + 1])
+        want = np.max(np.where(np.isfinite(P[t0:t1 + 1]), P[t0:t1 + 1], -np.inf), axis=0)
+        assert np.array_equal(R[j, :t1 + 1], want[:t1 + 1])
+    res = orc.prefill_layer(pbb, orc.MODE_ORACLE, Q, K, V)
+    for j in range(6):
+        sel = res.idx[j][res.idx[j] >= 0]
+        assert sel.max() <= min(44, j * 8 + 7)
+
+
+# ---------------------------------------------------------------- brute force on tiny inputs (both modes)
+
+@pytest.mark.parametrize("b,lw", [(1, 0), (4, 0), (1, 3), (8, 5)])
+def test_oracle_mode_matches_numpy_bruteforce(b, lw):
+    L, Hq, Hkv, d, k = 37, 4, 2, 8, 5
+    pb, Q, K, V = small_problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b=b, seed=11 + b,
+                                local_window=lw, local_bias=0.9 if lw else 0.0)
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    kw = dict(local_window=lw, local_bias=0.9 if lw else 0.0)
+    P = bf.mass(Q, K, 1 / math.sqrt(d), Hq // Hkv, **kw)
+    R, nv = bf.support_rows(P, b)
+    assert np.array_equal(nv, res.n_valid)
+    fin = np.isfinite(res.scores)
+    assert np.array_equal(fin, np.isfinite(R))
+    assert np.allclose(res.scores[fin], R[fin], rtol=1e-12, atol=0)
+    idx = bf.topk_rows(R, nv, k)
+    assert np.array_equal(idx, res.idx)
+    o = bf.sparse_attention(Q, K, V, 1 / math.sqrt(d), Hq // Hkv, idx, b, **kw)
+    assert np.allclose(res.out, o, rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("b,lw", [(1, 0), (4, 2)])
+def test_indexer_mode_matches_numpy_bruteforce(b, lw):
+    L, Hq, Hkv, d, k, hid, di = 33, 4, 2, 8, 6, 24, 8
+    pb, Q, K, V = small_problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b=b, seed=21, hidden=hid, d_idx=di,
+                                local_window=lw, local_bias=-0.6 if lw else 0.0)
+    X = rand_bf16(31, (L, hid))
+    Wq = rand_bf16(32, (hid, di), 1 / math.sqrt(hid))
+    Wk = rand_bf16(33, (hid, di), 1 / math.sqrt(hid))
+    res = orc.prefill_layer(pb, orc.MODE_INDEXER, Q, K, V, X, Wq, Wk)
+    # projection: fp64 matmul (library) then one RNE rounding; compare as values, allow a tie-flip nowhere
+    pq = orc.bf16_to_f64(X) @ orc.bf16_to_f64(Wq)
+    got = orc.bf16_to_f64(res.q_idx)
+    assert np.all(np.abs(got - pq) <= np.abs(pq) * 2.0 ** -8 + 1e-300)       # within half an ulp (8 sig. bits)
+    import torch
+    tq = torch.from_numpy(pq).to(torch.bfloat16).to(torch.float64).numpy()
+    assert (tq != got).mean() < 1e-3                                          # library cast agrees (bar double rounding)
+    kw = dict(local_window=lw, local_bias=-0.6 if lw else 0.0)
+    z = bf.indexer_logits(res.q_idx, res.k_idx, 1 / math.sqrt(di), **kw)
+    R, nv = bf.support_rows(z, b)
+    fin = np.isfinite(R)
+    assert np.array_equal(fin, np.isfinite(res.scores))
+    assert np.allclose(res.scores[fin], R[fin], rtol=1e-12, atol=1e-13)
+    idx = bf.topk_rows(R, nv, k)
+    assert np.array_equal(idx, res.idx)
+    o = bf.sparse_attention(Q, K, V, 1 / math.sqrt(d), Hq // Hkv, idx, b, **kw)
+    assert np.allclose(res.out, o, rtol=0, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P9: varlen
+
+@pytest.mark.parametrize("mode", [orc.MODE_ORACLE, orc.MODE_INDEXER])
+def test_varlen_pack_equals_separate_sequences(mode):
+    lens = [19, 8, 30, 5]
+    cu = np.concatenate([[0], np.cumsum(lens)])
+    L, Hq, Hkv, d, k, b, hid, di = int(cu[-1]), 4, 2, 8, 6, 8, 16, 8
+    Q, K, V = rand_bf16(1, (L, Hq, d)), rand_bf16(2, (L, Hkv, d)), rand_bf16(3, (L, Hkv, d))
+    X = rand_bf16(4, (L, hid))
+    Wq, Wk = rand_bf16(5, (hid, di), 0.25), rand_bf16(6, (hid, di), 0.25)
+    kw = dict(Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=b, hidden=hid, d_idx=di, local_window=3, local_bias=0.5)
+    pk = orc.Problem(L=L, cu_seqlens=cu, **kw)
+    packed = orc.prefill_layer(pk, mode, Q, K, V, X, Wq, Wk)
+    assert orc.num_rows(pk) == sum((n + b - 1) // b for n in lens) == len(packed.idx)
+    r0 = 0
+    for i, n in enumerate(lens):
+        s, e = int(cu[i]), int(cu[i + 1])
+        one = orc.prefill_layer(orc.Problem(L=n, **kw), mode, Q[s:e], K[s:e], V[s:e], X[s:e], Wq, Wk)
+        nr = len(one.idx)
+        shifted = np.where(one.idx >= 0, one.idx + s, -1)
+        assert np.array_equal(packed.idx[r0:r0 + nr], shifted)
+        assert np.array_equal(packed.cnt[r0:r0 + nr], one.cnt)
+        assert np.allclose(packed.out[s:e], one.out, rtol=0, atol=1e-15)
+        r0 += nr
+
+
+def test_empty_effective_support_gives_zero_output():
+    """k < b_sel: the first queries of a block may see none of the block's support (A9)."""
+    pb, Q, K, V = small_problem(L=16, Hq=2, Hkv=1, d=4, k=1, b=8)
+    res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    for t in range(16):
+        s = res.idx[t // 8, 0]
+        if s > t:
+            assert np.all(res.out[t] == 0.0)
+    sup = np.full((1, 1), 9, np.int32)
+    o, lse = orc.sparse_attn(pb, Q, K, V, [3], sup, want_lse=True)
+    assert np.all(o == 0) and np.all(np.isneginf(lse))

@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- sparse-prefill layer throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+A "step" is one pass of the whole hot path (sp_prefill_layer: projection -> scoring (+block max) ->
+causal top-k -> gather-sparse GQA attention) over one batch of synthetic input of BASELINE.json's
+config 3 (L=32768, Hq=32, Hkv=8, d=128, d_idx=128, k=2048, b_sel=64) -- the 32K / k=2048 configuration
+the metric is quoted on (`--workload c5` runs the 128K one).  `value` = tokens/s with inputs resident
+in HBM; `e2e` = the same through sp_prefill_layer_host with pinned HOST buffers (copies inside the
+timed region).  The dense GQA layer of the same library is timed in the same run.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c2|c1] [--impl reference]
+
+N > 1 (torchrun): the path does not shard (one GPU per layer call, no collectives) -> N independent
+replicas, value = N * L / max-over-ranks time ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "sparse_prefill_layer_tokens_per_s"
+UNIT = "tokens/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm=p["hbm_gbs"], tensor_burst=p["bf16_tflops"], tensor=p.get("bf16_tflops_sustained", p["bf16_tflops"]),
+                    source="measured")
+    return dict(hbm=6650.0, tensor_burst=1590.0, tensor=1400.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        super().__init__(daemon=True)
+        self.gpu = gpu_index
+        self.samples = []
+        self._stop = threading.Event()
+
+    def run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.gpu)], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                if len(f) >= 7:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def stop(self):
+        self._stop.set()
+        self.join(timeout=6)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[3 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm), "power_w_max": max(float(s[2]) for s in self.samples)}
+
+
+def kept_pairs(L, k):
+    k = min(k, L)
+    return k * L - k * (k - 1) // 2
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------------
+
+def oracle_sample_rate(cfg, inp, budget_rows=None):
+    """Times the oracle, as it stands, on a bounded sample of the workload; returns tokens/s and a
+    description.  Indexer mode: full k_idx projection (shared by every row, amortised over L tokens) +
+    `rows` support rows done completely (q projection, scores, block max, top-k, sparse attention)."""
+    import numpy as np
+    from oracle import oracle as orc
+    pbo = orc.Problem(L=cfg.L, Hq=cfg.Hq, Hkv=cfg.Hkv, d=cfg.d, k=cfg.k, b_sel=cfg.b_sel, hidden=cfg.hidden,
+                      d_idx=cfg.d_idx, local_window=cfg.local_window, local_bias=cfg.local_bias,
+                      cu_seqlens=cfg.cu_seqlens)
+    n_rows = orc.num_rows(pbo)
+    nsel = budget_rows or (8 if cfg.b_sel > 1 else 256)
+    rows = np.unique(np.linspace(0, n_rows - 1, nsel).astype(np.int64))
+    pos = []
+    for r in rows:
+        s0, t0, t1 = orc.row_info(pbo, int(r))
+        pos.extend(range(s0 + t0, s0 + t1 + 1))
+    pos = np.array(pos)
+    t_shared = 0.0
+    kw = {}
+    t0 = time.perf_counter()
+    if cfg.mode != "oracle":
+        ki = orc.project(pbo, inp["X"], inp["Wki"])
+        t_shared = time.perf_counter() - t0
+        t1 = time.perf_counter()
+        qi = np.zeros((cfg.L, cfg.d_idx), np.uint16)
+        qi[pos] = orc.project(pbo, inp["X"], inp["Wqi"], rows=pos)
+        kw = dict(q_idx=qi, k_idx=ki)
+        mode = orc.MODE_INDEXER
+    else:
+        t1 = time.perf_counter()
+        mode = orc.MODE_ORACLE
+    orc.prefill_layer(pbo, mode, inp["Q"], inp["K"], inp["V"], rows=rows, pos=pos, **kw)
+    t_rows = time.perf_counter() - t1
+    per_token = t_shared / cfg.L + t_rows / len(pos)
+    return dict(value=1.0 / per_token, unit=UNIT, cores=orc.max_threads(), kind="oracle",
+                sample=(f"{len(rows)} of {n_rows} support rows ({len(pos)} queries, evenly spaced) done completely in "
+                        f"{t_rows:.1f} s + the shared k_idx projection of all {cfg.L} tokens in {t_shared:.1f} s "
+                        f"amortised over L; extrapolated per token"),
+                seconds=t_shared + t_rows)
+
+
+def run_reference(args, cfg):
+    """--impl reference: the fp64 CPU oracle on the host cores, same config / metric / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2606_07703_b200 import inputs as gen
+    inp = gen.make_inputs(cfg)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample_rate(cfg, inp, budget_rows=1)
+    vals, secs = [], 0.0
+    last = None
+    for _ in range(args.steps):
+        last = oracle_sample_rate(cfg, inp, budget_rows=2 if cfg.b_sel > 1 else 64)
+        vals.append(last["value"])
+        secs += last["seconds"]
+    v = len(vals) / sum(1.0 / x for x in vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * cfg.L / v, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg),
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(cfg):
+    return {"workload": f"BASELINE.json configs[{cfg.cfg_id - 1}] ({cfg.name}): one causal GQA layer, {cfg.mode} mode",
+            "L": cfg.L, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "d": cfg.d, "k": cfg.k, "b_sel": cfg.b_sel,
+            "hidden": cfg.hidden, "d_idx": cfg.d_idx, "local_window": cfg.local_window, "batch": 1,
+            "parallelism": "replicas only (no sharding, no collectives)",
+            "l2": "no flush: per-step inputs (X+Q+K+V) exceed the 126 MB L2" }
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU leg
+# ------------------------------------------------------------------------------------------------
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c3")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+
+    from paper_2606_07703_b200 import inputs as gen
+    cfg = gen.ALL[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import numpy as np
+    import torch
+    from paper_2606_07703_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    B.lib()
+    peaks = load_peaks()
+    indexer = cfg.mode != "oracle"
+    gmode = B.SP_MODE_INDEXER if indexer else B.SP_MODE_ORACLE
+    stage = B.SP_STAGE_LAYER_INDEXER if indexer else B.SP_STAGE_LAYER_ORACLE
+
+    inp = gen.make_inputs(cfg)
+    names = ("X", "Wqi", "Wki", "Q", "K", "V") if indexer else ("Q", "K", "V")
+    host = {n: B.bf16_tensor(inp[n], "cpu").pin_memory() for n in names}
+    devt = {n: host[n].cuda(non_blocking=True) for n in names}
+    pb = B.Problem.from_config(cfg)
+    n_rows = pb.num_rows
+    O = torch.empty(cfg.L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+    O_dense = torch.empty_like(O)
+    idx = torch.empty(n_rows, cfg.k, dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(pb, stage)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.sp_prefill_layer(pb, gmode, devt.get("X"), devt.get("Wqi"), devt.get("Wki"), devt["Q"], devt["K"], devt["V"],
+                           O, idx, ws)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    launches = B.launch_count() - l0
+    ms_total = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * cfg.L / (ms_step * 1e-3)
+
+    # ---- dense GQA layer of the same library, same tensors, same run ----
+    def time_call(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    dense_reps = max(1, min(args.steps, 3))
+    dense_ms = time_call(lambda: B.sp_dense_gqa_attn(pb, devt["Q"], devt["K"], devt["V"], O_dense, None), dense_reps)
+
+    # ---- per-stage split through the staged C-ABI calls (same stream, CUDA events) ----
+    reps = max(1, min(args.steps, 5))
+    ld = (pb.max_seqlen + 3) // 4 * 4
+    panel = min(n_rows, max(1, (1 << 30) // (ld * 4)))
+    scores = torch.empty(panel, ld, dtype=torch.float32, device="cuda")
+    stages = {}
+    if indexer:
+        q_idx = torch.empty(cfg.L, cfg.d_idx, dtype=torch.bfloat16, device="cuda")
+        k_idx = torch.empty_like(q_idx)
+        ws_i = B.alloc_workspace(pb, B.SP_STAGE_INDEXER_SCORES)
+        t_both = time_call(lambda: B.sp_indexer_scores(pb, devt["X"], devt["Wqi"], devt["Wki"], q_idx, k_idx, False,
+                                                       0, panel, scores, ws_i), reps)
+        t_sc = time_call(lambda: B.sp_indexer_scores(pb, None, None, None, q_idx, k_idx, True, 0, panel, scores), reps)
+        stages["projection"] = max(t_both - t_sc, 0.0)
+        stages["scoring"] = t_sc * (n_rows / panel)
+    else:
+        lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device="cuda")
+        t_both = time_call(lambda: B.sp_oracle_mass(pb, devt["Q"], devt["K"], lse, False, 0, panel, scores), reps)
+        t_p2 = time_call(lambda: B.sp_oracle_mass(pb, devt["Q"], devt["K"], lse, True, 0, panel, scores), reps)
+        stages["mass_pass1_lse"] = max(t_both - t_p2, 0.0)
+        stages["mass_pass2"] = t_p2 * (n_rows / panel)
+    idx_p = torch.empty(panel, cfg.k, dtype=torch.int32, device="cuda")
+    stages["topk"] = time_call(lambda: B.sp_topk_support(pb, scores, 0, panel, idx_p), reps) * (n_rows / panel)
+    stages["sparse_attention"] = time_call(lambda: B.sp_sparse_gqa_attn(pb, devt["Q"], devt["K"], devt["V"], idx, O), reps)
+
+    # ---- algorithmic work ----
+    L, k, d, Hq, Hkv = cfg.L, cfg.k, cfg.d, cfg.Hq, cfg.Hkv
+    causal = L * (L + 1) // 2
+    # exact useful (query, key) pairs of the sparse attention: support entries with 0 <= s <= t
+    b = max(1, cfg.b_sel)
+    big = torch.where(idx >= 0, idx, torch.full_like(idx, 2 ** 30))
+    if cfg.cu_seqlens is None:
+        T = torch.arange(n_rows * b, device="cuda", dtype=torch.int32).view(n_rows, b)
+        cnt = torch.searchsorted(big, T.clamp(max=L - 1).contiguous(), right=True)
+        pairs = int((cnt * (T < L)).sum().item())
+    else:
+        pairs = kept_pairs(L, k)  # upper bound for packs; not used for a headline number
+    work = {
+        "projection": ("tensor", 4.0 * L * cfg.hidden * cfg.d_idx),
+        "scoring": ("tensor" if cfg.b_sel > 1 else "hbm", 2.0 * cfg.d_idx * causal if cfg.b_sel > 1 else 4.0 * causal),
+        "mass_pass1_lse": ("tensor", 2.0 * d * Hq * causal),
+        "mass_pass2": ("tensor", 2.0 * d * Hq * causal),
+        "topk": ("hbm", 4.0 * (causal / b if cfg.b_sel == 1 else sum(min(L, (j + 1) * b) for j in range(n_rows))) + 4.0 * n_rows * k),
+        "sparse_attention": ("tensor", 4.0 * d * Hq * pairs) if cfg.b_sel > 1 else ("hbm", 4.0 * Hkv * d * pairs),
+    }
+    dom = max(stages, key=lambda s: stages[s])
+    bound, amount = work[dom]
+    if bound == "tensor":
+        ach = amount / (stages[dom] * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor"], "unit": "TFLOP/s", "frac": ach / peaks["tensor"],
+                "frac_of_burst_peak": ach / peaks["tensor_burst"], "traffic": None}
+    else:
+        ach = amount / (stages[dom] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"], "traffic": None}
+    roof.update({"kernel": dom, "kernel_ms": stages[dom], "peak_source": peaks["source"],
+                 "algorithmic_units": amount})
+    stage_rates = {}
+    for s, ms in stages.items():
+        bd, amt = work[s]
+        if ms > 0:
+            stage_rates[s] = {"ms": ms, "bound": bd,
+                              "rate": amt / (ms * 1e-3) / (1e12 if bd == "tensor" else 1e9),
+                              "unit": "TFLOP/s" if bd == "tensor" else "GB/s",
+                              "frac": amt / (ms * 1e-3) / ((peaks["tensor"] * 1e12) if bd == "tensor" else (peaks["hbm"] * 1e9))}
+
+    # ---- end to end through the C ABI with HOST buffers ----
+    arena = torch.empty(B.layer_host_arena_bytes(pb, gmode), dtype=torch.uint8, device="cuda")
+    O_host = torch.empty(cfg.L, cfg.Hq, cfg.d, dtype=torch.bfloat16).pin_memory()
+
+    def e2e_step():
+        B.sp_prefill_layer_host(pb, gmode, host.get("X"), host.get("Wqi"), host.get("Wki"), host["Q"], host["K"],
+                                host["V"], O_host, arena)
+
+    e2e_reps = max(1, min(args.steps, 5))
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    a, bb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(e2e_reps):
+        e2e_step()
+    bb.record(stream)
+    barrier()
+    e2e_ms = a.elapsed_time(bb) / e2e_reps
+    if dist is not None:
+        t = torch.tensor([e2e_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    sampler.stop()
+    h2d = sum(host[n].numel() * 2 for n in names)
+    d2h = O_host.numel() * 2
+    # the host path must agree with the device path
+    same = bool(torch.equal(O_host.cuda(), O))
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "config": workload_config(cfg),
+        "clocks": sampler.summary(),
+        "e2e": {"value": world * cfg.L / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "matches_device_path": same},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "stages": stage_rates,
+        "dense_layer": {"ms": dense_ms, "tflops": 4.0 * d * Hq * causal / (dense_ms * 1e-3) / 1e12,
+                        "speedup_sparse_vs_dense": dense_ms / ms_step},
+        "paper_context": "TTFT ratios in the paper (whole model, other hardware): 1.93x Qwen3.5-9B GPU-80G vs FA2 @256K; "
+                         "1.71x Qwen3.5-0.8B NPU-64G vs vLLM-Ascend FA @256K (PAPER.md:434-440); not comparable to a layer",
+    }
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        cb = oracle_sample_rate(cfg, inp)
+        cb.pop("seconds", None)
+        line["cpu_baseline"] = cb
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

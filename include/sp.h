@@ -1,0 +1,163 @@
+/*
+ * sp.h -- C ABI of the B200 (sm_100a) sparse-prefill library: one causal GQA layer of
+ * "oracle-guided sparse prefill" (arxiv/paper_2606_07703; citations are /root/reference/PAPER.md lines).
+ *
+ *   score -> causal top-k -> (optional) query-block-shared support -> gather-sparse GQA attention
+ *
+ * Conventions that hold for EVERY entry point
+ *  - Pointers are DEVICE pointers unless the comment says HOST.  The caller owns every buffer, the
+ *    workspace and the stream.  The library allocates no device memory, never synchronises the device
+ *    and enqueues all work on `stream` (a cudaStream_t passed as void*).  Inputs are read-only.
+ *  - sp_params is read on the host at call time.
+ *  - Layouts (row-major, base pointers 16-byte aligned, bf16 = IEEE bfloat16 bit patterns):
+ *      Q [L,Hq,d]   K,V [L,Hkv,d]   O [L,Hq,d]   X [L,hidden]   Wqi,Wki [hidden,d_idx]
+ *      q_idx,k_idx [L,d_idx]   lse [L,Hq] fp32 (natural log)
+ *    Query head h reads KV head g(h) = h / (Hq/Hkv)  (contiguous groups).
+ *  - Positions are 0-based; query t may attend keys s <= t of ITS OWN sequence.
+ *    With cu_seqlens the L tokens are a pack of `batch` sequences; every s, t, block and n_valid below is
+ *    local to its sequence, while emitted indices are PACKED positions (local + cu_seqlens[i]).
+ *  - Support rows: per sequence of length n, b_sel==1 gives n rows (row = query);
+ *    b_sel>1 gives ceil(n/b_sel) rows, block j = local positions [j*b_sel, min((j+1)*b_sel, n)) (blocks
+ *    never straddle sequences; the last may be ragged).  Rows of all sequences are concatenated in order.
+ *    n_valid(row) = last local position of the row + 1.
+ *  - Score matrices (`scores`, `mass`) are fp32, one row per support row of the requested panel
+ *    [row_begin, row_begin+row_count), leading dimension ld >= max n_valid of the panel, column = key
+ *    position local to the row's sequence.  Columns >= n_valid(row) are NOT written and never read.
+ *  - Optional banded logit term (reading A20): when local_window > 0, local_bias is added to the
+ *    scaled logit wherever 0 <= t-s < local_window, in every stage that forms a causal logit.
+ *  - Return value: SP_OK (0) or a negative sp_status.  On any error nothing has been launched.  No
+ *    exceptions cross this ABI and nothing aborts.  There is no CPU fallback.
+ */
+#ifndef SP_H_
+#define SP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum sp_status {
+  SP_OK = 0,
+  SP_ERR_INVALID_ARG = -1, /* null / misaligned pointer, nonpositive size, Hq % Hkv, bad cu_seqlens, bad panel */
+  SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}, Hq/Hkv not in {1,2,4,8}, flags != 0 ...) */
+  SP_ERR_WORKSPACE = -3,   /* workspace too small (see sp_workspace_bytes)                                      */
+  SP_ERR_CUDA = -4         /* a CUDA launch / API error; text via sp_strerror                                   */
+} sp_status;
+
+typedef enum sp_mode {
+  SP_MODE_ORACLE = 0, /* support from dense attention mass  (Alg.1)  */
+  SP_MODE_INDEXER = 1 /* support from the head-collapsed indexer (Alg.2) */
+} sp_mode;
+
+typedef enum sp_stage {
+  SP_STAGE_INDEXER_SCORES = 0,
+  SP_STAGE_ORACLE_MASS = 1,
+  SP_STAGE_TOPK = 2,
+  SP_STAGE_SPARSE_ATTN = 3,
+  SP_STAGE_DENSE_ATTN = 4,
+  SP_STAGE_LAYER_ORACLE = 5,
+  SP_STAGE_LAYER_INDEXER = 6
+} sp_stage;
+
+/* The paper's problem statement for one layer call (PAPER.md:90-107 S,Hq,Hkv,g,d_h,k; :101-103,:178 b_sel;
+ * :270-274 d_idx). */
+typedef struct sp_params {
+  int32_t batch;                  /* sequences in the pack; 1 when cu_seqlens == NULL                     */
+  int32_t L;                      /* total packed tokens, >= 1                                            */
+  const int32_t *cu_seqlens;      /* DEVICE ptr [batch+1], cu[0]=0, cu[batch]=L; NULL = one sequence      */
+  const int32_t *cu_seqlens_host; /* HOST copy of the same array (needed iff cu_seqlens != NULL)          */
+  int32_t Hq, Hkv, d;             /* Hq % Hkv == 0, Hq/Hkv in {1,2,4,8}; d in {64,128}                    */
+  int32_t k;                      /* budget per support row, >= 1 */
+  int32_t b_sel;                  /* 1 = per-query support; >1 = one support per b_sel queries            */
+  int32_t hidden, d_idx;          /* indexer sizes; d_idx in {64,128}, hidden % 64 == 0 (indexer mode)    */
+  float scale;                    /* attention scale; 0 -> 1/sqrt(d) */
+  float idx_scale;                /* indexer scale;   0 -> 1/sqrt(d_idx) */
+  int32_t local_window;           /* 0 = off                                                              */
+  float local_bias;               /* added to the scaled logit when 0 <= t-s < local_window               */
+  uint32_t flags;                 /* reserved (ReLU / key LayerNorm / RoPE of PAPER.md:270-274): must be 0 */
+} sp_params;
+
+/* Number of support rows of the whole pack (host arithmetic only). Returns < 0 on invalid params. */
+int64_t sp_num_rows(const sp_params *p);
+
+/* Bytes of workspace `stage` (an sp_stage) needs for these params; written to *bytes_out.
+ * For the two LAYER stages the figure includes the score panel and the index buffer. */
+int sp_workspace_bytes(const sp_params *p, int stage, size_t *bytes_out);
+
+/* Indexer support-row scores (PAPER.md:270 projections, :274 scaled similarity without LN/RoPE/ReLU,
+ * :299 max-aggregate over each b_sel block; Alg.2 steps 2 and 4).
+ *   preprojected == 0: q_idx = bf16(X Wqi), k_idx = bf16(X Wki) are computed for ALL L tokens (fp32
+ *     accumulate, one round-to-nearest-even to bf16) and written to q_idx / k_idx (outputs, [L,d_idx]).
+ *   preprojected != 0: X, Wqi, Wki are ignored (may be NULL); q_idx / k_idx are inputs.
+ *   scores[r - row_begin, s] = max over queries t of support row r with s <= t of
+ *       idx_scale * <q_idx[t], k_idx[s]> (+ local term),  s in [0, n_valid(r)).       fp32, never rounded to bf16. */
+int sp_indexer_scores(const sp_params *p, const void *X, const void *Wqi, const void *Wki,
+                      void *q_idx, void *k_idx, int32_t preprojected,
+                      int32_t row_begin, int32_t row_count, float *scores, int64_t ld_scores,
+                      void *ws, size_t ws_bytes, void *stream);
+
+/* Attention-mass support-row scores (PAPER.md:123 P_t(s) = (1/Hq) sum_h A[t,h,s]; :154 block max; Alg.1
+ * steps 2-3).  Pass 1 computes the per-(t,h) softmax normaliser as a log-sum-exp over s <= t; pass 2
+ * rebuilds the probabilities and averages them over ALL Hq query heads.
+ *   lse: [L,Hq] fp32.  lse_ready == 0: pass 1 runs for every query of the panel and writes lse (output;
+ *        may be NULL, then it lives in the workspace).  lse_ready != 0: lse is an input (e.g. from
+ *        sp_dense_gqa_attn) and pass 1 is skipped.
+ *   mass[r - row_begin, s] = max over queries t of row r with s <= t of P_t(s),  s in [0, n_valid(r)). */
+int sp_oracle_mass(const sp_params *p, const void *Q, const void *K, float *lse, int32_t lse_ready,
+                   int32_t row_begin, int32_t row_count, float *mass, int64_t ld_mass,
+                   void *ws, size_t ws_bytes, void *stream);
+
+/* Causal top-k of each support row of the panel (PAPER.md:127 TopK_s(P,k); :145 sentinel padding; :156
+ * causally invalid positions masked before selection).  Row r ranks columns [0, n_valid(r)) of
+ * scores[r - row_begin, :]; the kept set is the first min(k, n_valid) elements of the order
+ * (score descending, index ascending) -- ties go to the lower index.
+ *   idx: [row_count, k] int32 packed positions, ascending, tail padded with -1.
+ *   cnt: [row_count] int32 = min(k, n_valid(r)); may be NULL. */
+int sp_topk_support(const sp_params *p, const float *scores, int64_t ld_scores,
+                    int32_t row_begin, int32_t row_count, int32_t *idx, int32_t *cnt,
+                    void *ws, size_t ws_bytes, void *stream);
+
+/* GQA attention recomputed only over the selected KV positions, online softmax (PAPER.md:107; :156 each
+ * query re-applies its own causal mask; Alg.1 step 5).
+ *   idx: [sp_num_rows(p), k] as produced by sp_topk_support for the WHOLE pack (row of query t =
+ *        its support row).  Entries < 0 or > t (or outside t's sequence) are ignored for query t.
+ *   O: [L,Hq,d] bf16 (fp32 accumulate).  Empty effective support -> O row = 0, lse = -inf.
+ *   lse: [L,Hq] fp32 or NULL. */
+int sp_sparse_gqa_attn(const sp_params *p, const void *Q, const void *K, const void *V,
+                       const int32_t *idx, void *O, float *lse, void *ws, size_t ws_bytes, void *stream);
+
+/* Dense causal GQA attention of the same layer: the same-library baseline and pass 1 of
+ * the attention mass.  O may be NULL (only lse is produced); lse may be NULL. */
+int sp_dense_gqa_attn(const sp_params *p, const void *Q, const void *K, const void *V, void *O, float *lse,
+                      void *ws, size_t ws_bytes, void *stream);
+
+/* One patched layer on one stream (PAPER.md:292 five-stage path without the paged-cache stage; Alg.1 steps
+ * 2-5 in SP_MODE_ORACLE, Alg.2 steps 2,4,5 in SP_MODE_INDEXER).  Support rows are processed in panels so the
+ * score workspace stays bounded.
+ *   X, Wqi, Wki: indexer mode only (ignored in oracle mode).  O: [L,Hq,d] bf16.
+ *   idx_out: [sp_num_rows(p), k] int32 or NULL (then the indices live in the workspace). */
+int sp_prefill_layer(const sp_params *p, int32_t mode, const void *X, const void *Wqi, const void *Wki,
+                     const void *Q, const void *K, const void *V, void *O, int32_t *idx_out,
+                     void *ws, size_t ws_bytes, void *stream);
+
+/* Same as sp_prefill_layer but X, Wqi, Wki, Q, K, V and O are HOST pointers (pinned memory recommended).
+ * `dev_arena` is DEVICE scratch of at least sp_layer_host_arena_bytes() bytes that receives the inputs, the
+ * output and the workspace.  Copies are enqueued on `stream` (cudaMemcpyAsync); O_host is valid once the
+ * stream has been synchronised by the caller. */
+int sp_layer_host_arena_bytes(const sp_params *p, int32_t mode, size_t *bytes_out);
+int sp_prefill_layer_host(const sp_params *p, int32_t mode, const void *X_host, const void *Wqi_host,
+                          const void *Wki_host, const void *Q_host, const void *K_host, const void *V_host,
+                          void *O_host, void *dev_arena, size_t arena_bytes, void *stream);
+
+/* Text for a status code; for SP_ERR_CUDA it includes the last CUDA error string seen by this library. */
+const char *sp_strerror(int code);
+
+/* Number of kernel launches this library has enqueued since load (for bench.py's gpu_launches). */
+int64_t sp_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SP_H_ */

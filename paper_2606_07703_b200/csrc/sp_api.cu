@@ -1,0 +1,395 @@
+// sp_api.cu -- the C ABI declared in include/sp.h: argument validation, workspace carving, panel
+// loops and stage chaining.  No device memory is allocated here and the device is never synchronised.
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "sp_common.cuh"
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+std::mutex g_err_mu;
+char g_err_text[512] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* where) {
+  std::lock_guard<std::mutex> lk(g_err_mu);
+  snprintf(g_err_text, sizeof(g_err_text), "SP_ERR_CUDA: %s: %s (%s)", where, cudaGetErrorName(e),
+           cudaGetErrorString(e));
+  return SP_ERR_CUDA;
+}
+#define SP_CUDA(call, where)                         \
+  do {                                               \
+    cudaError_t e__ = (call);                        \
+    if (e__ != cudaSuccess) return cuda_fail(e__, where); \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct HostGeom {
+  int batch, L, b;
+  const int32_t* cu;  // host or nullptr
+  int seq_start(int i) const { return cu ? cu[i] : 0; }
+  int seq_len(int i) const { return cu ? cu[i + 1] - cu[i] : L; }
+  int rows_of(int n) const { return (n + b - 1) / b; }
+  long long num_rows() const {
+    long long r = 0;
+    for (int i = 0; i < batch; ++i) r += rows_of(seq_len(i));
+    return r;
+  }
+  int max_seqlen() const {
+    int m = 0;
+    for (int i = 0; i < batch; ++i) m = seq_len(i) > m ? seq_len(i) : m;
+    return m;
+  }
+  // max n_valid over support rows [row_begin, row_begin + row_count)
+  int max_n_valid(long long row_begin, long long row_count) const {
+    long long r0 = 0;
+    int best = 0;
+    for (int i = 0; i < batch; ++i) {
+      const int n = seq_len(i);
+      const long long nr = rows_of(n);
+      const long long lo = row_begin > r0 ? row_begin : r0;
+      const long long hi = (row_begin + row_count < r0 + nr ? row_begin + row_count : r0 + nr) - 1;
+      if (lo <= hi) {
+        const long long j = hi - r0;  // last intersecting row of this sequence
+        const long long nv = (j + 1) * b < n ? (j + 1) * b : n;
+        if (nv > best) best = (int)nv;
+      }
+      r0 += nr;
+    }
+    return best;
+  }
+};
+
+int validate_common(const sp_params* p, bool need_attn, bool need_indexer) {
+  if (!p) return SP_ERR_INVALID_ARG;
+  if (p->L < 1 || p->batch < 1 || p->k < 1 || p->b_sel < 1) return SP_ERR_INVALID_ARG;
+  if (p->cu_seqlens) {
+    if (!p->cu_seqlens_host) return SP_ERR_INVALID_ARG;
+    const int32_t* cu = p->cu_seqlens_host;
+    if (cu[0] != 0 || cu[p->batch] != p->L) return SP_ERR_INVALID_ARG;
+    for (int i = 0; i < p->batch; ++i)
+      if (cu[i + 1] <= cu[i]) return SP_ERR_INVALID_ARG;
+  } else if (p->batch != 1) {
+    return SP_ERR_INVALID_ARG;
+  }
+  if (p->flags != 0) return SP_ERR_UNSUPPORTED;
+  if (p->local_window < 0) return SP_ERR_INVALID_ARG;
+  if (need_attn) {
+    if (p->Hq < 1 || p->Hkv < 1 || p->d < 1 || p->Hq % p->Hkv != 0) return SP_ERR_INVALID_ARG;
+    const int G = p->Hq / p->Hkv;
+    if (!(p->d == 64 || p->d == 128)) return SP_ERR_UNSUPPORTED;
+    if (!(G == 1 || G == 2 || G == 4 || G == 8)) return SP_ERR_UNSUPPORTED;
+  }
+  if (need_indexer) {
+    if (p->hidden < 1 || p->d_idx < 1) return SP_ERR_INVALID_ARG;
+    if (!(p->d_idx == 64 || p->d_idx == 128) || p->hidden % 64 != 0) return SP_ERR_UNSUPPORTED;
+  }
+  return SP_OK;
+}
+
+HostGeom host_geom(const sp_params* p) {
+  return HostGeom{p->batch, p->L, p->b_sel, p->cu_seqlens ? p->cu_seqlens_host : nullptr};
+}
+SpGeom dev_geom(const sp_params* p) { return SpGeom{p->batch, p->L, p->cu_seqlens, p->b_sel}; }
+float attn_scale(const sp_params* p) { return p->scale != 0.f ? p->scale : 1.0f / sqrtf((float)p->d); }
+float index_scale(const sp_params* p) { return p->idx_scale != 0.f ? p->idx_scale : 1.0f / sqrtf((float)p->d_idx); }
+
+int validate_panel(const sp_params* p, int32_t row_begin, int32_t row_count, int64_t ld, int* max_nv) {
+  const HostGeom hg = host_geom(p);
+  const long long nr = hg.num_rows();
+  if (row_begin < 0 || row_count < 0 || (long long)row_begin + row_count > nr) return SP_ERR_INVALID_ARG;
+  *max_nv = hg.max_n_valid(row_begin, row_count);
+  if (ld < *max_nv) return SP_ERR_INVALID_ARG;
+  return SP_OK;
+}
+
+// ---- workspace sizes ----
+size_t ws_indexer(const sp_params* p) { return align_up((size_t)2 * p->hidden * p->d_idx * 2); }
+size_t ws_mass(const sp_params* p) { return align_up((size_t)p->L * p->Hq * sizeof(float)); }
+
+constexpr size_t PANEL_BYTES = (size_t)1 << 30;  // score panel budget inside sp_prefill_layer
+
+struct LayerPlan {
+  int64_t ld;
+  long long n_rows, panel_rows;
+  size_t off_qidx, off_kidx, off_lse, off_scores, off_idx, off_stage, total;
+};
+
+LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws) {
+  LayerPlan pl{};
+  const HostGeom hg = host_geom(p);
+  pl.n_rows = hg.num_rows();
+  pl.ld = (int64_t)align_up((size_t)hg.max_seqlen(), 4);
+  long long pr = (long long)(PANEL_BYTES / ((size_t)pl.ld * sizeof(float)));
+  if (pr < 1) pr = 1;
+  if (p->b_sel == 1 && pr >= 64) pr = pr / 64 * 64;
+  if (pr > pl.n_rows) pr = pl.n_rows;
+  pl.panel_rows = pr;
+  size_t off = 0;
+  if (mode == SP_MODE_INDEXER) {
+    pl.off_qidx = off; off += align_up((size_t)p->L * p->d_idx * 2);
+    pl.off_kidx = off; off += align_up((size_t)p->L * p->d_idx * 2);
+    pl.off_stage = off; off += ws_indexer(p);
+  } else {
+    pl.off_lse = off; off += ws_mass(p);
+  }
+  pl.off_scores = off; off += align_up((size_t)pl.panel_rows * pl.ld * sizeof(float));
+  pl.off_idx = off;
+  if (idx_in_ws) off += align_up((size_t)pl.n_rows * p->k * sizeof(int32_t));
+  pl.total = off;
+  return pl;
+}
+
+}  // namespace
+
+void sp_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+extern "C" {
+
+int64_t sp_launch_count(void) { return g_launches.load(); }
+
+const char* sp_strerror(int code) {
+  switch (code) {
+    case SP_OK: return "SP_OK";
+    case SP_ERR_INVALID_ARG: return "SP_ERR_INVALID_ARG: null/misaligned pointer, bad size, bad cu_seqlens or bad panel";
+    case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED: shape outside the built set (d in {64,128}, Hq/Hkv in {1,2,4,8}, d_idx in {64,128}, hidden % 64 == 0, flags == 0)";
+    case SP_ERR_WORKSPACE: return "SP_ERR_WORKSPACE: workspace too small, see sp_workspace_bytes";
+    case SP_ERR_CUDA: return g_err_text;
+  }
+  return "unknown sp_status";
+}
+
+int64_t sp_num_rows(const sp_params* p) {
+  const int rc = validate_common(p, false, false);
+  if (rc != SP_OK) return rc;
+  return host_geom(p).num_rows();
+}
+
+int sp_workspace_bytes(const sp_params* p, int stage, size_t* bytes_out) {
+  if (!bytes_out) return SP_ERR_INVALID_ARG;
+  const bool idxr = stage == SP_STAGE_INDEXER_SCORES || stage == SP_STAGE_LAYER_INDEXER;
+  const bool attn = stage != SP_STAGE_INDEXER_SCORES && stage != SP_STAGE_TOPK;
+  const int rc = validate_common(p, attn, idxr);
+  if (rc != SP_OK) return rc;
+  switch (stage) {
+    case SP_STAGE_INDEXER_SCORES: *bytes_out = ws_indexer(p); return SP_OK;
+    case SP_STAGE_ORACLE_MASS: *bytes_out = ws_mass(p); return SP_OK;
+    case SP_STAGE_TOPK:
+    case SP_STAGE_SPARSE_ATTN:
+    case SP_STAGE_DENSE_ATTN: *bytes_out = 0; return SP_OK;
+    case SP_STAGE_LAYER_ORACLE: *bytes_out = plan_layer(p, SP_MODE_ORACLE, true).total; return SP_OK;
+    case SP_STAGE_LAYER_INDEXER: *bytes_out = plan_layer(p, SP_MODE_INDEXER, true).total; return SP_OK;
+  }
+  return SP_ERR_INVALID_ARG;
+}
+
+int sp_indexer_scores(const sp_params* p, const void* X, const void* Wqi, const void* Wki, void* q_idx, void* k_idx,
+                      int32_t preprojected, int32_t row_begin, int32_t row_count, float* scores, int64_t ld_scores,
+                      void* ws, size_t ws_bytes, void* stream) {
+  int rc = validate_common(p, false, true);
+  if (rc != SP_OK) return rc;
+  if (!q_idx || !k_idx || !scores || !aligned16(q_idx) || !aligned16(k_idx) || !aligned16(scores))
+    return SP_ERR_INVALID_ARG;
+  if (!preprojected && (!X || !Wqi || !Wki || !aligned16(X) || !aligned16(Wqi) || !aligned16(Wki)))
+    return SP_ERR_INVALID_ARG;
+  int max_nv = 0;
+  rc = validate_panel(p, row_begin, row_count, ld_scores, &max_nv);
+  if (rc != SP_OK) return rc;
+  if (!preprojected && (ws_bytes < ws_indexer(p) || !ws)) return SP_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!preprojected) SP_CUDA(sp_launch_project(X, Wqi, Wki, q_idx, k_idx, p->L, p->hidden, p->d_idx, ws, st), "projection");
+  SP_CUDA(sp_launch_indexer_scores(dev_geom(p), q_idx, k_idx, p->d_idx, index_scale(p), p->local_window,
+                                   p->local_bias, row_begin, row_count, max_nv, scores, ld_scores, st),
+          "indexer scores");
+  return SP_OK;
+}
+
+int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t row_begin,
+                   int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes, void* stream) {
+  int rc = validate_common(p, true, false);
+  if (rc != SP_OK) return rc;
+  if (!Q || !K || !mass || !aligned16(Q) || !aligned16(K) || !aligned16(mass)) return SP_ERR_INVALID_ARG;
+  if (lse_ready && !lse) return SP_ERR_INVALID_ARG;
+  int max_nv = 0;
+  rc = validate_panel(p, row_begin, row_count, ld_mass, &max_nv);
+  if (rc != SP_OK) return rc;
+  if (!lse) {
+    if (!ws || ws_bytes < ws_mass(p)) return SP_ERR_WORKSPACE;
+    lse = (float*)ws;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  const SpGeom g = dev_geom(p);
+  if (!lse_ready && row_count > 0) {
+    // pass 1 (Alg.1 step 2): softmax normalisers of the panel's queries.  The panel's queries are a
+    // contiguous packed range: from the first query of row_begin to the last query of the last row.
+    const HostGeom hg = host_geom(p);
+    long long r0 = 0;
+    int q_lo = -1, q_hi = -1;
+    for (int i = 0; i < hg.batch; ++i) {
+      const int n = hg.seq_len(i);
+      const long long nr = hg.rows_of(n);
+      const long long lo = row_begin > r0 ? row_begin : r0;
+      const long long hi = ((long long)row_begin + row_count < r0 + nr ? (long long)row_begin + row_count : r0 + nr) - 1;
+      if (lo <= hi) {
+        const int a = hg.seq_start(i) + (int)((lo - r0) * hg.b);
+        long long e = (hi - r0 + 1) * hg.b;
+        if (e > n) e = n;
+        const int b = hg.seq_start(i) + (int)e - 1;
+        if (q_lo < 0) q_lo = a;
+        q_hi = b;
+      }
+      r0 += nr;
+    }
+    SP_CUDA(sp_launch_attn(g, Q, K, nullptr, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
+                           p->local_bias, q_lo, q_hi - q_lo + 1, nullptr, lse, st),
+            "mass pass 1 (lse)");
+  }
+  SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
+                         row_count, max_nv, mass, ld_mass, st),
+          "mass pass 2");
+  return SP_OK;
+}
+
+int sp_topk_support(const sp_params* p, const float* scores, int64_t ld_scores, int32_t row_begin, int32_t row_count,
+                    int32_t* idx, int32_t* cnt, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
+  int rc = validate_common(p, false, false);
+  if (rc != SP_OK) return rc;
+  if (!scores || !idx || !aligned16(scores)) return SP_ERR_INVALID_ARG;
+  int max_nv = 0;
+  rc = validate_panel(p, row_begin, row_count, ld_scores, &max_nv);
+  if (rc != SP_OK) return rc;
+  SP_CUDA(sp_launch_topk(dev_geom(p), scores, ld_scores, row_begin, row_count, p->k, idx, cnt, (cudaStream_t)stream),
+          "top-k");
+  return SP_OK;
+}
+
+int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
+                       float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
+  const int rc = validate_common(p, true, false);
+  if (rc != SP_OK) return rc;
+  if (!Q || !K || !V || !idx || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+    return SP_ERR_INVALID_ARG;
+  SP_CUDA(sp_launch_attn(dev_geom(p), Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
+                         p->local_bias, 0, p->L, O, lse, (cudaStream_t)stream),
+          "sparse attention");
+  return SP_OK;
+}
+
+int sp_dense_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, void* O, float* lse,
+                      void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
+  const int rc = validate_common(p, true, false);
+  if (rc != SP_OK) return rc;
+  if (!Q || !K || (!V && O) || (!O && !lse) || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+    return SP_ERR_INVALID_ARG;
+  SP_CUDA(sp_launch_attn(dev_geom(p), Q, K, V, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
+                         p->local_bias, 0, p->L, O, lse, (cudaStream_t)stream),
+          "dense attention");
+  return SP_OK;
+}
+
+int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void* Wqi, const void* Wki, const void* Q,
+                     const void* K, const void* V, void* O, int32_t* idx_out, void* ws, size_t ws_bytes,
+                     void* stream) {
+  if (mode != SP_MODE_ORACLE && mode != SP_MODE_INDEXER) return SP_ERR_INVALID_ARG;
+  const int rc = validate_common(p, true, mode == SP_MODE_INDEXER);
+  if (rc != SP_OK) return rc;
+  if (!Q || !K || !V || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O)) return SP_ERR_INVALID_ARG;
+  if (mode == SP_MODE_INDEXER && (!X || !Wqi || !Wki || !aligned16(X) || !aligned16(Wqi) || !aligned16(Wki)))
+    return SP_ERR_INVALID_ARG;
+  const LayerPlan pl = plan_layer(p, mode, idx_out == nullptr);
+  if (!ws || !aligned16(ws) || ws_bytes < pl.total) return SP_ERR_WORKSPACE;
+  char* base = (char*)ws;
+  cudaStream_t st = (cudaStream_t)stream;
+  const SpGeom g = dev_geom(p);
+  const HostGeom hg = host_geom(p);
+  float* scores = (float*)(base + pl.off_scores);
+  int32_t* idx = idx_out ? idx_out : (int32_t*)(base + pl.off_idx);
+  void* q_idx = base + pl.off_qidx;
+  void* k_idx = base + pl.off_kidx;
+  float* lse = (float*)(base + pl.off_lse);
+
+  if (mode == SP_MODE_INDEXER) {
+    SP_CUDA(sp_launch_project(X, Wqi, Wki, q_idx, k_idx, p->L, p->hidden, p->d_idx, base + pl.off_stage, st), "projection");
+  } else {
+    SP_CUDA(sp_launch_attn(g, Q, K, nullptr, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
+                           p->local_bias, 0, p->L, nullptr, lse, st),
+            "mass pass 1 (lse)");
+  }
+  for (long long r0 = 0; r0 < pl.n_rows; r0 += pl.panel_rows) {
+    const int rcnt = (int)(pl.n_rows - r0 < pl.panel_rows ? pl.n_rows - r0 : pl.panel_rows);
+    const int max_nv = hg.max_n_valid(r0, rcnt);
+    if (mode == SP_MODE_INDEXER) {
+      SP_CUDA(sp_launch_indexer_scores(g, q_idx, k_idx, p->d_idx, index_scale(p), p->local_window, p->local_bias,
+                                       (int)r0, rcnt, max_nv, scores, pl.ld, st),
+              "indexer scores");
+    } else {
+      SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, (int)r0,
+                             rcnt, max_nv, scores, pl.ld, st),
+              "mass pass 2");
+    }
+    SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
+  }
+  SP_CUDA(sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, 0,
+                         p->L, O, nullptr, st),
+          "sparse attention");
+  return SP_OK;
+}
+
+int sp_layer_host_arena_bytes(const sp_params* p, int32_t mode, size_t* bytes_out) {
+  if (!bytes_out || (mode != SP_MODE_ORACLE && mode != SP_MODE_INDEXER)) return SP_ERR_INVALID_ARG;
+  const int rc = validate_common(p, true, mode == SP_MODE_INDEXER);
+  if (rc != SP_OK) return rc;
+  size_t b = 0;
+  b += align_up((size_t)p->L * p->Hq * p->d * 2) * 2;   // Q, O
+  b += align_up((size_t)p->L * p->Hkv * p->d * 2) * 2;  // K, V
+  if (mode == SP_MODE_INDEXER) {
+    b += align_up((size_t)p->L * p->hidden * 2);
+    b += align_up((size_t)p->hidden * p->d_idx * 2) * 2;
+  }
+  b += plan_layer(p, mode, true).total;
+  *bytes_out = b;
+  return SP_OK;
+}
+
+int sp_prefill_layer_host(const sp_params* p, int32_t mode, const void* X_host, const void* Wqi_host,
+                          const void* Wki_host, const void* Q_host, const void* K_host, const void* V_host,
+                          void* O_host, void* dev_arena, size_t arena_bytes, void* stream) {
+  size_t need = 0;
+  const int rc = sp_layer_host_arena_bytes(p, mode, &need);
+  if (rc != SP_OK) return rc;
+  if (!Q_host || !K_host || !V_host || !O_host) return SP_ERR_INVALID_ARG;
+  if (mode == SP_MODE_INDEXER && (!X_host || !Wqi_host || !Wki_host)) return SP_ERR_INVALID_ARG;
+  if (!dev_arena || !aligned16(dev_arena) || arena_bytes < need) return SP_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  char* a = (char*)dev_arena;
+  const size_t qb = (size_t)p->L * p->Hq * p->d * 2, kb = (size_t)p->L * p->Hkv * p->d * 2;
+  void* dQ = a; a += align_up(qb);
+  void* dO = a; a += align_up(qb);
+  void* dK = a; a += align_up(kb);
+  void* dV = a; a += align_up(kb);
+  void *dX = nullptr, *dWq = nullptr, *dWk = nullptr;
+  SP_CUDA(cudaMemcpyAsync(dQ, Q_host, qb, cudaMemcpyHostToDevice, st), "H2D Q");
+  SP_CUDA(cudaMemcpyAsync(dK, K_host, kb, cudaMemcpyHostToDevice, st), "H2D K");
+  SP_CUDA(cudaMemcpyAsync(dV, V_host, kb, cudaMemcpyHostToDevice, st), "H2D V");
+  if (mode == SP_MODE_INDEXER) {
+    const size_t xb = (size_t)p->L * p->hidden * 2, wb = (size_t)p->hidden * p->d_idx * 2;
+    dX = a; a += align_up(xb);
+    dWq = a; a += align_up(wb);
+    dWk = a; a += align_up(wb);
+    SP_CUDA(cudaMemcpyAsync(dX, X_host, xb, cudaMemcpyHostToDevice, st), "H2D X");
+    SP_CUDA(cudaMemcpyAsync(dWq, Wqi_host, wb, cudaMemcpyHostToDevice, st), "H2D Wqi");
+    SP_CUDA(cudaMemcpyAsync(dWk, Wki_host, wb, cudaMemcpyHostToDevice, st), "H2D Wki");
+  }
+  const size_t ws_bytes = arena_bytes - (size_t)(a - (char*)dev_arena);
+  const int rc2 = sp_prefill_layer(p, mode, dX, dWq, dWk, dQ, dK, dV, dO, nullptr, a, ws_bytes, stream);
+  if (rc2 != SP_OK) return rc2;
+  SP_CUDA(cudaMemcpyAsync(O_host, dO, qb, cudaMemcpyDeviceToHost, st), "D2H O");
+  return SP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,109 @@
+// sp_common.cuh -- shared device/host helpers of the sm_100a sparse-prefill kernels.
+// Geometry of support rows follows include/sp.h ("Support rows"), i.e. PAPER.md:101-103, :152.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sp.h"
+
+#define SP_LOG2E 1.4426950408889634f
+#define SP_LN2 0.6931471805599453f
+
+// Device-visible description of the pack and of the selection granularity.
+struct SpGeom {
+  int batch;
+  int L;
+  const int* cu;  // device cu_seqlens or nullptr
+  int b_sel;
+};
+
+struct SpRow {
+  int seq_start;  // packed position of the sequence's first token
+  int t_first;    // first local query position of the row
+  int t_last;     // last local query position of the row (n_valid = t_last + 1)
+  int seq_len;
+};
+
+__device__ __forceinline__ SpRow sp_row_info(const SpGeom& g, int row) {
+  const int b = g.b_sel;
+  if (g.cu == nullptr) {
+    const int t0 = row * b;
+    return SpRow{0, t0, min(t0 + b - 1, g.L - 1), g.L};
+  }
+  int r0 = 0;
+  for (int i = 0; i < g.batch; ++i) {
+    const int s = g.cu[i], n = g.cu[i + 1] - s;
+    const int nr = (n + b - 1) / b;
+    if (row < r0 + nr) {
+      const int j = row - r0;
+      return SpRow{s, j * b, min(j * b + b - 1, n - 1), n};
+    }
+    r0 += nr;
+  }
+  return SpRow{0, 0, -1, 0};
+}
+
+struct SpPos {
+  int seq_start;
+  int seq_len;
+  int row;  // support row of this packed position
+};
+
+__device__ __forceinline__ SpPos sp_pos_info(const SpGeom& g, int pos) {
+  const int b = g.b_sel;
+  if (g.cu == nullptr) return SpPos{0, g.L, pos / b};
+  int r0 = 0;
+  for (int i = 0; i < g.batch; ++i) {
+    const int s = g.cu[i], n = g.cu[i + 1] - s;
+    if (pos < s + n) return SpPos{s, n, r0 + (pos - s) / b};
+    r0 += (n + b - 1) / b;
+  }
+  return SpPos{0, 0, 0};
+}
+
+__device__ __forceinline__ float sp_bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float sp_bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
+__device__ __forceinline__ uint32_t sp_pack_bf16(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+__device__ __forceinline__ float sp_warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float sp_warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// ---- host-side launch helpers implemented in the individual .cu files ----
+struct SpLaunch {
+  cudaStream_t stream;
+};
+
+cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
+                           int32_t* idx, int32_t* cnt, cudaStream_t st);
+
+cudaError_t sp_launch_project(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
+                              int hidden, int d_idx, void* ws, cudaStream_t st);
+
+cudaError_t sp_launch_indexer_scores(const SpGeom& g, const void* q_idx, const void* k_idx, int d_idx,
+                                     float idx_scale, int local_window, float local_bias, int row_begin,
+                                     int row_count, int max_n_valid, float* scores, int64_t ld, cudaStream_t st);
+
+cudaError_t sp_launch_mass(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, int d,
+                           float scale, int local_window, float local_bias, int row_begin, int row_count,
+                           int max_n_valid, float* mass, int64_t ld, cudaStream_t st);
+
+// idx == nullptr -> dense causal attention.  O may be nullptr (lse only); lse may be nullptr.
+// [q_begin, q_begin+q_count) is the packed query range to process.
+cudaError_t sp_launch_attn(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,
+                           int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int q_begin,
+                           int q_count, void* O, float* lse, cudaStream_t st);
+
+void sp_count_launch(int n = 1);

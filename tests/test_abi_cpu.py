@@ -1,0 +1,101 @@
+"""CPU-only checks of the C-ABI boundary: libsp.so loads without a GPU, exports every symbol that
+include/sp.h declares, and rejects bad arguments with the documented codes before launching anything."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2606_07703_b200 import binding as B
+from paper_2606_07703_b200 import build as sp_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    sp_build.build()
+    return B.lib()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "sp.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(sp_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_functions()
+    assert set(names) == set(B.EXPORTS), (names, B.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_struct_size_matches_header(lib):
+    # 2 int32 + 2 pointers + 7 int32 + 2 float + int32 + float + uint32 = 8 + 16 + 28 + 8 + 12 = 72 bytes
+    assert C.sizeof(B.SpParams) == 72
+
+
+def P(**kw):
+    base = dict(L=256, Hq=8, Hkv=2, d=64, k=16, b_sel=1, hidden=128, d_idx=64, device="cpu")
+    base.update(kw)
+    return B.Problem(**base)
+
+
+def test_num_rows_and_workspace_are_host_arithmetic(lib):
+    assert P().num_rows == 256
+    assert P(b_sel=64, L=300).num_rows == 5
+    assert P(L=40, b_sel=8, cu_seqlens=[0, 19, 27, 40]).num_rows == 3 + 1 + 2
+    for st in range(7):
+        assert B.workspace_bytes(P(), st) >= 0
+    big = P(L=65536, Hq=32, Hkv=8, d=128, k=2048, hidden=4096, d_idx=128)
+    need = B.workspace_bytes(big, B.SP_STAGE_LAYER_INDEXER)
+    assert 1 << 30 < need < 3 << 30          # 1 GiB score panel + 537 MB of indices + projections
+
+
+@pytest.mark.parametrize("kw,code", [
+    (dict(L=0), B.SP_ERR_INVALID_ARG),
+    (dict(k=0), B.SP_ERR_INVALID_ARG),
+    (dict(b_sel=0), B.SP_ERR_INVALID_ARG),
+    (dict(Hq=6, Hkv=4), B.SP_ERR_INVALID_ARG),
+    (dict(d=96), B.SP_ERR_UNSUPPORTED),
+    (dict(Hq=32, Hkv=2), B.SP_ERR_UNSUPPORTED),
+    (dict(flags=1), B.SP_ERR_UNSUPPORTED),
+    (dict(d_idx=32), B.SP_ERR_UNSUPPORTED),
+    (dict(hidden=100), B.SP_ERR_UNSUPPORTED),
+    (dict(local_window=-1), B.SP_ERR_INVALID_ARG),
+    (dict(L=40, cu_seqlens=[0, 19, 19, 40]), B.SP_ERR_INVALID_ARG),
+    (dict(L=40, cu_seqlens=[0, 19, 41]), B.SP_ERR_INVALID_ARG),
+])
+def test_bad_params_are_rejected(lib, kw, code):
+    with pytest.raises(B.SpError) as ei:
+        B.workspace_bytes(P(**kw), B.SP_STAGE_LAYER_INDEXER)
+    assert ei.value.code == code
+
+
+def test_null_and_misaligned_pointers_and_panels(lib):
+    pb = P()
+    p = pb.c()
+    fake = C.c_void_p(0x1000)   # never dereferenced: validation fails first
+    odd = C.c_void_p(0x1008)
+    n = None
+    f = lib.sp_topk_support
+    assert f(C.byref(p), n, C.c_int64(256), 0, 4, fake, n, n, C.c_size_t(0), n) == B.SP_ERR_INVALID_ARG
+    assert f(C.byref(p), odd, C.c_int64(256), 0, 4, fake, n, n, C.c_size_t(0), n) == B.SP_ERR_INVALID_ARG
+    assert f(C.byref(p), fake, C.c_int64(256), 250, 10, fake, n, n, C.c_size_t(0), n) == B.SP_ERR_INVALID_ARG  # panel past the end
+    assert f(C.byref(p), fake, C.c_int64(100), 0, 256, fake, n, n, C.c_size_t(0), n) == B.SP_ERR_INVALID_ARG   # ld < n_valid
+    g = lib.sp_sparse_gqa_attn
+    assert g(C.byref(p), fake, fake, fake, n, fake, n, n, C.c_size_t(0), n) == B.SP_ERR_INVALID_ARG
+    h = lib.sp_prefill_layer
+    assert h(C.byref(p), 7, n, n, n, fake, fake, fake, fake, n, fake, C.c_size_t(1 << 40), n) == B.SP_ERR_INVALID_ARG
+    assert h(C.byref(p), B.SP_MODE_ORACLE, n, n, n, fake, fake, fake, fake, n, fake, C.c_size_t(16), n) == B.SP_ERR_WORKSPACE
+    assert h(C.byref(p), B.SP_MODE_INDEXER, n, n, n, fake, fake, fake, fake, n, fake, C.c_size_t(1 << 40), n) == B.SP_ERR_INVALID_ARG
+    assert b"SP_ERR_WORKSPACE" in lib.sp_strerror(B.SP_ERR_WORKSPACE)
+    assert lib.sp_launch_count() == 0
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    monkeypatch.setattr(B, "_lib", None)
+    monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/libsp.so")
+    with pytest.raises(RuntimeError):
+        B.lib()

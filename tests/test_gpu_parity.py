@@ -1,0 +1,342 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI, via the thin binding) against the fp64
+CPU oracle on the same seeded inputs.  Stage-isolated tests feed ORACLE-produced inputs to one GPU
+stage; chained tests run sp_prefill_layer end to end.  Rules and tolerances: tests/parity.py."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import parity
+from oracle import oracle as orc
+from paper_2606_07703_b200 import binding as B
+from paper_2606_07703_b200 import inputs as gen
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    B.lib()          # fails loudly if libsp.so is missing: there is no fallback
+    yield
+    torch.cuda.synchronize()
+
+
+import functools
+
+
+@functools.lru_cache(maxsize=2)
+def cached_inputs(cfg, with_indexer):
+    return gen.make_inputs(cfg, with_indexer=with_indexer)
+
+
+def orc_problem(cfg, **over):
+    kw = dict(L=cfg.L, Hq=cfg.Hq, Hkv=cfg.Hkv, d=cfg.d, k=cfg.k, b_sel=cfg.b_sel, hidden=cfg.hidden,
+              d_idx=cfg.d_idx, local_window=cfg.local_window, local_bias=cfg.local_bias,
+              cu_seqlens=cfg.cu_seqlens)
+    kw.update(over)
+    return orc.Problem(**kw)
+
+
+def dev(u16):
+    return B.bf16_tensor(u16, DEV)
+
+
+def bf16_bits(t):
+    return t.detach().cpu().view(torch.int16).numpy().view(np.uint16)
+
+
+def to_f64(t):
+    return t.detach().float().cpu().numpy().astype(np.float64)
+
+
+def mode_of(cfg, mode=None):
+    m = mode or cfg.mode
+    return (orc.MODE_ORACLE, B.SP_MODE_ORACLE) if m == "oracle" else (orc.MODE_INDEXER, B.SP_MODE_INDEXER)
+
+
+# ------------------------------------------------------------------ a5 top-k: exact
+
+def rand_scores(seed, rows, ld, quant=None):
+    rng = np.random.Generator(np.random.Philox(seed))
+    x = rng.standard_normal((rows, ld)).astype(np.float32)
+    if quant:
+        x = (np.round(x * quant) / quant).astype(np.float32)     # many exact ties
+    return x
+
+
+@pytest.mark.parametrize("L,b,k,cu,quant", [
+    (3000, 1, 256, None, None),
+    (3000, 1, 256, None, 8),
+    (5000, 64, 1024, None, 16),
+    (70001, 128, 2048, None, None),      # rows longer than the shared-memory row cache, ragged last block
+    (70001, 128, 2048, None, 4),
+    (4096, 64, 512, (0, 1000, 1700, 4096), 8),
+    (300, 8, 512, None, None),           # k > L: every row keeps its whole prefix
+    (1, 1, 4, None, None),
+])
+def test_topk_exact(L, b, k, cu, quant):
+    pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b, cu_seqlens=cu)
+    pbo = orc.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b, cu_seqlens=cu)
+    rows = pbg.num_rows
+    assert rows == orc.num_rows(pbo)
+    if b == 1 and rows > 600:            # per-query: test a panel in the middle and the ragged start
+        panels = [(0, 300), (rows - 300, 300)]
+    else:
+        panels = [(0, rows)]
+    ld = ((pbg.max_seqlen + 3) // 4) * 4
+    for r0, rc in panels:
+        x = rand_scores(100 + L + k, rc, ld, quant)
+        if quant == 4:
+            x[:] = 0.25                                            # one giant tie
+        info = [orc.row_info(pbo, r0 + i) for i in range(rc)]
+        nv = np.array([t1 + 1 for _, _, t1 in info], np.int32)
+        ss = np.array([s for s, _, _ in info], np.int32)
+        want_idx, want_cnt = orc.topk(x.astype(np.float64), nv, k, ss)
+        xs = torch.from_numpy(x).to(DEV)
+        idx = torch.full((rc, k), -7, dtype=torch.int32, device=DEV)
+        cnt = torch.full((rc,), -7, dtype=torch.int32, device=DEV)
+        B.sp_topk_support(pbg, xs, r0, rc, idx, cnt)
+        torch.cuda.synchronize()
+        assert np.array_equal(cnt.cpu().numpy(), want_cnt)
+        assert np.array_equal(idx.cpu().numpy(), want_idx)
+
+
+# ------------------------------------------------------------------ a1/a2/a3 indexer: stage-isolated
+
+SMALL_IDX = gen.shrink(gen.C2, 1500)                  # ragged vs 64 and 128, d_idx = 64, hidden = 1024
+SMALL_IDX128 = gen.shrink(gen.C3, 1100, hidden=512)   # d_idx = 128, local window on
+
+
+@pytest.mark.parametrize("cfg", [SMALL_IDX, SMALL_IDX128], ids=lambda c: c.name)
+def test_projection_matches_oracle(cfg):
+    inp = gen.make_inputs(cfg)
+    pbo = orc_problem(cfg)
+    pbg = B.Problem.from_config(cfg)
+    want_q = orc.project(pbo, inp["X"], inp["Wqi"])
+    want_k = orc.project(pbo, inp["X"], inp["Wki"])
+    q = torch.empty(cfg.L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
+    k = torch.empty_like(q)
+    rows = pbg.num_rows
+    sc = torch.empty(rows, cfg.L, dtype=torch.float32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
+    B.sp_indexer_scores(pbg, dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"]), q, k, False, 0, rows, sc, ws)
+    torch.cuda.synchronize()
+    for got, want in ((bf16_bits(q), want_q), (bf16_bits(k), want_k)):
+        diff = got != want
+        # fp32 vs fp64 accumulation may flip a rounding tie: rare, and never by more than one bf16 ulp
+        assert diff.mean() < 2e-3, diff.mean()
+        a = orc.bf16_to_f64(got[diff])
+        b = orc.bf16_to_f64(want[diff])
+        assert np.all(np.abs(a - b) <= np.abs(b) * 2.0 ** -7 + 1e-30)
+
+
+@pytest.mark.parametrize("cfg,b", [(SMALL_IDX, 64), (SMALL_IDX, 1), (SMALL_IDX128, 64), (SMALL_IDX128, 128),
+                                   (SMALL_IDX128, 1)], ids=lambda v: getattr(v, "name", str(v)))
+def test_indexer_scores_match_oracle(cfg, b):
+    inp = gen.make_inputs(cfg)
+    pbo = orc_problem(cfg, b_sel=b)
+    pbg = B.Problem.from_config(cfg, b_sel=b)
+    q_idx = orc.project(pbo, inp["X"], inp["Wqi"])
+    k_idx = orc.project(pbo, inp["X"], inp["Wki"])
+    rows = pbg.num_rows
+    R, nv = orc.support_scores(pbo, orc.MODE_INDEXER, q_idx, k_idx, np.arange(rows))
+    sc = torch.full((rows, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
+    B.sp_indexer_scores(pbg, None, None, None, dev(q_idx), dev(k_idx), True, 0, rows, sc)
+    got = to_f64(sc)
+    for r in range(rows):
+        n = int(nv[r])
+        assert np.all(np.abs(got[r, :n] - R[r, :n]) <= 1e-5 * np.maximum(1.0, np.abs(R[r, :n]))), r
+    # a panel in the middle gives the same rows
+    r0, rc = rows // 3, max(1, rows // 4)
+    sc2 = torch.full((rc, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
+    B.sp_indexer_scores(pbg, None, None, None, dev(q_idx), dev(k_idx), True, r0, rc, sc2)
+    got2 = to_f64(sc2)
+    for i in range(rc):
+        n = int(nv[r0 + i])
+        assert np.array_equal(got2[i, :n], got[r0 + i, :n])
+
+
+# ------------------------------------------------------------------ a4 attention mass: stage-isolated
+
+SMALL_ORC = gen.shrink(gen.C1, 700)                                   # d=64, G=4
+SMALL_ORC128 = gen.shrink(gen.C4_SWEEP[0], 520, Hq=8, Hkv=2)          # d=128, salience
+
+
+@pytest.mark.parametrize("cfg,b,lw", [(SMALL_ORC, 1, 0), (SMALL_ORC, 64, 0), (SMALL_ORC128, 1, 16),
+                                      (SMALL_ORC128, 64, 16)], ids=lambda v: getattr(v, "name", str(v)))
+def test_mass_matches_oracle(cfg, b, lw):
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(b_sel=b, local_window=lw, local_bias=0.75 if lw else 0.0)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    rows = pbg.num_rows
+    R, nv = orc.support_scores(pbo, orc.MODE_ORACLE, inp["Q"], inp["K"], np.arange(rows))
+    mass = torch.full((rows, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    B.sp_oracle_mass(pbg, dev(inp["Q"]), dev(inp["K"]), lse, False, 0, rows, mass)
+    got = to_f64(mass)
+    for r in range(rows):
+        n = int(nv[r])
+        assert np.all(np.abs(got[r, :n] - R[r, :n]) <= 1e-4 * R[r, :n] + 1e-12), r
+    # pass 1 alone: lse vs the oracle's dense log-sum-exp
+    _, lse_o = orc.dense_attn(pbo, inp["Q"], inp["K"], inp["V"], np.arange(0, cfg.L, 7), want_lse=True)
+    assert np.allclose(to_f64(lse)[::7], lse_o, rtol=0, atol=2e-5)
+    if b == 1:                           # per-query rows of P sum to 1
+        sums = np.array([got[r, :int(nv[r])].sum() for r in range(rows)])
+        assert np.allclose(sums, 1.0, atol=1e-4)
+
+
+# ------------------------------------------------------------------ a6/a7 attention: stage-isolated
+
+@pytest.mark.parametrize("cfg,b,k", [(SMALL_ORC, 1, 96), (SMALL_ORC, 64, 96), (SMALL_ORC128, 1, 64),
+                                     (SMALL_ORC128, 128, 200), (SMALL_ORC128, 64, 8)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_sparse_attention_on_oracle_support(cfg, b, k):
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(b_sel=b, k=k, local_window=12, local_bias=-0.5)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    res = orc.prefill_layer(pbo, orc.MODE_ORACLE, inp["Q"], inp["K"], inp["V"])
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    idx = torch.from_numpy(res.idx).to(DEV)
+    B.sp_sparse_gqa_attn(pbg, dev(inp["Q"]), dev(inp["K"]), dev(inp["V"]), idx, O, lse)
+    parity.compare_attention(to_f64(O), res.out)
+    sup = np.stack([res.idx[orc.row_of_pos(pbo, t)] for t in range(0, cfg.L, 5)])
+    _, lse_o = orc.sparse_attn(pbo, inp["Q"], inp["K"], inp["V"], np.arange(0, cfg.L, 5), sup, want_lse=True)
+    got = to_f64(lse)[::5]
+    fin = np.isfinite(lse_o)
+    assert np.array_equal(np.isfinite(got), fin)                     # empty support -> -inf (A9)
+    assert np.allclose(got[fin], lse_o[fin], rtol=0, atol=2e-5)
+
+
+@pytest.mark.parametrize("cfg", [SMALL_ORC, SMALL_ORC128], ids=lambda c: c.name)
+def test_dense_attention_matches_oracle(cfg):
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(local_window=9, local_bias=0.4)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    B.sp_dense_gqa_attn(pbg, dev(inp["Q"]), dev(inp["K"]), dev(inp["V"]), O, lse)
+    o, l = orc.dense_attn(pbo, inp["Q"], inp["K"], inp["V"], np.arange(cfg.L), want_lse=True)
+    parity.compare_attention(to_f64(O), o)
+    assert np.allclose(to_f64(lse), l, rtol=0, atol=2e-5)
+
+
+def test_varlen_small_pack_layer():
+    cfg = gen.shrink(gen.C5_VARLEN, 1000, cu_seqlens=(0, 300, 301, 690, 1000), hidden=256, k=100, b_sel=32)
+    run_layer_and_compare(cfg, rows=None, n_queries=None)
+
+
+# ------------------------------------------------------------------ chained: sp_prefill_layer vs the oracle
+
+def run_layer_and_compare(cfg, rows, n_queries, mode=None, seed=0, inputs=None):
+    """GPU: the whole layer.  Oracle: support rows `rows` (None = all) and up to n_queries of their queries."""
+    omode, gmode = mode_of(cfg, mode)
+    inp = inputs if inputs is not None else cached_inputs(cfg, gmode == B.SP_MODE_INDEXER)
+    pbo = orc_problem(cfg)
+    pbg = B.Problem.from_config(cfg)
+    n_rows = pbg.num_rows
+    assert n_rows == orc.num_rows(pbo) == cfg.num_rows
+    Q, K, V = dev(inp["Q"]), dev(inp["K"]), dev(inp["V"])
+    X = Wq = Wk = None
+    if gmode == B.SP_MODE_INDEXER:
+        X, Wq, Wk = dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"])
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    idx = torch.full((n_rows, cfg.k), -9, dtype=torch.int32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_LAYER_INDEXER if gmode == B.SP_MODE_INDEXER else B.SP_STAGE_LAYER_ORACLE)
+    B.sp_prefill_layer(pbg, gmode, X, Wq, Wk, Q, K, V, O, idx, ws)
+    torch.cuda.synchronize()
+    del ws
+
+    rows = np.arange(n_rows) if rows is None else np.asarray(sorted(set(int(r) % n_rows for r in rows)))
+    # queries whose outputs the oracle recomputes
+    pos = []
+    for r in rows:
+        s0, t0, t1 = orc.row_info(pbo, int(r))
+        pos.extend(range(s0 + t0, s0 + t1 + 1))
+    pos = np.array(pos)
+    if n_queries is not None and len(pos) > n_queries:
+        rng = np.random.Generator(np.random.Philox(1234 + seed))
+        keep = rng.choice(len(pos), n_queries, replace=False)
+        keep = np.union1d(keep, [0, len(pos) - 1])
+        pos = pos[np.sort(keep)]
+    kw = {}
+    if omode == orc.MODE_INDEXER:
+        # the oracle only reads q_idx of the sampled rows' queries and k_idx up to the last sampled key
+        need_q = []
+        for r in rows:
+            s0, t0, t1 = orc.row_info(pbo, int(r))
+            need_q.extend(range(s0 + t0, s0 + t1 + 1))
+        need_q = np.array(need_q)
+        qi = np.zeros((cfg.L, cfg.d_idx), np.uint16)
+        qi[need_q] = orc.project(pbo, inp["X"], inp["Wqi"], rows=need_q)
+        ki = np.zeros((cfg.L, cfg.d_idx), np.uint16)
+        need_k = np.arange(0, int(need_q.max()) + 1)
+        ki[need_k] = orc.project(pbo, inp["X"], inp["Wki"], rows=need_k)
+        kw["q_idx"], kw["k_idx"] = qi, ki
+    res = orc.prefill_layer(pbo, omode, inp["Q"], inp["K"], inp["V"], rows=rows, pos=pos, **kw)
+
+    idx_gpu = idx.cpu().numpy()
+    stats = parity.compare_supports(idx_gpu[rows], res.idx, res.scores, res.n_valid, cfg.k)
+    # chained: GPU end-to-end vs oracle end-to-end
+    o_gpu = to_f64(O[torch.from_numpy(pos).to(DEV)])
+    stats["chained"] = parity.compare_attention(o_gpu, res.out)
+    # stage-isolated: GPU attention on the ORACLE's supports for the sampled rows
+    idx_mix = idx.clone()
+    idx_mix[torch.from_numpy(rows).to(DEV)] = torch.from_numpy(res.idx).to(DEV)
+    O2 = torch.empty_like(O)
+    B.sp_sparse_gqa_attn(pbg, Q, K, V, idx_mix, O2)
+    stats["isolated"] = parity.compare_attention(to_f64(O2[torch.from_numpy(pos).to(DEV)]), res.out)
+    assert torch.isfinite(O.float()).all()
+    # structural checks on EVERY row of the full-size run (properties that hold at any size)
+    cnt = (idx_gpu >= 0).sum(axis=1)
+    nv_all = np.array([orc.row_info(pbo, r)[2] + 1 for r in range(0, n_rows, max(1, n_rows // 997))])
+    assert np.array_equal(cnt[::max(1, n_rows // 997)], np.minimum(cfg.k, nv_all))
+    return stats
+
+
+def test_config1_oracle_mode_full():
+    st = run_layer_and_compare(gen.C1, rows=None, n_queries=None)
+    assert st["strict"] >= 256
+
+
+def test_config2_indexer_block_shared_full_supports():
+    st = run_layer_and_compare(gen.C2, rows=None, n_queries=384)
+    assert st["strict"] + st["fuzzy"] == 128
+
+
+def test_config3_9b_layer_sampled():
+    rows = [0, 1, 31, 32, 33, 200, 389, 511]
+    run_layer_and_compare(gen.C3, rows=rows, n_queries=256)
+
+
+@pytest.mark.parametrize("cfg", gen.C4_SWEEP, ids=lambda c: c.name)
+@pytest.mark.parametrize("mode", ["oracle", "indexer"])
+def test_config4_sweep_sampled(cfg, mode):
+    L, k = cfg.L, cfg.k
+    rng = np.random.Generator(np.random.Philox(cfg.L))
+    rows = [0, 1, k - 2, k - 1, k, k + 1, L - 1, L // 2] + list(rng.integers(k, L, size=24))
+    run_layer_and_compare(cfg, rows=rows, n_queries=None, mode=mode)
+
+
+def test_config5_long_context_sampled():
+    rows = [0, 15, 16, 17, 500, 1023]
+    run_layer_and_compare(gen.C5, rows=rows, n_queries=192)
+
+
+def test_config5_varlen_pack_sampled():
+    cfg = gen.C5_VARLEN
+    rows = [0, 16, 127, 128, 150, 223, 224, 287, 288, 319]      # first/last block of every sequence
+    run_layer_and_compare(cfg, rows=rows, n_queries=256)
+
+
+# ------------------------------------------------------------------ degenerate cases
+
+@pytest.mark.parametrize("L,k,b", [(1, 4, 1), (5, 64, 1), (70, 3, 64), (130, 1, 64), (64, 64, 64)])
+def test_degenerate_shapes(L, k, b):
+    cfg = gen.shrink(gen.C1, L, k=k, b_sel=b)
+    run_layer_and_compare(cfg, rows=None, n_queries=None)

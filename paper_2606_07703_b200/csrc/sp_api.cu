@@ -6,9 +6,22 @@
 #include <cstring>
 #include <mutex>
 
+#include <cstdlib>
+
 #include "sp_common.cuh"
 
 namespace {
+
+// Debug switch (never set in tests/bench): SP_DEBUG_SIMT bitmask routes a stage to its CUDA-core kernel so the two
+// device implementations can be compared on the GPU box.  1 = projection, 2 = indexer scores, 4 = attention, 8 = mass.
+int debug_simt() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = getenv("SP_DEBUG_SIMT");
+    v = e ? atoi(e) : 0;
+  }
+  return v;
+}
 
 std::atomic<long long> g_launches{0};
 std::mutex g_err_mu;
@@ -108,6 +121,24 @@ int validate_panel(const sp_params* p, int32_t row_begin, int32_t row_count, int
   return SP_OK;
 }
 
+// ---- stage dispatch: tcgen05 kernels where the shape is in their built set, CUDA-core kernels otherwise ----
+cudaError_t run_project(const sp_params* p, const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx,
+                        void* ws, cudaStream_t st) {
+  if (!(debug_simt() & 1)) return sp_launch_project_tc(X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, st);
+  return sp_launch_project(X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, ws, st);
+}
+
+cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void* k_idx, int row_begin, int row_count,
+                               int max_nv, float* scores, int64_t ld, cudaStream_t st) {
+  const SpGeom g = dev_geom(p);
+  if (sp_tc_scores_supported(p->b_sel) && !(debug_simt() & 2))
+    return sp_launch_indexer_scores_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, q_idx, k_idx, p->d_idx,
+                                       index_scale(p), p->local_window, p->local_bias, row_begin, row_count, max_nv,
+                                       scores, ld, st);
+  return sp_launch_indexer_scores(g, q_idx, k_idx, p->d_idx, index_scale(p), p->local_window, p->local_bias, row_begin,
+                                  row_count, max_nv, scores, ld, st);
+}
+
 // ---- workspace sizes ----
 size_t ws_indexer(const sp_params* p) { return align_up((size_t)2 * p->hidden * p->d_idx * 2); }
 size_t ws_mass(const sp_params* p) { return align_up((size_t)p->L * p->Hq * sizeof(float)); }
@@ -202,10 +233,8 @@ int sp_indexer_scores(const sp_params* p, const void* X, const void* Wqi, const 
   if (rc != SP_OK) return rc;
   if (!preprojected && (ws_bytes < ws_indexer(p) || !ws)) return SP_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
-  if (!preprojected) SP_CUDA(sp_launch_project(X, Wqi, Wki, q_idx, k_idx, p->L, p->hidden, p->d_idx, ws, st), "projection");
-  SP_CUDA(sp_launch_indexer_scores(dev_geom(p), q_idx, k_idx, p->d_idx, index_scale(p), p->local_window,
-                                   p->local_bias, row_begin, row_count, max_nv, scores, ld_scores, st),
-          "indexer scores");
+  if (!preprojected) SP_CUDA(run_project(p, X, Wqi, Wki, q_idx, k_idx, ws, st), "projection");
+  SP_CUDA(run_indexer_scores(p, q_idx, k_idx, row_begin, row_count, max_nv, scores, ld_scores, st), "indexer scores");
   return SP_OK;
 }
 
@@ -314,7 +343,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
   float* lse = (float*)(base + pl.off_lse);
 
   if (mode == SP_MODE_INDEXER) {
-    SP_CUDA(sp_launch_project(X, Wqi, Wki, q_idx, k_idx, p->L, p->hidden, p->d_idx, base + pl.off_stage, st), "projection");
+    SP_CUDA(run_project(p, X, Wqi, Wki, q_idx, k_idx, base + pl.off_stage, st), "projection");
   } else {
     SP_CUDA(sp_launch_attn(g, Q, K, nullptr, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
                            p->local_bias, 0, p->L, nullptr, lse, st),
@@ -324,9 +353,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
     const int rcnt = (int)(pl.n_rows - r0 < pl.panel_rows ? pl.n_rows - r0 : pl.panel_rows);
     const int max_nv = hg.max_n_valid(r0, rcnt);
     if (mode == SP_MODE_INDEXER) {
-      SP_CUDA(sp_launch_indexer_scores(g, q_idx, k_idx, p->d_idx, index_scale(p), p->local_window, p->local_bias,
-                                       (int)r0, rcnt, max_nv, scores, pl.ld, st),
-              "indexer scores");
+      SP_CUDA(run_indexer_scores(p, q_idx, k_idx, (int)r0, rcnt, max_nv, scores, pl.ld, st), "indexer scores");
     } else {
       SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, (int)r0,
                              rcnt, max_nv, scores, pl.ld, st),

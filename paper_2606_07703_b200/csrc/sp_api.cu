@@ -139,6 +139,24 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
                                   row_count, max_nv, scores, ld, st);
 }
 
+// idx == nullptr -> dense.  [q_begin, q_begin + q_count) must be the whole pack for the tcgen05 kernel.
+cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
+                     int q_count, void* O, float* lse, cudaStream_t st) {
+  const SpGeom g = dev_geom(p);
+  const int G = p->Hq / p->Hkv;
+  const bool whole = q_begin == 0 && q_count == p->L;
+  if (whole && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k)) {
+    const HostGeom hg = host_geom(p);
+    const int QT = 256 / G;
+    long long chunks = 0;
+    for (int i = 0; i < hg.batch; ++i) chunks += (hg.seq_len(i) + QT - 1) / QT;
+    return sp_launch_attn_tc(g, hg.num_rows(), chunks, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p),
+                             p->local_window, p->local_bias, O, lse, st);
+  }
+  return sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
+                        q_begin, q_count, O, lse, st);
+}
+
 // ---- workspace sizes ----
 size_t ws_indexer(const sp_params* p) { return align_up((size_t)2 * p->hidden * p->d_idx * 2); }
 size_t ws_mass(const sp_params* p) { return align_up((size_t)p->L * p->Hq * sizeof(float)); }
@@ -274,9 +292,7 @@ int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse,
       }
       r0 += nr;
     }
-    SP_CUDA(sp_launch_attn(g, Q, K, nullptr, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
-                           p->local_bias, q_lo, q_hi - q_lo + 1, nullptr, lse, st),
-            "mass pass 1 (lse)");
+    SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, q_lo, q_hi - q_lo + 1, nullptr, lse, st), "mass pass 1 (lse)");
   }
   SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
                          row_count, max_nv, mass, ld_mass, st),
@@ -303,9 +319,7 @@ int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const v
   if (rc != SP_OK) return rc;
   if (!Q || !K || !V || !idx || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
     return SP_ERR_INVALID_ARG;
-  SP_CUDA(sp_launch_attn(dev_geom(p), Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
-                         p->local_bias, 0, p->L, O, lse, (cudaStream_t)stream),
-          "sparse attention");
+  SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, lse, (cudaStream_t)stream), "sparse attention");
   return SP_OK;
 }
 
@@ -315,9 +329,7 @@ int sp_dense_gqa_attn(const sp_params* p, const void* Q, const void* K, const vo
   if (rc != SP_OK) return rc;
   if (!Q || !K || (!V && O) || (!O && !lse) || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
     return SP_ERR_INVALID_ARG;
-  SP_CUDA(sp_launch_attn(dev_geom(p), Q, K, V, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
-                         p->local_bias, 0, p->L, O, lse, (cudaStream_t)stream),
-          "dense attention");
+  SP_CUDA(run_attn(p, Q, K, V, nullptr, 0, p->L, O, lse, (cudaStream_t)stream), "dense attention");
   return SP_OK;
 }
 
@@ -345,9 +357,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
   if (mode == SP_MODE_INDEXER) {
     SP_CUDA(run_project(p, X, Wqi, Wki, q_idx, k_idx, base + pl.off_stage, st), "projection");
   } else {
-    SP_CUDA(sp_launch_attn(g, Q, K, nullptr, nullptr, 0, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
-                           p->local_bias, 0, p->L, nullptr, lse, st),
-            "mass pass 1 (lse)");
+    SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, 0, p->L, nullptr, lse, st), "mass pass 1 (lse)");
   }
   for (long long r0 = 0; r0 < pl.n_rows; r0 += pl.panel_rows) {
     const int rcnt = (int)(pl.n_rows - r0 < pl.panel_rows ? pl.n_rows - r0 : pl.panel_rows);
@@ -361,9 +371,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
     }
     SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
   }
-  SP_CUDA(sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, 0,
-                         p->L, O, nullptr, st),
-          "sparse attention");
+  SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st), "sparse attention");
   return SP_OK;
 }
 

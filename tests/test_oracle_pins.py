@@ -87,17 +87,24 @@ def test_config1_pair_count():
 
 # ---------------------------------------------------------------- P7: hand-worked case
 
+def _golden_handworked():
+    rec = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "handworked_L4.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            head, vals = line.split(":")
+            name, row = head.split()
+            rec.setdefault(name, {})[int(row)] = [Fraction(v) for v in vals.split()]
+    return rec
+
+
 def test_handworked_L4():
-    """L=4, Hq=2, Hkv=1, d=1.  q[t,0]=1, q[t,1]=0, k_s = s, scale = ln 2, v_s = s.
-    Head 0 has logits s*ln2 -> weights 2^s; head 1 is uniform.  From PAPER.md:94, :123:
-      P_1 = ((1/3+1/2)/2, (2/3+1/2)/2) = (5/12, 7/12)
-      P_2 = ((1/7+1/3)/2, (2/7+1/3)/2, (4/7+1/3)/2) = (5/21, 13/42, 19/42)
-      P_3 = ((1/15+1/4)/2, (2/15+1/4)/2, (4/15+1/4)/2, (8/15+1/4)/2) = (19,23,31,47)/120
-    Per-query k=2 (PAPER.md:127, :107): S_1={0,1}, S_2={1,2}, S_3={2,3};
-      o[1]=(2/3,1/2), o[2]=(5/3,3/2), o[3]=(8/3,5/2), o[0]=(0,0).
-    Block b=2,k=2 (PAPER.md:154,:156): block {2,3}: R=(5/21,13/42,19/42,47/120) -> S={2,3};
-      query 2 re-masks to {2} -> o[2]=(2,2); query 3 -> (8/3,5/2). Block {0,1}: S={0,1}."""
-    F = Fraction
+    """tests/golden/handworked_L4.txt: L=4, Hq=2, Hkv=1, d=1, q[t,0]=1, q[t,1]=0, k_s=s, scale=ln 2, v_s=s.
+    Head 0 has logits s*ln2 -> weights 2^s; head 1 is uniform.  Exact rationals derived by hand from
+    PAPER.md:94, :123 (P), :127/:107 (per-query k=2) and :154/:156 (block b=2 with per-query re-mask)."""
+    G = _golden_handworked()
     one = gen.f32_to_bf16(np.array([1.0], np.float32))[0]
     Q = np.zeros((4, 2, 1), np.uint16)
     Q[:, 0, 0] = one
@@ -105,27 +112,24 @@ def test_handworked_L4():
     V = K.copy()
     pb = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=2, b_sel=1, scale=math.log(2.0))
     P = orc.query_scores(pb, orc.MODE_ORACLE, Q, K, np.arange(4))
-    want = [[F(1)], [F(5, 12), F(7, 12)], [F(5, 21), F(13, 42), F(19, 42)],
-            [F(19, 120), F(23, 120), F(31, 120), F(47, 120)]]
     for t in range(4):
-        assert np.allclose(P[t, :t + 1], [float(x) for x in want[t]], rtol=0, atol=1e-15)
+        assert np.allclose(P[t, :t + 1], [float(x) for x in G["P"][t]], rtol=0, atol=1e-15)
         assert np.all(np.isneginf(P[t, t + 1:]))
     res = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
-    assert res.idx.tolist() == [[0, -1], [0, 1], [1, 2], [2, 3]]
+    assert res.idx.tolist() == [[int(x) for x in G["idx_k2"][t]] for t in range(4)]
     assert res.cnt.tolist() == [1, 2, 2, 2]
-    o = res.out[:, :, 0]
-    want_o = [[0, 0], [F(2, 3), F(1, 2)], [F(5, 3), F(3, 2)], [F(8, 3), F(5, 2)]]
-    assert np.allclose(o, np.array(want_o, dtype=float), rtol=0, atol=1e-14)
+    want_o = np.array([[float(x) for x in G["o_k2"][t]] for t in range(4)])
+    assert np.allclose(res.out[:, :, 0], want_o, rtol=0, atol=1e-14)
     # block-shared
     pbb = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=2, b_sel=2, scale=math.log(2.0))
     R, nv = orc.support_scores(pbb, orc.MODE_ORACLE, Q, K, [0, 1])
     assert nv.tolist() == [2, 4]
-    assert np.allclose(R[1], [5 / 21, 13 / 42, 19 / 42, 47 / 120], atol=1e-15)
-    assert np.allclose(R[0, :2], [1.0, 7 / 12], atol=1e-15) and np.all(np.isneginf(R[0, 2:]))
+    assert np.allclose(R[1], [float(x) for x in G["R_b2"][1]], atol=1e-15)
+    assert np.allclose(R[0, :2], [float(x) for x in G["R_b2"][0]], atol=1e-15) and np.all(np.isneginf(R[0, 2:]))
     resb = orc.prefill_layer(pbb, orc.MODE_ORACLE, Q, K, V)
-    assert resb.idx.tolist() == [[0, 1], [2, 3]]
-    want_ob = [[0, 0], [F(2, 3), F(1, 2)], [2, 2], [F(8, 3), F(5, 2)]]
-    assert np.allclose(resb.out[:, :, 0], np.array(want_ob, dtype=float), rtol=0, atol=1e-14)
+    assert resb.idx.tolist() == [[int(x) for x in G["idx_b2"][r]] for r in range(2)]
+    want_ob = np.array([[float(x) for x in G["o_b2"][t]] for t in range(4)])
+    assert np.allclose(resb.out[:, :, 0], want_ob, rtol=0, atol=1e-14)
     # k=1: the mass is increasing in s for both heads, so S_t={t} and o[t]=v_t=t
     pb1 = orc.Problem(L=4, Hq=2, Hkv=1, d=1, k=1, b_sel=1, scale=math.log(2.0))
     r1 = orc.prefill_layer(pb1, orc.MODE_ORACLE, Q, K, V)

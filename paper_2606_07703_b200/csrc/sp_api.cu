@@ -145,7 +145,7 @@ cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const voi
   const SpGeom g = dev_geom(p);
   const int G = p->Hq / p->Hkv;
   const bool whole = q_begin == 0 && q_count == p->L;
-  if (whole && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k)) {
+  if (whole && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k, p->d)) {
     const HostGeom hg = host_geom(p);
     const int QT = 256 / G;
     long long chunks = 0;

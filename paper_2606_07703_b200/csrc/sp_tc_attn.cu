@@ -1,18 +1,20 @@
 // sp_tc_attn.cu -- GQA attention with online softmax on tcgen05 / TMEM (PAPER.md:94 dense, :107 + :156 sparse).
 //
-// One CTA = one chunk of up to 256/G consecutive queries of ONE support row x one KV head: the G query heads of
-// the KV group are stacked along the MMA M dimension (row R = query * G + head), so one gathered K/V tile is
-// shared by 256 rows (two M = 128 tiles).  Key tiles hold 64 keys.
-//   SPARSE: the keys are the support row's index list (gathered rows, cp.async 16-byte vectors, 128-byte swizzle
-//           written by hand so the tile has the image TMA SWIZZLE_128B would have produced);
-//   DENSE : the keys are the causal prefix of the sequence (same loader, consecutive rows).
-// Warp roles: warps 0-3 / 4-7 softmax of M tile 0 / 1 (thread = row, TMEM lane = row), warp 8 MMA issuer
-// (one elected thread), warps 9-12 K/V/Q loaders.  Per key tile and M tile:
-//   S = Q K^T (tcgen05.mma, fp32 in TMEM, double buffered) -> tcgen05.ld -> scale, mask by KEY POSITION VALUE,
-//   online softmax with lazy rescaling of the TMEM-resident O accumulator -> P (bf16) to shared memory ->
-//   O += P V (tcgen05.mma, V read MN-major from the same row-major tile).
-// Only tiles that can contain a masked or locally-biased element take the per-element path (flags computed
-// once per CTA from the index list).
+// PERSISTENT kernel, one CTA per SM.  A work item = one chunk of up to 256/G consecutive queries of ONE support
+// row x one KV head: the G query heads of the KV group are stacked along the MMA M dimension (row R = query * G +
+// head), so one gathered K/V tile is shared by 256 rows (two M = 128 tiles).  Key tiles hold 64 keys.
+//   SPARSE: the keys are the support row's index list, staged once per item in shared memory; K/V rows are
+//           gathered with cp.async 16-byte vectors written in the SWIZZLE_128B image TMA would have produced;
+//   DENSE : the keys are the causal prefix of the sequence (same loader, consecutive rows), heavy chunks first.
+// Warp roles: warps 0-3 / 4-7 softmax of M tile 0 / 1 (thread = row = TMEM lane), warp 8 MMA issuer (one
+// thread), warps 9-12 index staging + Q/K/V loaders (13-15 idle).  Rings (K, V stages; S double buffered per M tile in TMEM)
+// run ACROSS items, so the loaders prefetch the next item's index list, K and V while the current one finishes.
+// Per key tile and M tile:
+//   S = Q K^T (tcgen05.mma SS, fp32 in TMEM) -> tcgen05.ld -> scale, mask by KEY POSITION VALUE, online softmax
+//   with lazy rescaling of the TMEM-resident O accumulator -> P (bf16x2) written back over S with tcgen05.st ->
+//   O += P V (tcgen05.mma with A = P from TMEM, B = V read MN-major from the row-major tile).
+// Only tiles that can contain a masked or locally-biased element take the per-element path (flags computed by
+// the loaders while staging the index list).
 #include "sp_common.cuh"
 #include "sp_tc.cuh"
 
@@ -20,9 +22,10 @@ using namespace sptc;
 
 namespace {
 
-constexpr int AT_KT = 64;        // keys per tile
-constexpr int AT_STAGES = 3;     // K/V ring
-constexpr int AT_THREADS = 416;  // 8 softmax warps + 1 MMA warp + 4 loader warps
+constexpr int AT_KT = 64;          // keys per tile
+constexpr int AT_MAX_STAGES = 6;   // K/V ring depth is chosen at launch from the shared-memory budget
+constexpr int AT_THREADS = 512;    // 8 softmax warps + 1 MMA warp + 4 loader warps + 3 idle (whole warpgroups for setmaxnreg)
+constexpr int AT_LOAD_WARPS = 4;
 constexpr int AT_MMA_WARP = 8;
 constexpr int AT_LOAD_WARP0 = 9;
 constexpr float AT_RESCALE_THRESHOLD = 8.0f;  // log2 units: O is rescaled only when the row max grew by > 2^8
@@ -30,121 +33,137 @@ constexpr float AT_RESCALE_THRESHOLD = 8.0f;  // log2 units: O is rescaled only 
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t* bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void loader_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+// D[tmem] (+)= A[tmem] * B[smem]: A = 128 lanes x (K/2) 32-bit columns of packed bf16 pairs (K-major).
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                        uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
+// packed fp32 pairs (sm_100 FFMA2 / FADD2)
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t bf16x2_rn(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
 
 struct AtBarriers {
-  uint64_t qfull;
-  uint64_t kfull[AT_STAGES], kempty[AT_STAGES], vfull[AT_STAGES], vempty[AT_STAGES];
-  uint64_t sfull[2][2], sempty[2][2];
-  uint64_t pfull[2], pempty[2];
+  uint64_t qfull, qempty;
+  uint64_t kfull[AT_MAX_STAGES], kempty[AT_MAX_STAGES], vfull[AT_MAX_STAGES], vempty[AT_MAX_STAGES];
+  uint64_t sfull[2][2];  // MMA -> softmax: S tile (M tile, buffer) is in TMEM
+  uint64_t sdone[2][2];  // softmax -> MMA: S has been read (and P written over it)
+  uint64_t ofull[2];     // MMA -> softmax: one completion per PV of that M tile (lazy-rescale path)
+  uint64_t ofin[2];      // MMA -> softmax: one completion per ITEM, after its last PV (epilogue).  A parity wait on
+                         // ofull could alias here: the softmax may be two PVs ahead of the tensor pipe.
+  uint64_t oempty[2];    // softmax -> MMA: the item's O accumulator has been read out
+  uint64_t idxfull[2], idxempty[2];
 };
+
+struct AtItem {
+  int seq_start, t0, t1, kvh, row;
+};
+
+// Work item `id` -> queries and KV head.  Identical in every warp role.
+template <int G, bool SPARSE>
+__device__ __forceinline__ bool at_item(const SpGeom& g, int id, int Hkv, int cpr, int n_chunks, AtItem& it) {
+  constexpr int QT = 256 / G;
+  it.kvh = id % Hkv;
+  const int x = id / Hkv;
+  if (SPARSE) {
+    it.row = x / cpr;
+    const SpRow ri = sp_row_info(g, it.row);
+    it.seq_start = ri.seq_start;
+    it.t0 = ri.t_first + (x % cpr) * QT;
+    it.t1 = min(it.t0 + QT - 1, ri.t_last);
+    return it.t0 <= ri.t_last;
+  } else {
+    SpGeom g2 = g;
+    g2.b_sel = QT;
+    it.row = n_chunks - 1 - x;  // heavy (late) chunks first
+    const SpRow ri = sp_row_info(g2, it.row);
+    it.seq_start = ri.seq_start;
+    it.t0 = ri.t_first;
+    it.t1 = ri.t_last;
+    return it.t1 >= it.t0;
+  }
+}
+
+// The i-th item of CTA c out of P: boustrophedon over rounds so that per-CTA totals balance when the cost falls
+// monotonically with the item id (dense causal chunks).  Returns -1 when the round has no item for this CTA.
+__device__ __forceinline__ int at_item_id(int i, int c, int P, int n_items) {
+  const int id = i * P + ((i & 1) ? P - 1 - c : c);
+  return id < n_items ? id : -1;
+}
 
 template <int D, int G, bool SPARSE, bool WITH_O>
 __global__ void __launch_bounds__(AT_THREADS, 1)
 sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
-                  int local_window, float local_bias, int chunks_per_row, __nv_bfloat16* __restrict__ O,
-                  float* __restrict__ lse) {
-  constexpr int QT = 256 / G;             // queries per CTA
+                  int local_window, float local_bias, int chunks_per_row, int n_chunks, int n_items, int n_stages,
+                  int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
   constexpr int KB = D / 64;              // 64-wide column blocks of a row
   constexpr int CPR = D / 8;              // 16-byte chunks per row
   constexpr uint32_t Q_BLK = 256 * 128;   // bytes of one column block of the Q tile (256 rows)
   constexpr uint32_t KV_BLK = AT_KT * 128;
   constexpr uint32_t KV_TILE = KB * KV_BLK;
-  constexpr uint32_t P_TILE = 128 * 128;  // 128 rows x 64 keys bf16
-  constexpr uint32_t TM_O = 0, TM_S = 256;
+  constexpr uint32_t TM_O = 0, TM_S = 256;  // O: M tile mt at columns [mt*D, mt*D+D); S: (mt, b) at 256 + mt*128 + b*64
 
   extern __shared__ uint8_t smem_raw[];
   __shared__ AtBarriers bar;
   __shared__ uint32_t tmem_slot;
-  __shared__ int n_eff_sh;
+  __shared__ int n_eff_sh[2];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int kvh = blockIdx.y;
   const int Hq = Hkv * G;
-
-  // ---- which queries ----
-  int seq_start, t0, t1, row = 0;
-  if (SPARSE) {
-    row = blockIdx.x / chunks_per_row;
-    const int ci = blockIdx.x % chunks_per_row;
-    const SpRow ri = sp_row_info(g, row);
-    seq_start = ri.seq_start;
-    t0 = ri.t_first + ci * QT;
-    t1 = min(t0 + QT - 1, ri.t_last);
-    if (t0 > ri.t_last) return;
-  } else {
-    SpGeom g2 = g;
-    g2.b_sel = QT;
-    const SpRow ri = sp_row_info(g2, (int)(gridDim.x - 1 - blockIdx.x));  // heavy (late) chunks first
-    seq_start = ri.seq_start;
-    t0 = ri.t_first;
-    t1 = ri.t_last;
-    if (t1 < t0) return;
-  }
-  const int nq = t1 - t0 + 1;
-  const int n_mt = (nq * G > 128) ? 2 : 1;
-  const int32_t* sup = SPARSE ? idx + (size_t)row * k : nullptr;
+  const int NS = n_stages;
+  const int P = gridDim.x, cta = blockIdx.x;
 
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint8_t* sQ = smem;
   uint8_t* sK = sQ + KB * Q_BLK;
-  uint8_t* sV = sK + AT_STAGES * KV_TILE;
-  uint8_t* sP = sV + AT_STAGES * KV_TILE;
-  uint32_t* flags = reinterpret_cast<uint32_t*>(sP + 2 * P_TILE);  // SPARSE: one word per key tile
+  uint8_t* sV = sK + NS * KV_TILE;
+  int* sIdx = reinterpret_cast<int*>(sV + (WITH_O ? NS * KV_TILE : 0));    // SPARSE: [2][kpad]
+  uint32_t* sFlag = reinterpret_cast<uint32_t*>(sIdx + 2 * kpad);          // SPARSE: [2][kpad / 64]
+  const int ntmax = kpad / AT_KT;
 
-  // first query (packed) of each M tile and the position threshold below which a key needs no per-element work
   const int win = local_window > 0 ? local_window : 0;
-  const int qa0 = seq_start + t0, qa1 = seq_start + t0 + 128 / G;
-
-  // ---- prologue: tile count and per-tile flags ----
-  int nt;
-  int nt_mt[2];
-  if (SPARSE) {
-    const int nt_max = (k + AT_KT - 1) / AT_KT;
-    if (threadIdx.x == 0) n_eff_sh = 0;
-    for (int i = threadIdx.x; i < nt_max; i += AT_THREADS) flags[i] = (i * AT_KT + AT_KT > k) ? 3u : 0u;
-    __syncthreads();
-    int my_last = 0;
-    for (int i = threadIdx.x; i < k; i += AT_THREADS) {
-      const int p = __ldg(sup + i);
-      if (p >= 0) my_last = i + 1;
-      uint32_t f = 0;
-      if (p < seq_start || p > qa0 - win) f |= 1u;
-      if (p < seq_start || p > qa1 - win) f |= 2u;
-      if (f) atomicOr(&flags[i / AT_KT], f);
-    }
-    if (my_last) atomicMax(&n_eff_sh, my_last);
-    __syncthreads();
-    nt = (n_eff_sh + AT_KT - 1) / AT_KT;
-    nt_mt[0] = nt_mt[1] = nt;
-  } else {
-    nt = t1 / AT_KT + 1;
-    nt_mt[0] = min(t0 + 128 / G - 1, t1) / AT_KT + 1;
-    nt_mt[1] = nt;
-  }
   const bool scale_pos = scale > 0.f;
   const float sl2 = scale * SP_LOG2E, lb2 = local_bias * SP_LOG2E;
-
-  if (nt == 0) {  // empty support: O = 0, lse = -inf (reading A9)
-    if (warp < 8) {
-      const int R = warp * 32 + lane;
-      const int ql = R / G, h = R % G;
-      if (ql < nq) {
-        const size_t orow = ((size_t)(seq_start + t0 + ql) * Hq + kvh * G + h);
-        if (WITH_O) {
-          uint4 z = make_uint4(0, 0, 0, 0);
-          for (int c = 0; c < CPR; ++c) reinterpret_cast<uint4*>(O + orow * D)[c] = z;
-        }
-        if (lse) lse[orow] = -INFINITY;
-      }
-    }
-    return;
-  }
 
   // ---- barriers, TMEM ----
   if (threadIdx.x == 0) {
     mbar_init(&bar.qfull, 128);
-    for (int s = 0; s < AT_STAGES; ++s) {
+    mbar_init(&bar.qempty, 1);
+    for (int s = 0; s < AT_MAX_STAGES; ++s) {
       mbar_init(&bar.kfull[s], 128);
       mbar_init(&bar.vfull[s], 128);
       mbar_init(&bar.kempty[s], 1);
@@ -153,10 +172,13 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     for (int m = 0; m < 2; ++m) {
       for (int b = 0; b < 2; ++b) {
         mbar_init(&bar.sfull[m][b], 1);
-        mbar_init(&bar.sempty[m][b], 128);
+        mbar_init(&bar.sdone[m][b], 128);
       }
-      mbar_init(&bar.pfull[m], 128);
-      mbar_init(&bar.pempty[m], 1);
+      mbar_init(&bar.ofull[m], 1);
+      mbar_init(&bar.ofin[m], 1);
+      mbar_init(&bar.oempty[m], 128);
+      mbar_init(&bar.idxfull[m], 128);
+      mbar_init(&bar.idxempty[m], 256);
     }
     fence_barrier_init();
   }
@@ -166,251 +188,384 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   tc_fence_after_sync();
   const uint32_t tmem = tmem_slot;
 
-  if (warp >= AT_LOAD_WARP0) {
+  // register budget: 512 x 128 at launch -> softmax warpgroups 192, the other two warpgroups 64
+  // (each role's code is dominated by its own setmaxnreg so ptxas allocates per role)
+  if (warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");  // idle warps
+  } else if (warp >= AT_LOAD_WARP0) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
     // =========================================== loaders ===========================================
     const int ptid = threadIdx.x - AT_LOAD_WARP0 * 32;  // 0..127
-    {  // Q tile: row R = query * G + head; rows past the chunk repeat its last query (outputs never written)
-      for (int e = ptid; e < 256 * CPR; e += 128) {
-        const int R = e / CPR, c = e % CPR;
-        if (R >= n_mt * 128) break;
-        const int ql = min(R / G, nq - 1), h = R % G;
-        const __nv_bfloat16* src = Q + ((size_t)(seq_start + t0 + ql) * Hq + kvh * G + h) * D + c * 8;
-        cp_async16(smem_u32(sQ + (c / 8) * Q_BLK) + sw128_offset(R, c % 8), src);
-      }
-      cp_async_arrive_noinc(&bar.qfull);
-    }
     constexpr int KPP = 128 / CPR;       // keys per pass of the 128 loader threads
     constexpr int PASSES = AT_KT / KPP;  // passes per tile
     const int c = ptid % CPR;
     const int key0 = ptid / CPR;
-    for (int j = 0; j < nt; ++j) {
-      const int s = j % AT_STAGES, u = j / AT_STAGES;
-      int pos[PASSES];
-#pragma unroll
-      for (int i = 0; i < PASSES; ++i) {
-        const int col = j * AT_KT + key0 + i * KPP;
-        int p;
-        if (SPARSE) {
-          p = col < k ? __ldg(sup + col) : -1;
-          if (p < seq_start || p > seq_start + t1) p = seq_start;  // masked later; any valid row will do
-        } else {
-          p = seq_start + min(col, t1);
+    const uint32_t kv_off = (uint32_t)(c / 8) * KV_BLK;
+    uint32_t gk = 0, n_q = 0, n_it = 0;
+    for (int i = 0; i * P < n_items; ++i) {
+      const int id = at_item_id(i, cta, P, n_items);
+      AtItem it;
+      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+      const int nq = it.t1 - it.t0 + 1;
+      const int n_mt = (nq * G > 128) ? 2 : 1;
+      int nt;
+      const int* si = nullptr;
+      if (SPARSE) {
+        // ---- stage the support row's index list; per-tile flags; number of useful tiles ----
+        const int ib = n_it & 1, iu = n_it >> 1;
+        if (iu > 0) mbar_wait(&bar.idxempty[ib], (iu - 1) & 1);
+        int* siw = sIdx + ib * kpad;
+        uint32_t* fl = sFlag + ib * ntmax;
+        for (int t = ptid; t < ntmax; t += 128) fl[t] = 0u;
+        if (ptid == 0) n_eff_sh[ib] = 0;
+        loader_bar_sync();
+        const int32_t* sup = idx + (size_t)it.row * k;
+        const int qa0 = it.seq_start + it.t0, qa1 = qa0 + 128 / G, plast = it.seq_start + it.t1;
+        int my_last = 0;
+        for (int e = ptid; e < kpad; e += 128) {
+          const int p = e < k ? __ldg(sup + e) : -1;
+          const bool ok = p >= it.seq_start && p <= plast;
+          siw[e] = ok ? p : -1;
+          uint32_t f = 0;
+          if (!ok || p > qa0 - win) f |= 1u;
+          if (!ok || p > qa1 - win) f |= 2u;
+          if (ok) my_last = e + 1;
+          if (f) atomicOr(&fl[e / AT_KT], f);
         }
-        pos[i] = p;
+        if (my_last) atomicMax(&n_eff_sh[ib], my_last);
+        loader_bar_sync();
+        nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
+        mbar_arrive(&bar.idxfull[ib]);
+        si = siw;
+      } else {
+        nt = it.t1 / AT_KT + 1;
       }
-      if (u > 0) mbar_wait(&bar.kempty[s], (u - 1) & 1);
+      ++n_it;
+      if (nt == 0) continue;
+      const __nv_bfloat16* Kh = K + (size_t)it.kvh * D + c * 8;
+      const __nv_bfloat16* Vh = V + (size_t)it.kvh * D + c * 8;
+      const size_t rstride = (size_t)Hkv * D;
+      auto load_tile = [&](int j) {
+        const uint32_t gj = gk + j;
+        const int s = gj % NS;
+        const uint32_t u = gj / NS;
+        size_t off[PASSES];
 #pragma unroll
-      for (int i = 0; i < PASSES; ++i) {
-        const int key = key0 + i * KPP;
-        cp_async16(smem_u32(sK + s * KV_TILE + (c / 8) * KV_BLK) + sw128_offset(key, c % 8),
-                   K + ((size_t)pos[i] * Hkv + kvh) * D + c * 8);
-      }
-      cp_async_arrive_noinc(&bar.kfull[s]);
-      if (WITH_O) {
-        if (u > 0) mbar_wait(&bar.vempty[s], (u - 1) & 1);
-#pragma unroll
-        for (int i = 0; i < PASSES; ++i) {
-          const int key = key0 + i * KPP;
-          cp_async16(smem_u32(sV + s * KV_TILE + (c / 8) * KV_BLK) + sw128_offset(key, c % 8),
-                     V + ((size_t)pos[i] * Hkv + kvh) * D + c * 8);
+        for (int pi = 0; pi < PASSES; ++pi) {
+          const int col = j * AT_KT + key0 + pi * KPP;
+          int p;
+          if (SPARSE) {
+            p = si[col];
+            if (p < 0) p = it.seq_start;  // masked later; any valid row will do
+          } else {
+            p = it.seq_start + min(col, it.t1);
+          }
+          off[pi] = (size_t)p * rstride;
         }
-        cp_async_arrive_noinc(&bar.vfull[s]);
+        if (u > 0) mbar_wait(&bar.kempty[s], (u - 1) & 1);
+        const uint32_t kdst = smem_u32(sK + s * KV_TILE) + kv_off;
+#pragma unroll
+        for (int pi = 0; pi < PASSES; ++pi)
+          cp_async16(kdst + sw128_offset(key0 + pi * KPP, c % 8), Kh + off[pi]);
+        cp_async_arrive_noinc(&bar.kfull[s]);
+        if (WITH_O) {
+          if (u > 0) mbar_wait(&bar.vempty[s], (u - 1) & 1);
+          const uint32_t vdst = smem_u32(sV + s * KV_TILE) + kv_off;
+#pragma unroll
+          for (int pi = 0; pi < PASSES; ++pi)
+            cp_async16(vdst + sw128_offset(key0 + pi * KPP, c % 8), Vh + off[pi]);
+          cp_async_arrive_noinc(&bar.vfull[s]);
+        }
+      };
+      // The first tiles only need ring slots whose MMAs were issued before the previous item's last S MMA, so they
+      // are prefetched BEFORE waiting for the Q buffer (released by that last S MMA).
+      const int pre = min(nt, NS - 2);
+      for (int j = 0; j < pre; ++j) load_tile(j);
+      {  // Q tile: row R = query * G + head; rows past the chunk repeat its last query (outputs never written)
+        if (n_q > 0) mbar_wait(&bar.qempty, (n_q - 1) & 1);
+        for (int e = ptid; e < n_mt * 128 * CPR; e += 128) {
+          const int R = e / CPR, cc = e % CPR;
+          const int ql = min(R / G, nq - 1), h = R % G;
+          const __nv_bfloat16* src = Q + ((size_t)(it.seq_start + it.t0 + ql) * Hq + it.kvh * G + h) * D + cc * 8;
+          cp_async16(smem_u32(sQ + (cc / 8) * Q_BLK) + sw128_offset(R, cc % 8), src);
+        }
+        cp_async_arrive_noinc(&bar.qfull);
+        ++n_q;
       }
+      for (int j = pre; j < nt; ++j) load_tile(j);
+      gk += nt;
     }
     cp_async_wait<0>();
   } else if (warp == AT_MMA_WARP) {
     // =========================================== MMA issuer ===========================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
     if (lane == 0) {
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, AT_KT, 0, 0);  // S = Q K^T : both K-major
-      constexpr uint32_t idesc_o = umma_idesc_bf16(128, D, 0, 1);      // O += P V : V is MN-major
-      mbar_wait(&bar.qfull, 0);
-      tc_fence_after_sync();
-      const uint32_t q_addr = smem_u32(sQ), k_addr = smem_u32(sK), v_addr = smem_u32(sV), p_addr = smem_u32(sP);
-      auto issue_s = [&](int j) {
-        const int s = j % AT_STAGES;
-        mbar_wait(&bar.kfull[s], (j / AT_STAGES) & 1);
+      constexpr uint32_t idesc_o = umma_idesc_bf16(128, D, 0, 1);      // O += P V : P from TMEM, V MN-major
+      const uint32_t q_addr = smem_u32(sQ), k_addr = smem_u32(sK), v_addr = smem_u32(sV);
+      uint32_t gk = 0, n_q = 0, n_it = 0;
+      uint32_t cs[2] = {0, 0}, cp[2] = {0, 0}, n_o[2] = {0, 0};
+      for (int i = 0; i * P < n_items; ++i) {
+        const int id = at_item_id(i, cta, P, n_items);
+        AtItem it;
+        if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+        const int nq = it.t1 - it.t0 + 1;
+        const int n_mt = (nq * G > 128) ? 2 : 1;
+        int nt, nt_mt[2];
+        if (SPARSE) {
+          const int ib = n_it & 1, iu = n_it >> 1;
+          mbar_wait(&bar.idxfull[ib], iu & 1);
+          nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
+          nt_mt[0] = nt_mt[1] = nt;
+        } else {
+          nt = it.t1 / AT_KT + 1;
+          nt_mt[0] = min(it.t0 + 128 / G - 1, it.t1) / AT_KT + 1;
+          nt_mt[1] = nt;
+        }
+        ++n_it;
+        if (nt == 0) continue;
+        mbar_wait(&bar.qfull, n_q & 1);
+        fence_proxy_async_smem();
         tc_fence_after_sync();
-        for (int mt = 0; mt < n_mt; ++mt) {
-          if (j >= nt_mt[mt]) continue;
-          const int b = j & 1, n = j >> 1;
-          if (n > 0) {
-            mbar_wait(&bar.sempty[mt][b], (n - 1) & 1);
-            tc_fence_after_sync();
-          }
-#pragma unroll
-          for (int kk = 0; kk < D / 16; ++kk) {
-            const uint64_t ad = umma_desc_sw128(q_addr + (kk / 4) * Q_BLK + mt * 16384 + (kk % 4) * 32, 16, 1024);
-            const uint64_t bd = umma_desc_sw128(k_addr + s * KV_TILE + (kk / 4) * KV_BLK + (kk % 4) * 32, 16, 1024);
-            umma_ss(tmem + TM_S + mt * 128 + b * 64, ad, bd, idesc_s, kk != 0);
-          }
-          umma_commit(&bar.sfull[mt][b]);
-        }
-        umma_commit(&bar.kempty[s]);
-      };
-      auto issue_pv = [&](int j) {
-        const int s = j % AT_STAGES;
-        mbar_wait(&bar.vfull[s], (j / AT_STAGES) & 1);
-        for (int mt = 0; mt < n_mt; ++mt) {
-          if (j >= nt_mt[mt]) continue;
-          mbar_wait(&bar.pfull[mt], j & 1);
+        auto issue_s = [&](int j) {
+          const int s = (gk + j) % NS;
+          mbar_wait(&bar.kfull[s], ((gk + j) / NS) & 1);
+          fence_proxy_async_smem();
           tc_fence_after_sync();
+          for (int mt = 0; mt < n_mt; ++mt) {
+            if (j >= nt_mt[mt]) continue;
+            const uint32_t b = cs[mt] & 1, n = cs[mt] >> 1;
+            if (!WITH_O && n > 0) {  // with PV the buffer is released by the (ordered) PV that consumed its P
+              mbar_wait(&bar.sdone[mt][b], (n - 1) & 1);
+              tc_fence_after_sync();
+            }
 #pragma unroll
-          for (int kk = 0; kk < AT_KT / 16; ++kk) {
-            const uint64_t ad = umma_desc_sw128(p_addr + mt * P_TILE + kk * 32, 16, 1024);
-            const uint64_t bd = umma_desc_sw128(v_addr + s * KV_TILE + kk * 2048, KV_BLK, 1024);
-            umma_ss(tmem + TM_O + mt * 128, ad, bd, idesc_o, (j | kk) != 0);
+            for (int kk = 0; kk < D / 16; ++kk) {
+              const uint64_t ad = umma_desc_sw128(q_addr + (kk / 4) * Q_BLK + mt * 16384 + (kk % 4) * 32, 16, 1024);
+              const uint64_t bd = umma_desc_sw128(k_addr + s * KV_TILE + (kk / 4) * KV_BLK + (kk % 4) * 32, 16, 1024);
+              umma_ss(tmem + TM_S + mt * 128 + b * 64, ad, bd, idesc_s, kk != 0);
+            }
+            umma_commit(&bar.sfull[mt][b]);
+            ++cs[mt];
           }
-          umma_commit(&bar.pempty[mt]);
+          umma_commit(&bar.kempty[s]);
+        };
+        auto issue_pv = [&](int j) {
+          const int s = (gk + j) % NS;
+          mbar_wait(&bar.vfull[s], ((gk + j) / NS) & 1);
+          fence_proxy_async_smem();
+          for (int mt = 0; mt < n_mt; ++mt) {
+            if (j >= nt_mt[mt]) continue;
+            const uint32_t b = cp[mt] & 1, n = cp[mt] >> 1;
+            mbar_wait(&bar.sdone[mt][b], n & 1);
+            if (j == 0 && n_o[mt] > 0) mbar_wait(&bar.oempty[mt], (n_o[mt] - 1) & 1);
+            tc_fence_after_sync();
+#pragma unroll
+            for (int kk = 0; kk < AT_KT / 16; ++kk) {
+              const uint64_t bd = umma_desc_sw128(v_addr + s * KV_TILE + kk * 2048, KV_BLK, 1024);
+              umma_ts(tmem + TM_O + mt * D, tmem + TM_S + mt * 128 + b * 64 + kk * 8, bd, idesc_o, (j | kk) != 0);
+            }
+            umma_commit(&bar.ofull[mt]);
+            if (j == nt_mt[mt] - 1) umma_commit(&bar.ofin[mt]);
+            ++cp[mt];
+          }
+          umma_commit(&bar.vempty[s]);
+        };
+        issue_s(0);
+        for (int j = 0; j < nt; ++j) {
+          if (j + 1 < nt) issue_s(j + 1);
+          else umma_commit(&bar.qempty);  // every S MMA of the item has been issued: Q may be overwritten when they finish
+          if (WITH_O) issue_pv(j);
         }
-        umma_commit(&bar.vempty[s]);
-      };
-      issue_s(0);
-      for (int j = 0; j < nt; ++j) {
-        if (j + 1 < nt) issue_s(j + 1);
-        if (WITH_O) issue_pv(j);
+        if (WITH_O) {
+          for (int mt = 0; mt < n_mt; ++mt) ++n_o[mt];
+        } else {
+          for (int mt = 0; mt < n_mt; ++mt) cp[mt] = cs[mt];
+        }
+        ++n_q;
+        gk += nt;
       }
     }
     __syncwarp();
-  } else if (warp / 4 < n_mt) {
+  } else {
     // =========================================== softmax ===========================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
     const int mt = warp / 4;
     const int r = (warp % 4) * 32 + lane;  // row inside the M tile == TMEM lane
     const int R = mt * 128 + r;
     const int ql = R / G, h = R % G;
-    const bool row_valid = ql < nq;
-    const int tl = t0 + min(ql, nq - 1);  // local query position of this row
-    const int tp = seq_start + tl;        // packed
     const uint32_t lane_base = (uint32_t)((warp % 4) * 32) << 16;
-    const uint32_t t_s = tmem + lane_base + TM_S + mt * 128;
-    const uint32_t t_o = tmem + lane_base + TM_O + mt * 128;
-    const int qa_local = t0 + mt * (128 / G);
-    float m_run = -INFINITY, l_run = 0.f;
-    const int my_nt = nt_mt[mt];
-    for (int j = 0; j < my_nt; ++j) {
-      const int b = j & 1;
-      mbar_wait(&bar.sfull[mt][b], (j >> 1) & 1);
-      tc_fence_after_sync();
-      uint32_t v[AT_KT];
-      tmem_ld_x32(t_s + b * 64, v);
-      tmem_ld_x32(t_s + b * 64 + 32, v + 32);
-      tmem_ld_wait();
-      tc_fence_before_sync();
-      mbar_arrive(&bar.sempty[mt][b]);
-
-      bool flagged;
-      if (SPARSE) flagged = ((flags[j] >> mt) & 1u) != 0;
-      else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
-      flagged = flagged || !scale_pos;
-      float mx;
-      if (!flagged) {
-        float a = __uint_as_float(v[0]);
-#pragma unroll
-        for (int cc = 1; cc < AT_KT; ++cc) a = fmaxf(a, __uint_as_float(v[cc]));
-        mx = a * sl2;
+    const uint32_t t_o = tmem + lane_base + TM_O + mt * D;
+    const uint64_t sl2_2 = f2_pack(sl2, sl2);
+    uint32_t cs = 0, n_it = 0, n_ep = 0;  // S tiles consumed by this M tile (== PVs issued for it), items seen, epilogues
+    for (int i = 0; i * P < n_items; ++i) {
+      const int id = at_item_id(i, cta, P, n_items);
+      AtItem it;
+      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+      const int nq = it.t1 - it.t0 + 1;
+      const int n_mt = (nq * G > 128) ? 2 : 1;
+      int my_nt;
+      const int ib = n_it & 1;
+      const int* si = sIdx + ib * kpad;
+      const uint32_t* fl = sFlag + ib * ntmax;
+      if (SPARSE) {
+        mbar_wait(&bar.idxfull[ib], (n_it >> 1) & 1);
+        my_nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
       } else {
-        mx = -INFINITY;
-#pragma unroll
-        for (int cc = 0; cc < AT_KT; ++cc) {
-          const int col = j * AT_KT + cc;
-          bool ok;
-          int dist;
-          if (SPARSE) {
-            const int p = col < k ? __ldg(sup + col) : -1;
-            ok = p >= seq_start && p <= tp;
-            dist = tp - p;
-          } else {
-            ok = col <= tl;
-            dist = tl - col;
-          }
-          float x = -INFINITY;
-          if (ok) x = fmaf(__uint_as_float(v[cc]), sl2, (win > 0 && dist < win) ? lb2 : 0.f);
-          v[cc] = __float_as_uint(x);  // already scaled
-          mx = fmaxf(mx, x);
-        }
+        my_nt = (mt == 0 ? min(it.t0 + 128 / G - 1, it.t1) : it.t1) / AT_KT + 1;
       }
-      // ---- running max with lazy rescale of the TMEM accumulator ----
-      const float m_new = fmaxf(m_run, mx);
-      const bool need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
-      bool waited_pv = false;
-      if (__any_sync(0xffffffffu, need)) {
-        const float f = need ? exp2f(m_run - m_new) : 1.f;  // m_run = -inf -> 0
-        if (WITH_O && j > 0) {
-          mbar_wait(&bar.pempty[mt], (j - 1) & 1);  // PV(j-1) has finished updating O
+      ++n_it;
+      const bool row_valid = ql < nq;
+      const int tl = it.t0 + min(ql, nq - 1);  // local query position of this row
+      const int tp = it.seq_start + tl;        // packed
+      const size_t orow = ((size_t)tp * Hq + it.kvh * G + h);
+      const int qa_local = it.t0 + mt * (128 / G);
+
+      if (mt < n_mt && my_nt > 0) {
+        float m_run = -INFINITY, l_run = 0.f;
+        for (int j = 0; j < my_nt; ++j, ++cs) {
+          const uint32_t b = cs & 1;
+          const uint32_t t_s = tmem + lane_base + TM_S + mt * 128 + b * 64;
+          mbar_wait(&bar.sfull[mt][b], (cs >> 1) & 1);
           tc_fence_after_sync();
-          waited_pv = true;
+          uint32_t v[AT_KT];
+          tmem_ld_x32(t_s, v);
+          tmem_ld_x32(t_s + 32, v + 32);
+          tmem_ld_wait();
+
+          bool flagged;
+          if (SPARSE) flagged = ((fl[j] >> mt) & 1u) != 0;
+          else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
+          flagged = flagged || !scale_pos;
+          float mx;
+          if (!flagged) {
+            float a0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1]));
+            float a1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
+            float a2 = fmaxf(__uint_as_float(v[4]), __uint_as_float(v[5]));
+            float a3 = fmaxf(__uint_as_float(v[6]), __uint_as_float(v[7]));
+#pragma unroll
+            for (int cc = 8; cc < AT_KT; cc += 8) {
+              a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
+              a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
+              a2 = fmaxf(a2, fmaxf(__uint_as_float(v[cc + 4]), __uint_as_float(v[cc + 5])));
+              a3 = fmaxf(a3, fmaxf(__uint_as_float(v[cc + 6]), __uint_as_float(v[cc + 7])));
+            }
+            mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
+          } else {
+            mx = -INFINITY;
+#pragma unroll
+            for (int cc = 0; cc < AT_KT; ++cc) {
+              const int col = j * AT_KT + cc;
+              bool ok;
+              int dist;
+              if (SPARSE) {
+                const int p = si[col];
+                ok = p >= 0 && p <= tp;
+                dist = tp - p;
+              } else {
+                ok = col <= tl;
+                dist = tl - col;
+              }
+              float x = -INFINITY;
+              if (ok) x = fmaf(__uint_as_float(v[cc]), sl2, (win > 0 && dist < win) ? lb2 : 0.f);
+              v[cc] = __float_as_uint(x);  // already scaled
+              mx = fmaxf(mx, x);
+            }
+          }
+          // ---- running max with lazy rescale of the TMEM accumulator ----
+          const float m_new = fmaxf(m_run, mx);
+          const bool need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
+          if (__any_sync(0xffffffffu, need)) {
+            const float f = need ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
+            if (WITH_O && j > 0) {
+              mbar_wait(&bar.ofull[mt], (cs - 1) & 1);  // PV(j-1) has finished updating O
+              tc_fence_after_sync();
+#pragma unroll
+              for (int c0 = 0; c0 < D; c0 += 32) {
+                uint32_t o[32];
+                tmem_ld_x32(t_o + c0, o);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 32; ++q) o[q] = __float_as_uint(__uint_as_float(o[q]) * f);
+                tmem_st_x32(t_o + c0, o);
+              }
+              tmem_st_wait();
+            }
+            l_run *= f;
+            if (need) m_run = m_new;
+          }
+          const float m_off = (m_run == -INFINITY) ? 0.f : m_run;
+          uint32_t pk[AT_KT / 2];
+          uint64_t sum2 = 0ull;
+          if (!flagged) {
+            const uint64_t nm2 = f2_pack(-m_off, -m_off);
+#pragma unroll
+            for (int cc = 0; cc < AT_KT; cc += 2) {
+              float x0, x1;
+              f2_unpack(f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2), x0, x1);
+              const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+              sum2 = f2_add(sum2, f2_pack(p0, p1));
+              pk[cc / 2] = bf16x2_rn(p0, p1);
+            }
+          } else {
+#pragma unroll
+            for (int cc = 0; cc < AT_KT; cc += 2) {
+              const float p0 = ex2_approx(__uint_as_float(v[cc]) - m_off);
+              const float p1 = ex2_approx(__uint_as_float(v[cc + 1]) - m_off);
+              sum2 = f2_add(sum2, f2_pack(p0, p1));
+              pk[cc / 2] = bf16x2_rn(p0, p1);
+            }
+          }
+          {
+            float s0, s1;
+            f2_unpack(sum2, s0, s1);
+            l_run += s0 + s1;
+          }
+          if (WITH_O) {
+            tmem_st_x32(t_s, pk);  // P (64 keys as 32 bf16x2 columns) over the first half of S
+            tmem_st_wait();
+          }
+          tc_fence_before_sync();
+          mbar_arrive(&bar.sdone[mt][b]);
+        }
+        // ---- epilogue ----
+        if (WITH_O) {
+          mbar_wait(&bar.ofin[mt], n_ep & 1);
+          ++n_ep;
+          tc_fence_after_sync();
+          const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
 #pragma unroll
           for (int c0 = 0; c0 < D; c0 += 32) {
             uint32_t o[32];
             tmem_ld_x32(t_o + c0, o);
             tmem_ld_wait();
+            if (c0 + 32 == D) {  // O is in registers: the next item's first PV may overwrite the accumulator
+              tc_fence_before_sync();
+              mbar_arrive(&bar.oempty[mt]);
+            }
+            if (row_valid) {
 #pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-            tmem_st_x32(t_o + c0, o);
-          }
-          tmem_st_wait();
-        }
-        l_run *= f;
-        if (need) m_run = m_new;
-      }
-      const float m_off = (m_run == -INFINITY) ? 0.f : m_run;
-      float sum = 0.f;
-      uint32_t pk[AT_KT / 2];
-      if (!flagged) {
-#pragma unroll
-        for (int cc = 0; cc < AT_KT; cc += 2) {
-          const float p0 = exp2f(fmaf(__uint_as_float(v[cc]), sl2, -m_off));
-          const float p1 = exp2f(fmaf(__uint_as_float(v[cc + 1]), sl2, -m_off));
-          sum += p0 + p1;
-          pk[cc / 2] = sp_pack_bf16(p0, p1);
-        }
-      } else {
-#pragma unroll
-        for (int cc = 0; cc < AT_KT; cc += 2) {
-          const float p0 = exp2f(__uint_as_float(v[cc]) - m_off);
-          const float p1 = exp2f(__uint_as_float(v[cc + 1]) - m_off);
-          sum += p0 + p1;
-          pk[cc / 2] = sp_pack_bf16(p0, p1);
-        }
-      }
-      l_run += sum;
-      if (WITH_O) {
-        if (j > 0 && !waited_pv) mbar_wait(&bar.pempty[mt], (j - 1) & 1);  // PV(j-1) no longer reads P
-        uint8_t* prow = sP + mt * P_TILE;
-#pragma unroll
-        for (int c8 = 0; c8 < 8; ++c8) {
-          const uint4 w = make_uint4(pk[4 * c8], pk[4 * c8 + 1], pk[4 * c8 + 2], pk[4 * c8 + 3]);
-          *reinterpret_cast<uint4*>(prow + sw128_offset(r, c8)) = w;
-        }
-        fence_proxy_async_smem();
-        tc_fence_before_sync();
-        mbar_arrive(&bar.pfull[mt]);
-      }
-    }
-    // ---- epilogue ----
-    const size_t orow = ((size_t)tp * Hq + kvh * G + h);
-    if (WITH_O) {
-      mbar_wait(&bar.pempty[mt], (my_nt - 1) & 1);
-      tc_fence_after_sync();
-      const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
-#pragma unroll
-      for (int c0 = 0; c0 < D; c0 += 32) {
-        uint32_t o[32];
-        tmem_ld_x32(t_o + c0, o);
-        tmem_ld_wait();
-        if (row_valid) {
-#pragma unroll
-          for (int i = 0; i < 32; i += 8) {
-            uint4 w;
-            w.x = sp_pack_bf16(__uint_as_float(o[i]) * inv, __uint_as_float(o[i + 1]) * inv);
-            w.y = sp_pack_bf16(__uint_as_float(o[i + 2]) * inv, __uint_as_float(o[i + 3]) * inv);
-            w.z = sp_pack_bf16(__uint_as_float(o[i + 4]) * inv, __uint_as_float(o[i + 5]) * inv);
-            w.w = sp_pack_bf16(__uint_as_float(o[i + 6]) * inv, __uint_as_float(o[i + 7]) * inv);
-            *reinterpret_cast<uint4*>(O + orow * D + c0 + i) = w;
+              for (int q = 0; q < 32; q += 8) {
+                uint4 w;
+                w.x = bf16x2_rn(__uint_as_float(o[q]) * inv, __uint_as_float(o[q + 1]) * inv);
+                w.y = bf16x2_rn(__uint_as_float(o[q + 2]) * inv, __uint_as_float(o[q + 3]) * inv);
+                w.z = bf16x2_rn(__uint_as_float(o[q + 4]) * inv, __uint_as_float(o[q + 5]) * inv);
+                w.w = bf16x2_rn(__uint_as_float(o[q + 6]) * inv, __uint_as_float(o[q + 7]) * inv);
+                *reinterpret_cast<uint4*>(O + orow * D + c0 + q) = w;
+              }
+            }
           }
         }
+        if (lse != nullptr && row_valid) lse[orow] = l_run > 0.f ? (m_run + log2f(l_run)) * SP_LN2 : -INFINITY;
+      } else if (my_nt == 0 && row_valid) {  // empty support: O = 0, lse = -inf (reading A9)
+        if (WITH_O) {
+          const uint4 z = make_uint4(0, 0, 0, 0);
+          for (int cc = 0; cc < CPR; ++cc) reinterpret_cast<uint4*>(O + orow * D)[cc] = z;
+        }
+        if (lse) lse[orow] = -INFINITY;
       }
+      if (SPARSE) mbar_arrive(&bar.idxempty[ib]);
     }
-    if (lse != nullptr && row_valid) lse[orow] = l_run > 0.f ? (m_run + log2f(l_run)) * SP_LN2 : -INFINITY;
   }
   tc_fence_before_sync();
   __syncthreads();
@@ -418,16 +573,39 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
 }
 
 template <int D>
-size_t attn_smem_bytes(int k, bool sparse) {
+size_t attn_smem_bytes(int kpad, bool sparse, bool with_o, int stages) {
   const size_t kb = D / 64;
-  return kb * 256 * 128 + 2 * AT_STAGES * kb * AT_KT * 128 + 2 * 128 * 128 + (sparse ? 4 * (size_t)((k + AT_KT - 1) / AT_KT) : 0) +
-         16 + 1024;
+  return 1024 + kb * 256 * 128 + (size_t)stages * (with_o ? 2 : 1) * kb * AT_KT * 128 +
+         (sparse ? (size_t)2 * kpad * 4 + (size_t)2 * (kpad / AT_KT) * 4 : 0);
+}
+
+constexpr size_t AT_SMEM_LIMIT = 227 * 1024 - 512;  // dynamic limit minus the static barriers / slots
+
+template <int D>
+int attn_pick_stages(int kpad, bool sparse, bool with_o) {
+  int s = AT_MAX_STAGES;
+  while (s >= 2 && attn_smem_bytes<D>(kpad, sparse, with_o, s) > AT_SMEM_LIMIT) --s;
+  return s;  // < 2 -> unsupported
+}
+
+int at_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
 }
 
 template <int D, int G, bool SPARSE, bool WITH_O>
-cudaError_t launch_one(const SpGeom& g, dim3 grid, size_t smem, cudaStream_t st, const void* Q, const void* K,
-                       const void* V, const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, void* O,
-                       float* lse) {
+cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
+                       const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks,
+                       int n_items, void* O, float* lse) {
+  const int kpad = SPARSE ? (k + AT_KT - 1) / AT_KT * AT_KT : 0;
+  const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O);
+  if (stages < 2) return cudaErrorInvalidValue;
+  const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages);
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
     cudaError_t e = cudaFuncSetAttribute(sp_tc_attn_kernel<D, G, SPARSE, WITH_O>,
@@ -435,34 +613,34 @@ cudaError_t launch_one(const SpGeom& g, dim3 grid, size_t smem, cudaStream_t st,
     if (e != cudaSuccess) return e;
     attr_smem = smem;
   }
+  const int grid = n_items < at_sm_count() ? n_items : at_sm_count();
   sp_tc_attn_kernel<D, G, SPARSE, WITH_O><<<grid, AT_THREADS, smem, st>>>(
       g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, cpr,
-      (__nv_bfloat16*)O, lse);
+      n_chunks, n_items, stages, kpad, (__nv_bfloat16*)O, lse);
   return cudaGetLastError();
 }
 
 template <int D, int G>
-cudaError_t launch_dg(const SpGeom& g, dim3 grid, cudaStream_t st, const void* Q, const void* K, const void* V,
-                      const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, void* O, float* lse) {
-  const bool sparse = idx != nullptr;
-  const size_t smem = attn_smem_bytes<D>(k, sparse);
-  if (smem > 227 * 1024) return cudaErrorInvalidValue;
-  if (sparse) {
-    if (O) return launch_one<D, G, true, true>(g, grid, smem, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
-    return launch_one<D, G, true, false>(g, grid, smem, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
+cudaError_t launch_dg(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V, const int32_t* idx,
+                      int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks, int n_items, void* O,
+                      float* lse) {
+  if (idx != nullptr) {
+    if (O) return launch_one<D, G, true, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    return launch_one<D, G, true, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
   }
-  if (O) return launch_one<D, G, false, true>(g, grid, smem, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
-  return launch_one<D, G, false, false>(g, grid, smem, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
+  if (O) return launch_one<D, G, false, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+  return launch_one<D, G, false, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
 }
 
 template <int D>
-cudaError_t launch_d(int G, const SpGeom& g, dim3 grid, cudaStream_t st, const void* Q, const void* K, const void* V,
-                     const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, void* O, float* lse) {
+cudaError_t launch_d(int G, const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
+                     const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks,
+                     int n_items, void* O, float* lse) {
   switch (G) {
-    case 1: return launch_dg<D, 1>(g, grid, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
-    case 2: return launch_dg<D, 2>(g, grid, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
-    case 4: return launch_dg<D, 4>(g, grid, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
-    case 8: return launch_dg<D, 8>(g, grid, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, O, lse);
+    case 1: return launch_dg<D, 1>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    case 2: return launch_dg<D, 2>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    case 4: return launch_dg<D, 4>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    case 8: return launch_dg<D, 8>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
   }
   return cudaErrorInvalidValue;
 }
@@ -471,10 +649,11 @@ cudaError_t launch_d(int G, const SpGeom& g, dim3 grid, cudaStream_t st, const v
 
 // The tcgen05 attention covers dense attention always and sparse attention when a support row's queries fill a
 // useful part of an M tile; per-query (b_sel == 1) supports are gather-bound and stay on the CUDA-core kernel.
-bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k) {
+bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d) {
   if (!sparse) return true;
   if (b_sel * G < 32) return false;
-  return 4 * (size_t)((k + AT_KT - 1) / AT_KT) <= 16 * 1024;
+  const int kpad = (k + AT_KT - 1) / AT_KT * AT_KT;
+  return (d == 128 ? attn_pick_stages<128>(kpad, true, true) : attn_pick_stages<64>(kpad, true, true)) >= 2;
 }
 
 // idx == nullptr -> dense causal attention over the whole pack.  n_chunks_dense = sum_i ceil(n_i / (256/G)).
@@ -487,9 +666,12 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
   const int cpr = sparse ? (g.b_sel + QT - 1) / QT : 1;
   const long long nx = sparse ? n_rows * cpr : n_chunks_dense;
   if (nx <= 0) return cudaSuccess;
-  dim3 grid((unsigned)nx, (unsigned)Hkv);
-  cudaError_t e = d == 128 ? launch_d<128>(G, g, grid, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr, O, lse)
-                           : launch_d<64>(G, g, grid, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr, O, lse);
+  if (nx * Hkv > 0x7fffffffLL) return cudaErrorInvalidValue;
+  const int n_items = (int)(nx * Hkv);
+  cudaError_t e = d == 128 ? launch_d<128>(G, g, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr,
+                                           (int)nx, n_items, O, lse)
+                           : launch_d<64>(G, g, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr,
+                                          (int)nx, n_items, O, lse);
   sp_count_launch();
   return e;
 }

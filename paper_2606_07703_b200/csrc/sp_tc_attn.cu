@@ -33,6 +33,11 @@ constexpr float AT_RESCALE_THRESHOLD = 8.0f;  // log2 units: O is rescaled only 
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t* bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void loader_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 // D[tmem] (+)= A[tmem] * B[smem]: A = 128 lanes x (K/2) 32-bit columns of packed bf16 pairs (K-major).
@@ -298,12 +303,20 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     cp_async_wait<0>();
   } else if (warp == AT_MMA_WARP) {
     // =========================================== MMA issuer ===========================================
+    // The whole warp runs the (warp-uniform) control flow and the mbarrier waits; one elected lane issues every
+    // tcgen05.mma / tcgen05.commit.  Descriptors are a precomputed base plus a compile-time offset, ring stages
+    // and phases are tracked incrementally: the issue path must stay well under the ~40 cycles one MMA occupies
+    // the tensor pipe.
     asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
-    if (lane == 0) {
+    {
+      const bool leader = elect_one();
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, AT_KT, 0, 0);  // S = Q K^T : both K-major
       constexpr uint32_t idesc_o = umma_idesc_bf16(128, D, 0, 1);      // O += P V : P from TMEM, V MN-major
-      const uint32_t q_addr = smem_u32(sQ), k_addr = smem_u32(sK), v_addr = smem_u32(sV);
-      uint32_t gk = 0, n_q = 0, n_it = 0;
+      const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ), 16, 1024);
+      const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
+      const uint64_t vdesc0 = umma_desc_sw128(smem_u32(sV), KV_BLK, 1024);
+      uint32_t k_s = 0, k_ph = 0, v_s = 0, v_ph = 0;  // K / V ring positions of the next tile to consume
+      uint32_t n_q = 0, n_it = 0;
       uint32_t cs[2] = {0, 0}, cp[2] = {0, 0}, n_o[2] = {0, 0};
       for (int i = 0; i * P < n_items; ++i) {
         const int id = at_item_id(i, cta, P, n_items);
@@ -328,53 +341,67 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
         fence_proxy_async_smem();
         tc_fence_after_sync();
         auto issue_s = [&](int j) {
-          const int s = (gk + j) % NS;
-          mbar_wait(&bar.kfull[s], ((gk + j) / NS) & 1);
+          mbar_wait(&bar.kfull[k_s], k_ph);
           fence_proxy_async_smem();
           tc_fence_after_sync();
-          for (int mt = 0; mt < n_mt; ++mt) {
-            if (j >= nt_mt[mt]) continue;
+          const uint64_t kd = kdesc0 + (uint64_t)((k_s * KV_TILE) >> 4);
+#pragma unroll
+          for (int mt = 0; mt < 2; ++mt) {
+            if (mt >= n_mt || j >= nt_mt[mt]) continue;
             const uint32_t b = cs[mt] & 1, n = cs[mt] >> 1;
             if (!WITH_O && n > 0) {  // with PV the buffer is released by the (ordered) PV that consumed its P
               mbar_wait(&bar.sdone[mt][b], (n - 1) & 1);
               tc_fence_after_sync();
             }
+            if (leader) {
+              const uint32_t d_s = tmem + TM_S + mt * 128 + b * 64;
+              const uint64_t qd = qdesc0 + (uint64_t)((mt * 16384) >> 4);
 #pragma unroll
-            for (int kk = 0; kk < D / 16; ++kk) {
-              const uint64_t ad = umma_desc_sw128(q_addr + (kk / 4) * Q_BLK + mt * 16384 + (kk % 4) * 32, 16, 1024);
-              const uint64_t bd = umma_desc_sw128(k_addr + s * KV_TILE + (kk / 4) * KV_BLK + (kk % 4) * 32, 16, 1024);
-              umma_ss(tmem + TM_S + mt * 128 + b * 64, ad, bd, idesc_s, kk != 0);
+              for (int kk = 0; kk < D / 16; ++kk) {
+                umma_ss(d_s, qd + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
+                        kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
+              }
+              umma_commit(&bar.sfull[mt][b]);
             }
-            umma_commit(&bar.sfull[mt][b]);
             ++cs[mt];
           }
-          umma_commit(&bar.kempty[s]);
+          if (leader) umma_commit(&bar.kempty[k_s]);
+          if (++k_s == (uint32_t)NS) {
+            k_s = 0;
+            k_ph ^= 1;
+          }
         };
         auto issue_pv = [&](int j) {
-          const int s = (gk + j) % NS;
-          mbar_wait(&bar.vfull[s], ((gk + j) / NS) & 1);
+          mbar_wait(&bar.vfull[v_s], v_ph);
           fence_proxy_async_smem();
-          for (int mt = 0; mt < n_mt; ++mt) {
-            if (j >= nt_mt[mt]) continue;
+          const uint64_t vd = vdesc0 + (uint64_t)((v_s * KV_TILE) >> 4);
+#pragma unroll
+          for (int mt = 0; mt < 2; ++mt) {
+            if (mt >= n_mt || j >= nt_mt[mt]) continue;
             const uint32_t b = cp[mt] & 1, n = cp[mt] >> 1;
             mbar_wait(&bar.sdone[mt][b], n & 1);
             if (j == 0 && n_o[mt] > 0) mbar_wait(&bar.oempty[mt], (n_o[mt] - 1) & 1);
             tc_fence_after_sync();
+            if (leader) {
+              const uint32_t d_o = tmem + TM_O + mt * D, a_p = tmem + TM_S + mt * 128 + b * 64;
 #pragma unroll
-            for (int kk = 0; kk < AT_KT / 16; ++kk) {
-              const uint64_t bd = umma_desc_sw128(v_addr + s * KV_TILE + kk * 2048, KV_BLK, 1024);
-              umma_ts(tmem + TM_O + mt * D, tmem + TM_S + mt * 128 + b * 64 + kk * 8, bd, idesc_o, (j | kk) != 0);
+              for (int kk = 0; kk < AT_KT / 16; ++kk)
+                umma_ts(d_o, a_p + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_o, (j | kk) != 0);
+              umma_commit(&bar.ofull[mt]);
+              if (j == nt_mt[mt] - 1) umma_commit(&bar.ofin[mt]);
             }
-            umma_commit(&bar.ofull[mt]);
-            if (j == nt_mt[mt] - 1) umma_commit(&bar.ofin[mt]);
             ++cp[mt];
           }
-          umma_commit(&bar.vempty[s]);
+          if (leader) umma_commit(&bar.vempty[v_s]);
+          if (++v_s == (uint32_t)NS) {
+            v_s = 0;
+            v_ph ^= 1;
+          }
         };
         issue_s(0);
         for (int j = 0; j < nt; ++j) {
           if (j + 1 < nt) issue_s(j + 1);
-          else umma_commit(&bar.qempty);  // every S MMA of the item has been issued: Q may be overwritten when they finish
+          else if (leader) umma_commit(&bar.qempty);  // every S MMA of the item is issued: Q is free when they finish
           if (WITH_O) issue_pv(j);
         }
         if (WITH_O) {
@@ -383,7 +410,6 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
           for (int mt = 0; mt < n_mt; ++mt) cp[mt] = cs[mt];
         }
         ++n_q;
-        gk += nt;
       }
     }
     __syncwarp();

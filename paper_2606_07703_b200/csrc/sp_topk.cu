@@ -1,21 +1,30 @@
 // sp_topk.cu -- causal top-k of support-row scores (PAPER.md:127 TopK_s(P,k); :145 sentinel padding;
 // :156 invalid positions masked before selection).  Exact: compare/integer work only.
 //
-// One CTA per support row.  The kept set is the first min(k, n) elements of the total order
-// (score descending, index ascending), emitted in ascending index order, tail padded with -1:
-//   1. 4-pass MSB-first radix select (8 bits per pass) on an order-preserving uint32 image of the
-//      fp32 score finds the exact key T of the k-th largest element and how many elements equal
-//      to T must still be taken (`need_eq`).
-//   2. One index-ordered compaction pass keeps every element with key > T and the first `need_eq`
-//      elements with key == T  ->  ties go to the lower index, output is ascending.
-// The row is staged in shared memory when it fits (one global read), else re-read (L2 resident).
+// One CTA (1024 threads) per support row.  The kept set is the first min(k, n) elements of the total order
+// (score descending, index ascending), emitted in ascending index order, tail padded with -1.  With
+// key = order-preserving uint32 image of the fp32 score, the kept set is { key > T } plus the first `need_eq`
+// elements with key == T in index order, T = key of the k-th largest element.  Finding (T, need_eq):
+//   1. a 1024-element pseudo-random sample of the row is sorted (bitonic: shuffles inside a warp, shared memory
+//      across warps); two of its order statistics bracket T with high probability: klo <= T <= khi;
+//   2. ONE pass over the row (staged in shared memory when it fits, else re-read from L2): every warp owns a
+//      contiguous segment, counts its elements above khi and appends those inside [klo, khi] to its private
+//      candidate list (no atomics);
+//   3. if the bracket holds (count(>khi) < k <= count(>khi) + candidates, no list overflowed) T is found by a
+//      bit-by-bit bisection over the few candidates (register resident; only the bits below the common prefix
+//      of klo and khi are undecided); otherwise an exact 4-pass radix select over the whole row takes over
+//      (always correct; only slower).
+//   4. one index-ordered compaction pass; the per-warp output bases come from the candidate lists (or from a
+//      counting pass in the fallback).  Ties go to the lower index and the output is ascending by construction.
 #include "sp_common.cuh"
 
 namespace {
 
-constexpr int TOPK_THREADS = 512;
-constexpr int TOPK_WARPS = TOPK_THREADS / 32;
-constexpr int TOPK_SMEM_FLOATS = 48 * 1024;  // 192 KB row cache
+constexpr int TK_THREADS = 1024;
+constexpr int TK_WARPS = TK_THREADS / 32;
+constexpr int TK_CACHE = 40 * 1024;       // keys staged in shared memory (160 KB)
+constexpr int TK_CAND_PER_WARP = 256;     // private candidate list per warp (32 x 256 x 4 B = 32 KB)
+constexpr int TK_SAMPLE = 1024;
 
 __device__ __forceinline__ uint32_t order_key(float x) {
   uint32_t u = __float_as_uint(x);
@@ -29,24 +38,27 @@ __device__ __forceinline__ uint32_t load_key(const float* __restrict__ x, const 
   return order_key(__ldg(x + i));
 }
 
-template <bool CACHED>
-__device__ void topk_row(const float* __restrict__ x, uint32_t* keys, int n, int k, int seq_start,
-                         int32_t* __restrict__ out, uint32_t* hist, uint32_t* sh) {
-  const int tid = threadIdx.x;
-  const int lane = tid & 31, warp = tid >> 5;
+struct TkShared {
+  uint32_t hist[256];
+  uint32_t wgt[TK_WARPS], weq[TK_WARPS];  // per-warp totals (elements above khi / T; equal to T)
+  uint32_t wcand[TK_WARPS];               // per-warp candidate counts
+  uint32_t bis[34];                       // [32]: candidates above T
+  uint32_t part[2][TK_WARPS];             // bisection: per-warp partial counts, double buffered by step parity
+  uint32_t sel[2];                        // radix select scratch
+  uint32_t T, need_eq, ok;
+};
 
-  if (CACHED) {
-    for (int i = tid; i < n; i += TOPK_THREADS) keys[i] = order_key(__ldg(x + i));
-  }
-  // ---- radix select ----
-  uint32_t prefix = 0;       // high bits of T decided so far
-  uint32_t need = (uint32_t)k;  // rank still to be located inside the current prefix bucket
+// ---- exact fallback: 4-pass MSB-first radix select (8 bits per pass) -> sh.T, sh.need_eq ----
+template <bool CACHED>
+__device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, int n, int k, TkShared& sh) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t prefix = 0, need = (uint32_t)k;
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-    if (tid < 256) hist[tid] = 0;
+    if (tid < 256) sh.hist[tid] = 0;
     __syncthreads();
     const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
-    for (int i0 = 0; i0 < n; i0 += TOPK_THREADS) {
+    for (int i0 = 0; i0 < n; i0 += TK_THREADS) {
       const int i = i0 + tid;
       bool act = false;
       uint32_t bin = 0;
@@ -55,21 +67,19 @@ __device__ void topk_row(const float* __restrict__ x, uint32_t* keys, int n, int
         act = ((key & hi_mask) == prefix);
         bin = (key >> shift) & 255u;
       }
-      // warp-aggregated histogram update: scores cluster in a few high-byte bins
       const uint32_t amask = __ballot_sync(0xffffffffu, act);
       if (act) {
         const uint32_t peers = __match_any_sync(amask, bin);
-        if (lane == __ffs(peers) - 1) atomicAdd(&hist[bin], (uint32_t)__popc(peers));
+        if (lane == __ffs(peers) - 1) atomicAdd(&sh.hist[bin], (uint32_t)__popc(peers));
       }
     }
     __syncthreads();
-    // locate the bin holding rank `need` counting from the top: warp 0 scans 256 bins, 8 per lane
-    if (warp == 0) {
+    if (warp == 0) {  // locate the bin holding rank `need` counting from the top: 8 bins per lane
       uint32_t c[8];
       uint32_t tot = 0;
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        c[j] = hist[255 - (lane * 8 + j)];  // descending bin order
+        c[j] = sh.hist[255 - (lane * 8 + j)];
         tot += c[j];
       }
       uint32_t incl = tot;
@@ -78,13 +88,13 @@ __device__ void topk_row(const float* __restrict__ x, uint32_t* keys, int n, int
         const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += v;
       }
-      uint32_t before = incl - tot;  // elements in bins above this lane's 8 bins
+      uint32_t before = incl - tot;
       if (before < need && need <= incl) {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           if (need <= before + c[j]) {
-            sh[0] = 255u - (uint32_t)(lane * 8 + j);
-            sh[1] = need - before;
+            sh.sel[0] = 255u - (uint32_t)(lane * 8 + j);
+            sh.sel[1] = need - before;
             break;
           }
           before += c[j];
@@ -92,69 +102,224 @@ __device__ void topk_row(const float* __restrict__ x, uint32_t* keys, int n, int
       }
     }
     __syncthreads();
-    prefix |= sh[0] << shift;
-    need = sh[1];
+    prefix |= sh.sel[0] << shift;
+    need = sh.sel[1];
     __syncthreads();
   }
-  const uint32_t T = prefix;
-  const uint32_t need_eq = need;  // >= 1
+  if (tid == 0) {
+    sh.T = prefix;
+    sh.need_eq = need;
+  }
+  __syncthreads();
+}
 
-  // ---- index-ordered compaction ----
-  uint32_t run_gt = 0, run_eq = 0;  // totals of earlier chunks
-  uint32_t* wsum = sh + 2;          // [2 * TOPK_WARPS]
-  for (int i0 = 0; i0 < n; i0 += TOPK_THREADS) {
-    const int i = i0 + tid;
+template <bool CACHED>
+__device__ void topk_row(const float* __restrict__ x, uint32_t* keys, uint32_t* cand, int n, int k, int seq_start,
+                         int32_t* __restrict__ out, TkShared& sh) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+
+  if (CACHED) {  // stage the row once: 8 independent loads in flight per thread
+    int i = tid;
+    for (; i + 7 * TK_THREADS < n; i += 8 * TK_THREADS) {
+      float v[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) v[j] = __ldg(x + i + j * TK_THREADS);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) keys[i + j * TK_THREADS] = order_key(v[j]);
+    }
+    for (; i < n; i += TK_THREADS) keys[i] = order_key(__ldg(x + i));
+  }
+  if (tid < 34) sh.bis[tid] = 0;
+  // warp segments: contiguous, a multiple of 32 elements
+  const int seg = ((n + TK_WARPS - 1) / TK_WARPS + 31) & ~31;
+  const int seg0 = min(warp * seg, n), seg1 = min(seg0 + seg, n);
+  uint32_t* my_cand = cand + warp * TK_CAND_PER_WARP;
+
+  // ---- 1. bracket [klo, khi] from a sorted sample (short rows: everything is a candidate) ----
+  uint32_t klo = 0u, khi = 0xffffffffu;
+  if (n > TK_WARPS * TK_CAND_PER_WARP) {
+    const int stride = n / TK_SAMPLE;  // >= 8
+    uint32_t v;
+    {
+      const uint32_t h = ((uint32_t)tid * 2654435761u) >> 12;
+      const int i = tid * stride + (int)(h % (uint32_t)stride);
+      __syncthreads();  // keys staged
+      v = load_key<CACHED>(x, keys, i);
+    }
+    // bitonic sort, descending; partners closer than a warp exchange by shuffle, the others through `cand`
+    for (int size = 2; size <= TK_SAMPLE; size <<= 1) {
+      const bool desc = (tid & size) == 0;
+      for (int st = size >> 1; st > 0; st >>= 1) {
+        uint32_t pv;
+        if (st >= 32) {
+          cand[tid] = v;
+          __syncthreads();
+          pv = cand[tid ^ st];
+          __syncthreads();
+        } else {
+          pv = __shfl_xor_sync(0xffffffffu, v, st);
+        }
+        const bool keep_max = desc == ((tid & st) == 0);
+        v = keep_max ? max(v, pv) : min(v, pv);
+      }
+    }
+    cand[tid] = v;
+    __syncthreads();
+    const float frac = (float)k / (float)n;
+    const float r = frac * TK_SAMPLE;  // expected sample rank (from the top) of T
+    const int margin = (int)ceilf(3.5f * sqrtf(r * (1.f - frac))) + 4;
+    const int ih = (int)floorf(r) - margin, il = (int)ceilf(r) + margin;
+    if (ih > 0) khi = cand[ih];
+    if (il < TK_SAMPLE - 1) klo = cand[il];
+  }
+  __syncthreads();  // sample reads done before the candidate lists reuse the buffer; keys staged
+
+  // ---- 2. one pass: count above khi, collect candidates per warp ----
+  uint32_t my_gt = 0, ncand = 0;  // ncand is warp-uniform
+  for (int i0 = seg0; i0 < seg1; i0 += 32) {
+    const int i = i0 + lane;
+    bool c = false;
+    uint32_t key = 0u;
+    if (i < seg1) {
+      key = load_key<CACHED>(x, keys, i);
+      my_gt += key > khi;
+      c = key >= klo && key <= khi;
+    }
+    const uint32_t m = __ballot_sync(0xffffffffu, c);
+    if (c) {
+      const uint32_t slot = ncand + __popc(m & lt);
+      if (slot < TK_CAND_PER_WARP) my_cand[slot] = key;
+    }
+    ncand += __popc(m);
+  }
+  const uint32_t warp_gt = __reduce_add_sync(0xffffffffu, my_gt);
+  if (lane == 0) {
+    sh.wgt[warp] = warp_gt;
+    sh.wcand[warp] = ncand;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    const uint32_t tg = __reduce_add_sync(0xffffffffu, sh.wgt[lane]);
+    const uint32_t tc = __reduce_add_sync(0xffffffffu, sh.wcand[lane]);
+    const uint32_t mx = __reduce_max_sync(0xffffffffu, sh.wcand[lane]);
+    if (lane == 0) {
+      sh.ok = (mx <= TK_CAND_PER_WARP && tg < (uint32_t)k && (uint32_t)k <= tg + tc) ? 1u : 0u;
+      sh.sel[0] = tg;
+    }
+  }
+  __syncthreads();
+  uint32_t T, need_eq;
+  uint32_t base_gt, base_eq;  // selected-before counts at the start of this warp's segment
+  if (sh.ok) {
+    // ---- 3. bisection over the candidates: T = need-th largest candidate key ----
+    const uint32_t need = (uint32_t)k - sh.sel[0];
+    uint32_t ck[TK_CAND_PER_WARP / 32];
+#pragma unroll
+    for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) {
+      const uint32_t e = lane + 32 * j;
+      ck[j] = e < ncand ? my_cand[e] : 0u;  // key 0 never counts: thresholds below are >= 1 ... see note
+    }
+    // note: a padding key of 0 is only counted by the threshold 0 itself, which is never tested (bit steps OR in
+    // at least one bit)
+    // T lies in [klo, khi]: the bits above their highest differing bit are already known
+    const uint32_t diff = klo ^ khi;
+    const int top = diff ? 31 - __clz(diff) : -1;  // highest undecided bit
+    uint32_t t = top < 0 ? khi : (top >= 31 ? 0u : (khi & ~((2u << top) - 1u)));
+    for (int bit = top; bit >= 0; --bit) {
+      const uint32_t c0 = t | (1u << bit);
+      uint32_t cnt = 0;
+#pragma unroll
+      for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) cnt += ck[j] >= c0;
+      cnt = __reduce_add_sync(0xffffffffu, cnt);
+      uint32_t* part = sh.part[bit & 1];
+      if (lane == 0) part[warp] = cnt;
+      __syncthreads();
+      if (__reduce_add_sync(0xffffffffu, part[lane]) >= need) t = c0;
+    }
+    T = t;
+    {
+      uint32_t g = 0, e = 0;
+#pragma unroll
+      for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) {
+        g += ck[j] > T;
+        e += (ck[j] == T) && (lane + 32 * j < ncand);
+      }
+      g = __reduce_add_sync(0xffffffffu, g);
+      e = __reduce_add_sync(0xffffffffu, e);
+      if (lane == 0) {
+        if (g) atomicAdd(&sh.bis[32], g);
+        sh.wgt[warp] = warp_gt + g;  // elements of this segment with key > T
+        sh.weq[warp] = e;
+      }
+    }
+    __syncthreads();
+    need_eq = need - sh.bis[32];
+  } else {
+    radix_select<CACHED>(x, keys, n, k, sh);
+    T = sh.T;
+    need_eq = sh.need_eq;
+    uint32_t g = 0, e = 0;
+    for (int i = seg0 + lane; i < seg1; i += 32) {
+      const uint32_t key = load_key<CACHED>(x, keys, i);
+      g += key > T;
+      e += key == T;
+    }
+    g = __reduce_add_sync(0xffffffffu, g);
+    e = __reduce_add_sync(0xffffffffu, e);
+    if (lane == 0) {
+      sh.wgt[warp] = g;
+      sh.weq[warp] = e;
+    }
+    __syncthreads();
+  }
+  {
+    const uint32_t g = lane < warp ? sh.wgt[lane] : 0u, e = lane < warp ? sh.weq[lane] : 0u;
+    base_gt = __reduce_add_sync(0xffffffffu, g);
+    base_eq = __reduce_add_sync(0xffffffffu, e);
+  }
+
+  // ---- 4. index-ordered compaction of this warp's segment ----
+  uint32_t run_gt = base_gt, run_eq = base_eq;
+  for (int i0 = seg0; i0 < seg1; i0 += 32) {
+    const int i = i0 + lane;
     bool gt = false, eq = false;
-    if (i < n) {
+    if (i < seg1) {
       const uint32_t key = load_key<CACHED>(x, keys, i);
       gt = key > T;
       eq = key == T;
     }
     const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
-    const uint32_t lt = (1u << lane) - 1u;
-    if (lane == 0) {
-      wsum[warp] = __popc(mg);
-      wsum[TOPK_WARPS + warp] = __popc(me);
-    }
-    __syncthreads();
-    uint32_t bg = run_gt, be = run_eq, tg = 0, te = 0;
-#pragma unroll
-    for (int w = 0; w < TOPK_WARPS; ++w) {
-      const uint32_t a = wsum[w], b = wsum[TOPK_WARPS + w];
-      if (w < warp) { bg += a; be += b; }
-      tg += a;
-      te += b;
-    }
-    const uint32_t my_gt = bg + __popc(mg & lt);
-    const uint32_t my_eq = be + __popc(me & lt);
-    if (gt || (eq && my_eq < need_eq)) out[my_gt + min(my_eq, need_eq)] = seq_start + i;
-    run_gt += tg;
-    run_eq += te;
-    __syncthreads();
-    if (run_eq >= need_eq && run_gt + need_eq >= (uint32_t)k) break;  // uniform: all k slots written
+    const uint32_t pg = run_gt + __popc(mg & lt);
+    const uint32_t pe = run_eq + __popc(me & lt);
+    if (gt || (eq && pe < need_eq)) out[pg + min(pe, need_eq)] = seq_start + i;
+    run_gt += __popc(mg);
+    run_eq += __popc(me);
   }
 }
 
-__global__ void __launch_bounds__(TOPK_THREADS)
-sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int k,
+__global__ void __launch_bounds__(TK_THREADS, 1)
+sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
                int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
-  extern __shared__ uint32_t keys[];
-  __shared__ uint32_t hist[256];
-  __shared__ uint32_t sh[2 + 2 * TOPK_WARPS];
-  const int r = blockIdx.x;
+  extern __shared__ uint32_t tk_smem[];
+  __shared__ TkShared sh;
+  uint32_t* keys = tk_smem;
+  uint32_t* cand = tk_smem + TK_CACHE;
+  // long rows first: the row count is rarely a multiple of the SM count and the tail should be short rows
+  const int r = row_count - 1 - (int)blockIdx.x;
   const SpRow ri = sp_row_info(g, row_begin + r);
   const int n = ri.t_last + 1;
   int32_t* out = idx + (size_t)r * k;
   const int keep = min(n, k);
   if (threadIdx.x == 0 && cnt) cnt[r] = keep;
-  for (int j = keep + threadIdx.x; j < k; j += TOPK_THREADS) out[j] = -1;
+  for (int j = keep + threadIdx.x; j < k; j += TK_THREADS) out[j] = -1;
   if (n <= k) {
-    for (int j = threadIdx.x; j < n; j += TOPK_THREADS) out[j] = ri.seq_start + j;
+    for (int j = threadIdx.x; j < n; j += TK_THREADS) out[j] = ri.seq_start + j;
     return;
   }
   const float* x = scores + (size_t)r * ld;
-  if (n <= TOPK_SMEM_FLOATS) topk_row<true>(x, keys, n, k, ri.seq_start, out, hist, sh);
-  else topk_row<false>(x, keys, n, k, ri.seq_start, out, hist, sh);
+  if (n <= TK_CACHE) topk_row<true>(x, keys, cand, n, k, ri.seq_start, out, sh);
+  else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
 }
 
 }  // namespace
@@ -162,14 +327,14 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
                            int32_t* idx, int32_t* cnt, cudaStream_t st) {
   static bool attr_done = false;
-  const size_t smem = (size_t)TOPK_SMEM_FLOATS * sizeof(uint32_t);
+  const size_t smem = (size_t)(TK_CACHE + TK_WARPS * TK_CAND_PER_WARP) * sizeof(uint32_t);
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(sp_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
   if (row_count <= 0) return cudaSuccess;
-  sp_topk_kernel<<<row_count, TOPK_THREADS, smem, st>>>(g, scores, ld, row_begin, k, idx, cnt);
+  sp_topk_kernel<<<row_count, TK_THREADS, smem, st>>>(g, scores, ld, row_begin, row_count, k, idx, cnt);
   sp_count_launch();
   return cudaGetLastError();
 }

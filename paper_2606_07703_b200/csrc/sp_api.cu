@@ -139,6 +139,16 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
                                   row_count, max_nv, scores, ld, st);
 }
 
+cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const float* lse, int row_begin, int row_count,
+                     int max_nv, float* mass, int64_t ld, cudaStream_t st) {
+  const SpGeom g = dev_geom(p);
+  if (sp_tc_mass_supported(p->b_sel, p->d) && !(debug_simt() & 8))
+    return sp_launch_mass_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, Q, K, lse, p->Hq, p->Hkv, p->d,
+                             attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st);
+  return sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
+                        row_count, max_nv, mass, ld, st);
+}
+
 // idx == nullptr -> dense.  [q_begin, q_begin + q_count) must be the whole pack for the tcgen05 kernel.
 cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
                      int q_count, void* O, float* lse, cudaStream_t st) {
@@ -294,9 +304,7 @@ int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse,
     }
     SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, q_lo, q_hi - q_lo + 1, nullptr, lse, st), "mass pass 1 (lse)");
   }
-  SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
-                         row_count, max_nv, mass, ld_mass, st),
-          "mass pass 2");
+  SP_CUDA(run_mass(p, Q, K, lse, row_begin, row_count, max_nv, mass, ld_mass, st), "mass pass 2");
   return SP_OK;
 }
 
@@ -365,9 +373,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
     if (mode == SP_MODE_INDEXER) {
       SP_CUDA(run_indexer_scores(p, q_idx, k_idx, (int)r0, rcnt, max_nv, scores, pl.ld, st), "indexer scores");
     } else {
-      SP_CUDA(sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, (int)r0,
-                             rcnt, max_nv, scores, pl.ld, st),
-              "mass pass 2");
+      SP_CUDA(run_mass(p, Q, K, lse, (int)r0, rcnt, max_nv, scores, pl.ld, st), "mass pass 2");
     }
     SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
   }

@@ -114,6 +114,11 @@ cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host,
                                         int d_idx, float idx_scale, int local_window, float local_bias, int row_begin,
                                         int row_count, int max_n_valid, float* scores, int64_t ld, cudaStream_t st);
 
+bool sp_tc_mass_supported(int b_sel, int d);
+cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
+                              int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
+                              int row_count, float* mass, int64_t ld, cudaStream_t st);
+
 bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d);
 cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, const void* Q, const void* K,
                               const void* V, const int32_t* idx, int k, int Hq, int Hkv, int d, float scale,

@@ -1,0 +1,398 @@
+// sp_tc_mass.cu -- oracle attention mass, pass 2, on tcgen05 / TMEM / TMA (Alg.1 step 3 :143):
+//   P[t,s] = (1/Hq) sum_h exp(z[t,h,s] - lse[t,h]),  z = scale <q_{t,h}, k_{s,g(h)}> (+ local term),  s <= t
+// for per-query supports (b_sel == 1; block-shared oracle rows stay on the CUDA-core kernel of sp_simt.cu).
+//
+// Persistent, warp specialised.  A work item = 128 consecutive queries of one sequence (MMA M, TMEM lane =
+// query, so lse[t,h] is a per-thread scalar) x 256 consecutive keys (MMA N); only lower-triangular items exist.
+// For each of the Hq heads: TMA brings the head's Q tile (ring) and, once per KV group, the K tile (double
+// buffered); S_h = Q_h K_g^T lands in one of two 256-column TMEM accumulators; two epilogue warpgroups (128
+// key columns each) read it back, form exp2(sl2 * s - lse2) with packed fp32 FMAs + MUFU.EX2 and add into
+// 128 register accumulators per thread, so the head sum never leaves the register file; after the last head
+// the mean is written.  The exponential unit, not the tensor pipe, bounds this kernel (one ex2 per 2d flops).
+// Items are cut into equal contiguous ranges, one per CTA.
+#include "sp_common.cuh"
+#include "sp_tc.cuh"
+
+using namespace sptc;
+
+namespace {
+
+constexpr int MS_MQ = 128;        // queries per item (MMA M)
+constexpr int MS_NK = 256;        // keys per item (MMA N)
+constexpr int MS_THREADS = 384;   // warps 0-3 / 4-7: epilogue of key columns 0-127 / 128-255; 8: TMA; 9: MMA; 10-11 idle
+constexpr int MS_QSTAGES = 3;
+
+__device__ __forceinline__ uint8_t* ms_align1024(uint8_t* p) {
+  return reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(p) + 1023) & ~(uintptr_t)1023);
+}
+__device__ __forceinline__ bool ms_elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ uint64_t ms_pack(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void ms_unpack(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ms_fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t ms_add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ float ms_ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+struct MsTile {
+  int seq_start, n, q0;  // sequence start (packed), sequence length, first LOCAL query of the 128-query tile
+};
+
+// linear query-tile index over the pack -> geometry
+__device__ __forceinline__ MsTile ms_tile_info(const SpGeom& g, int qt) {
+  if (g.cu == nullptr) return MsTile{0, g.L, qt * MS_MQ};
+  int t0 = 0;
+  for (int i = 0; i < g.batch; ++i) {
+    const int s = g.cu[i], n = g.cu[i + 1] - s;
+    const int nt = (n + MS_MQ - 1) / MS_MQ;
+    if (qt < t0 + nt) return MsTile{s, n, (qt - t0) * MS_MQ};
+    t0 += nt;
+  }
+  return MsTile{0, 0, 0};
+}
+// key tiles of a query tile: every 256-key tile that starts at or below the tile's last query
+__device__ __forceinline__ int ms_nkt(const MsTile& t) { return (min(t.q0 + MS_MQ, t.n) - 1) / MS_NK + 1; }
+
+struct MsRange {
+  long long lo, hi;
+};
+__device__ __forceinline__ MsRange ms_cta_range(const SpGeom& g, int qt_begin, int qt_count, int cta, int P) {
+  long long U = 0;
+  for (int i = 0; i < qt_count; ++i) U += ms_nkt(ms_tile_info(g, qt_begin + i));
+  MsRange r;
+  r.lo = (U * cta + P - 1) / P;
+  r.hi = (U * (cta + 1) + P - 1) / P;
+  return r;
+}
+__device__ __forceinline__ void ms_segment(int nkt, long long B, const MsRange& r, int& kt_lo, int& kt_hi) {
+  const long long a = r.lo > B ? r.lo - B : 0, z = r.hi < B + nkt ? r.hi - B : nkt;
+  kt_lo = (int)a;
+  kt_hi = z > a ? (int)z : (int)a;
+}
+
+struct MsBarriers {
+  uint64_t qfull[MS_QSTAGES], qempty[MS_QSTAGES];
+  uint64_t kfull[2], kempty[2];
+  uint64_t accfull[2], accempty[2];
+};
+
+template <int D>
+__global__ void __launch_bounds__(MS_THREADS, 1)
+sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK, SpGeom g,
+                  const float* __restrict__ lse, int Hq, int Hkv, float scale, int local_window, float local_bias,
+                  int row_begin, int row_count, int qt_begin, int qt_count, float* __restrict__ mass, int64_t ld) {
+  constexpr int KB = D / 64;
+  constexpr uint32_t A_BYTES = MS_MQ * 128;  // per 64-wide K block: 128 queries
+  constexpr uint32_t B_BYTES = MS_NK * 128;  // per 64-wide K block: 256 keys
+  constexpr uint32_t Q_STAGE = KB * A_BYTES, K_BUF = KB * B_BYTES;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ MsBarriers bar;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* smem = ms_align1024(smem_raw);
+  uint8_t* sQ = smem;                         // [stage][kb] boxes of 128 rows x 128 B
+  uint8_t* sK = smem + MS_QSTAGES * Q_STAGE;  // [buf][kb] boxes of 256 rows x 128 B
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int G = Hq / Hkv;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < MS_QSTAGES; ++s) {
+      mbar_init(&bar.qfull[s], 1);
+      mbar_init(&bar.qempty[s], 1);
+    }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&bar.kfull[b], 1);
+      mbar_init(&bar.kempty[b], 1);
+      mbar_init(&bar.accfull[b], 1);
+      mbar_init(&bar.accempty[b], 256);
+    }
+    fence_barrier_init();
+    tma_prefetch_desc(&tmQ);
+    tma_prefetch_desc(&tmK);
+  }
+  if (warp == 9) tmem_alloc<512>(&tmem_slot);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem = tmem_slot;
+  const MsRange rg = ms_cta_range(g, qt_begin, qt_count, blockIdx.x, gridDim.x);
+
+  if (warp >= 10) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+  } else if (warp == 8) {
+    // =========================================== TMA producer ===========================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    if (lane == 0) {
+      uint32_t q_s = 0, q_ph = 0, k_n = 0;  // Q ring position; K tiles loaded so far
+      long long B = 0;
+      for (int i = 0; i < qt_count; ++i) {
+        const MsTile ti = ms_tile_info(g, qt_begin + i);
+        const int nkt = ms_nkt(ti);
+        int kt_lo, kt_hi;
+        ms_segment(nkt, B, rg, kt_lo, kt_hi);
+        B += nkt;
+        for (int kt = kt_lo; kt < kt_hi; ++kt) {
+          for (int h = 0; h < Hq; ++h) {
+            if (h % G == 0) {
+              const uint32_t kb_i = k_n & 1;
+              mbar_wait(&bar.kempty[kb_i], ((k_n >> 1) & 1) ^ 1);
+              mbar_expect_tx(&bar.kfull[kb_i], K_BUF);
+#pragma unroll
+              for (int kb = 0; kb < KB; ++kb)
+                tma_load_2d(sK + kb_i * K_BUF + kb * B_BYTES, &tmK, &bar.kfull[kb_i], (h / G) * D + kb * 64,
+                            ti.seq_start + kt * MS_NK);
+              ++k_n;
+            }
+            mbar_wait(&bar.qempty[q_s], q_ph ^ 1);
+            mbar_expect_tx(&bar.qfull[q_s], Q_STAGE);
+#pragma unroll
+            for (int kb = 0; kb < KB; ++kb)
+              tma_load_2d(sQ + q_s * Q_STAGE + kb * A_BYTES, &tmQ, &bar.qfull[q_s], h * D + kb * 64,
+                          ti.seq_start + ti.q0);
+            if (++q_s == MS_QSTAGES) {
+              q_s = 0;
+              q_ph ^= 1;
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 9) {
+    // =========================================== MMA issuer ===========================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    const bool leader = ms_elect_one();
+    constexpr uint32_t idesc = umma_idesc_bf16(MS_MQ, MS_NK, 0, 0);
+    const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ), 16, 1024);
+    const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
+    uint32_t q_s = 0, q_ph = 0, k_n = 0, hc = 0;  // hc: heads issued so far (accumulator = hc & 1)
+    long long B = 0;
+    for (int i = 0; i < qt_count; ++i) {
+      const MsTile ti = ms_tile_info(g, qt_begin + i);
+      const int nkt = ms_nkt(ti);
+      int kt_lo, kt_hi;
+      ms_segment(nkt, B, rg, kt_lo, kt_hi);
+      B += nkt;
+      for (int kt = kt_lo; kt < kt_hi; ++kt) {
+        for (int h = 0; h < Hq; ++h, ++hc) {
+          if (h % G == 0) {
+            mbar_wait(&bar.kfull[k_n & 1], (k_n >> 1) & 1);
+            ++k_n;
+          }
+          const uint32_t kb_i = (k_n - 1) & 1;
+          mbar_wait(&bar.qfull[q_s], q_ph);
+          const uint32_t ab = hc & 1, an = hc >> 1;
+          if (an > 0) mbar_wait(&bar.accempty[ab], (an - 1) & 1);
+          tc_fence_after_sync();
+          if (leader) {
+            const uint64_t qd = qdesc0 + (uint64_t)((q_s * Q_STAGE) >> 4);
+            const uint64_t kd = kdesc0 + (uint64_t)((kb_i * K_BUF) >> 4);
+#pragma unroll
+            for (int k = 0; k < D / 16; ++k)
+              umma_ss(tmem + ab * MS_NK, qd + (uint64_t)(((k / 4) * A_BYTES + (k % 4) * 32) >> 4),
+                      kd + (uint64_t)(((k / 4) * B_BYTES + (k % 4) * 32) >> 4), idesc, k != 0);
+            umma_commit(&bar.accfull[ab]);
+            umma_commit(&bar.qempty[q_s]);
+            if (h % G == G - 1) umma_commit(&bar.kempty[kb_i]);
+          }
+          if (++q_s == MS_QSTAGES) {
+            q_s = 0;
+            q_ph ^= 1;
+          }
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // =========================================== epilogue ===========================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
+    const int e = warp >> 2;   // key columns [128 e, 128 e + 128)
+    const int wq = warp & 3;   // TMEM lane quarter
+    const int r = wq * 32 + lane;  // query row inside the tile
+    const uint32_t tbase = tmem + ((uint32_t)(wq * 32) << 16) + e * 128;
+    const int win = local_window > 0 ? local_window : 0;
+    const float sl2 = scale * SP_LOG2E, lb2 = local_bias * SP_LOG2E;
+    const uint64_t sl2_2 = ms_pack(sl2, sl2);
+    const float inv_hq = 1.f / (float)Hq;
+    const bool vec_ok = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(mass) & 15u) == 0;
+    uint32_t hc = 0;
+    long long B = 0;
+    for (int i = 0; i < qt_count; ++i) {
+      const MsTile ti = ms_tile_info(g, qt_begin + i);
+      const int nkt = ms_nkt(ti);
+      int kt_lo, kt_hi;
+      ms_segment(nkt, B, rg, kt_lo, kt_hi);
+      B += nkt;
+      const int tl = ti.q0 + r;                      // local query of this thread
+      const bool t_ok = tl < ti.n;
+      const int tw0 = ti.q0 + wq * 32;               // warp-uniform: first / last valid query of the warp
+      const int tw1 = min(tw0 + 31, ti.n - 1);
+      const float* lse_row = lse + (size_t)(ti.seq_start + min(tl, ti.n - 1)) * Hq;
+      for (int kt = kt_lo; kt < kt_hi; ++kt) {
+        const int sc0 = kt * MS_NK + e * 128;  // local key of this warpgroup's column 0
+        uint64_t acc[64];
+#pragma unroll
+        for (int c = 0; c < 64; ++c) acc[c] = 0ull;
+        float lse2_next = __ldg(lse_row) * SP_LOG2E;
+        for (int h = 0; h < Hq; ++h, ++hc) {
+          const float lse2 = lse2_next;
+          if (h + 1 < Hq) lse2_next = __ldg(lse_row + h + 1) * SP_LOG2E;
+          const uint32_t ab = hc & 1;
+          mbar_wait(&bar.accfull[ab], (hc >> 1) & 1);
+          tc_fence_after_sync();
+          const uint64_t nl2 = ms_pack(-lse2, -lse2);
+#pragma unroll
+          for (int c0 = 0; c0 < 128; c0 += 32) {
+            const int s_lo = sc0 + c0, s_hi = s_lo + 31;
+            uint32_t v[32];
+            const bool any = s_lo <= tw1;  // warp-uniform: some (t, s) of this chunk is causal
+            if (any) {
+              tmem_ld_x32(tbase + ab * MS_NK + c0, v);
+              tmem_ld_wait();
+            }
+            if (c0 == 96) {  // the accumulator is in registers (or not needed): the next head's MMA may overwrite it
+              tc_fence_before_sync();
+              mbar_arrive(&bar.accempty[ab]);
+            }
+            if (!any) continue;
+            if (s_hi <= tw0 - win && tw0 + 31 < ti.n) {
+              // interior chunk: every pair causal, outside the local window, every query valid
+#pragma unroll
+              for (int j = 0; j < 32; j += 2) {
+                float x0, x1;
+                ms_unpack(ms_fma2(ms_pack(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), sl2_2, nl2), x0, x1);
+                acc[(c0 + j) >> 1] = ms_add2(acc[(c0 + j) >> 1], ms_pack(ms_ex2(x0), ms_ex2(x1)));
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; j += 2) {
+                float p[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                  const int s = s_lo + j + u;
+                  float x = fmaf(__uint_as_float(v[j + u]), sl2, -lse2);
+                  if (win > 0 && tl - s < win) x += lb2;
+                  p[u] = (t_ok && s <= tl) ? ms_ex2(x) : 0.f;
+                }
+                acc[(c0 + j) >> 1] = ms_add2(acc[(c0 + j) >> 1], ms_pack(p[0], p[1]));
+              }
+            }
+          }
+        }
+        // ---- mean over heads, write this thread's row segment ----
+        const int row = ti.seq_start + tl;  // b_sel == 1: support row == packed position
+        if (t_ok && row >= row_begin && row < row_begin + row_count && sc0 <= tl) {
+          float* dst = mass + (size_t)(row - row_begin) * ld + sc0;
+          if (vec_ok && sc0 + 127 <= tl) {
+#pragma unroll
+            for (int c = 0; c < 64; c += 2) {
+              float a0, a1, a2, a3;
+              ms_unpack(acc[c], a0, a1);
+              ms_unpack(acc[c + 1], a2, a3);
+              reinterpret_cast<float4*>(dst)[c >> 1] = make_float4(a0 * inv_hq, a1 * inv_hq, a2 * inv_hq, a3 * inv_hq);
+            }
+          } else {
+#pragma unroll
+            for (int c = 0; c < 64; ++c) {
+              float a0, a1;
+              ms_unpack(acc[c], a0, a1);
+              if (sc0 + 2 * c <= tl) dst[2 * c] = a0 * inv_hq;
+              if (sc0 + 2 * c + 1 <= tl) dst[2 * c + 1] = a1 * inv_hq;
+            }
+          }
+        }
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 9) tmem_dealloc<512>(tmem);
+}
+
+int ms_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
+}
+
+template <int D>
+cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, float scale,
+                           int lw, float lb, int row_begin, int row_count, int qt_begin, int qt_count, long long items,
+                           float* mass, int64_t ld, cudaStream_t st) {
+  CUtensorMap tmQ, tmK;
+  cudaError_t e;
+  if ((e = sp_make_tmap_bf16(&tmQ, Q, g.L, (uint64_t)Hq * D, (uint64_t)Hq * D, MS_MQ)) != cudaSuccess) return e;
+  if ((e = sp_make_tmap_bf16(&tmK, K, g.L, (uint64_t)Hkv * D, (uint64_t)Hkv * D, MS_NK)) != cudaSuccess) return e;
+  constexpr size_t smem = (size_t)(D / 64) * (MS_QSTAGES * MS_MQ * 128 + 2 * MS_NK * 128) + 1024;
+  static bool attr_done = false;
+  if (!attr_done) {
+    e = cudaFuncSetAttribute(sp_tc_mass_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  long long grid = items < ms_sm_count() ? items : ms_sm_count();
+  if (grid < 1) grid = 1;
+  sp_tc_mass_kernel<D><<<(unsigned)grid, MS_THREADS, smem, st>>>(tmQ, tmK, g, lse, Hq, Hkv, scale, lw, lb, row_begin,
+                                                                row_count, qt_begin, qt_count, mass, ld);
+  sp_count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+bool sp_tc_mass_supported(int b_sel, int d) { return b_sel == 1 && (d == 64 || d == 128); }
+
+// cu_host: HOST copy of cu_seqlens (nullptr = one sequence).  b_sel == 1: support rows are packed positions.
+cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
+                              int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
+                              int row_count, float* mass, int64_t ld, cudaStream_t st) {
+  if (row_count <= 0) return cudaSuccess;
+  // 128-query tiles (per sequence) that intersect the packed query range [row_begin, row_begin + row_count)
+  long long t0 = 0, items = 0;
+  long long qlo = -1, qhi = -1;
+  const long long p_lo = row_begin, p_hi = (long long)row_begin + row_count - 1;
+  for (int i = 0; i < g.batch; ++i) {
+    const long long s = cu_host ? cu_host[i] : 0;
+    const int n = cu_host ? cu_host[i + 1] - cu_host[i] : g.L;
+    const long long nt = (n + MS_MQ - 1) / MS_MQ;
+    const long long lo = p_lo > s ? p_lo : s, hi = p_hi < s + n - 1 ? p_hi : s + n - 1;
+    if (lo <= hi) {
+      const long long a = (lo - s) / MS_MQ, z = (hi - s) / MS_MQ;
+      if (qlo < 0) qlo = t0 + a;
+      qhi = t0 + z;
+      for (long long j = a; j <= z; ++j) {
+        const long long q_last = (j + 1) * MS_MQ < n ? (j + 1) * MS_MQ - 1 : n - 1;
+        items += q_last / MS_NK + 1;
+      }
+    }
+    t0 += nt;
+  }
+  if (qlo < 0) return cudaSuccess;
+  const int cnt = (int)(qhi - qlo + 1);
+  return d == 128 ? launch_mass_tc<128>(g, Q, K, lse, Hq, Hkv, scale, local_window, local_bias, row_begin, row_count,
+                                        (int)qlo, cnt, items, mass, ld, st)
+                  : launch_mass_tc<64>(g, Q, K, lse, Hq, Hkv, scale, local_window, local_bias, row_begin, row_count,
+                                       (int)qlo, cnt, items, mass, ld, st);
+}

@@ -6,8 +6,8 @@
 //   SPARSE: the keys are the support row's index list, staged once per item in shared memory; K/V rows are
 //           gathered with cp.async 16-byte vectors written in the SWIZZLE_128B image TMA would have produced;
 //   DENSE : the keys are the causal prefix of the sequence (same loader, consecutive rows), heavy chunks first.
-// Warp roles: warps 0-3 / 4-7 softmax of M tile 0 / 1 (thread = row = TMEM lane), warp 8 MMA issuer (one
-// thread), warps 9-12 index staging + Q/K/V loaders (13-15 idle).  Rings (K, V stages; S double buffered per M tile in TMEM)
+// Warp roles: warps 0-3 / 4-7 softmax of M tile 0 / 1 (thread = row = TMEM lane), warps 9-12 index staging +
+// Q/K/V loaders, warps 8, 13 issue the S MMAs of M tile 0 / 1 and warps 14, 15 their PV MMAs (one lane each).  Rings (K, V stages; S double buffered per M tile in TMEM)
 // run ACROSS items, so the loaders prefetch the next item's index list, K and V while the current one finishes.
 // Per key tile and M tile:
 //   S = Q K^T (tcgen05.mma SS, fp32 in TMEM) -> tcgen05.ld -> scale, mask by KEY POSITION VALUE, online softmax
@@ -24,7 +24,7 @@ namespace {
 
 constexpr int AT_KT = 64;          // keys per tile
 constexpr int AT_MAX_STAGES = 6;   // K/V ring depth is chosen at launch from the shared-memory budget
-constexpr int AT_THREADS = 512;    // 8 softmax warps + 1 MMA warp + 4 loader warps + 3 idle (whole warpgroups for setmaxnreg)
+constexpr int AT_THREADS = 512;    // 8 softmax warps + 4 loader warps + 4 MMA-issuing warps (whole warpgroups for setmaxnreg)
 constexpr int AT_LOAD_WARPS = 4;
 constexpr int AT_MMA_WARP = 8;
 constexpr int AT_LOAD_WARP0 = 9;
@@ -87,6 +87,7 @@ struct AtBarriers {
   uint64_t sfull[2][2];  // MMA -> softmax: S tile (M tile, buffer) is in TMEM
   uint64_t sdone[2][2];  // softmax -> MMA: S has been read (and P written over it)
   uint64_t ofull[2];     // MMA -> softmax: one completion per PV of that M tile (lazy-rescale path)
+  uint64_t pfree[2][2];  // PV issuer -> S issuer: the PV that read P from S buffer (M tile, buffer) has finished
   uint64_t ofin[2];      // MMA -> softmax: one completion per ITEM, after its last PV (epilogue).  A parity wait on
                          // ofull could alias here: the softmax may be two PVs ahead of the tensor pipe.
   uint64_t oempty[2];    // softmax -> MMA: the item's O accumulator has been read out
@@ -167,12 +168,12 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   // ---- barriers, TMEM ----
   if (threadIdx.x == 0) {
     mbar_init(&bar.qfull, 128);
-    mbar_init(&bar.qempty, 1);
+    mbar_init(&bar.qempty, 2);
     for (int s = 0; s < AT_MAX_STAGES; ++s) {
       mbar_init(&bar.kfull[s], 128);
       mbar_init(&bar.vfull[s], 128);
-      mbar_init(&bar.kempty[s], 1);
-      mbar_init(&bar.vempty[s], 1);
+      mbar_init(&bar.kempty[s], 2);
+      mbar_init(&bar.vempty[s], 2);
     }
     for (int m = 0; m < 2; ++m) {
       for (int b = 0; b < 2; ++b) {
@@ -181,6 +182,8 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       }
       mbar_init(&bar.ofull[m], 1);
       mbar_init(&bar.ofin[m], 1);
+      mbar_init(&bar.pfree[m][0], 1);
+      mbar_init(&bar.pfree[m][1], 1);
       mbar_init(&bar.oempty[m], 128);
       mbar_init(&bar.idxfull[m], 128);
       mbar_init(&bar.idxempty[m], 256);
@@ -195,9 +198,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
 
   // register budget: 512 x 128 at launch -> softmax warpgroups 192, the other two warpgroups 64
   // (each role's code is dominated by its own setmaxnreg so ptxas allocates per role)
-  if (warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");  // idle warps
-  } else if (warp >= AT_LOAD_WARP0) {
+  if (warp >= AT_LOAD_WARP0 && warp < AT_LOAD_WARP0 + AT_LOAD_WARPS) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
     // =========================================== loaders ===========================================
     const int ptid = threadIdx.x - AT_LOAD_WARP0 * 32;  // 0..127
@@ -301,113 +302,114 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       gk += nt;
     }
     cp_async_wait<0>();
-  } else if (warp == AT_MMA_WARP) {
-    // =========================================== MMA issuer ===========================================
-    // The whole warp runs the (warp-uniform) control flow and the mbarrier waits; one elected lane issues every
-    // tcgen05.mma / tcgen05.commit.  Descriptors are a precomputed base plus a compile-time offset, ring stages
-    // and phases are tracked incrementally: the issue path must stay well under the ~40 cycles one MMA occupies
-    // the tensor pipe.
+  } else if (warp == AT_MMA_WARP || warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS) {
+    // =========================================== MMA issuers ===========================================
+    // Four issuing warps: S = Q K^T of M tile 0 / 1 (warps 8, 13) and O += P V of M tile 0 / 1 (warps 14, 15).
+    // One warp issuing everything needs ~200 dependent uniform-datapath instructions per key tile (~2000
+    // cycles) and paces the whole CTA; split four ways every issuer stays well under the 1024 cycles the
+    // tensor pipe needs per tile.  The whole warp runs the (warp-uniform) control flow and the mbarrier waits;
+    // one elected lane issues tcgen05.mma / tcgen05.commit.  K / V stages and the Q buffer are released by
+    // BOTH M tiles (barrier count 2; an M tile without work for a tile arrives without MMAs).
     asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
-    {
-      const bool leader = elect_one();
+    const bool leader = elect_one();
+    const int role_pv = warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS + 1;  // warps 14, 15
+    const int mt = (warp == AT_MMA_WARP || warp == AT_LOAD_WARP0 + AT_LOAD_WARPS + 1) ? 0 : 1;
+    if (!(role_pv && !WITH_O)) {
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, AT_KT, 0, 0);  // S = Q K^T : both K-major
       constexpr uint32_t idesc_o = umma_idesc_bf16(128, D, 0, 1);      // O += P V : P from TMEM, V MN-major
-      const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ), 16, 1024);
+      const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ) + mt * 16384, 16, 1024);
       const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
       const uint64_t vdesc0 = umma_desc_sw128(smem_u32(sV), KV_BLK, 1024);
-      uint32_t k_s = 0, k_ph = 0, v_s = 0, v_ph = 0;  // K / V ring positions of the next tile to consume
-      uint32_t n_q = 0, n_it = 0;
-      uint32_t cs[2] = {0, 0}, cp[2] = {0, 0}, n_o[2] = {0, 0};
+      uint32_t r_s = 0, r_ph = 0;            // K (S role) or V (PV role) ring position of the next tile
+      uint32_t n_q = 0, n_it = 0, n_o = 0;   // items with work / items seen / items this M tile was active in
+      uint32_t ct = 0;                       // tiles issued by this warp (S buffer = ct & 1)
       for (int i = 0; i * P < n_items; ++i) {
         const int id = at_item_id(i, cta, P, n_items);
         AtItem it;
         if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
         const int nq = it.t1 - it.t0 + 1;
         const int n_mt = (nq * G > 128) ? 2 : 1;
-        int nt, nt_mt[2];
+        int nt, my_nt;
         if (SPARSE) {
           const int ib = n_it & 1, iu = n_it >> 1;
           mbar_wait(&bar.idxfull[ib], iu & 1);
           nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
-          nt_mt[0] = nt_mt[1] = nt;
+          my_nt = nt;
         } else {
           nt = it.t1 / AT_KT + 1;
-          nt_mt[0] = min(it.t0 + 128 / G - 1, it.t1) / AT_KT + 1;
-          nt_mt[1] = nt;
+          my_nt = mt == 0 ? min(it.t0 + 128 / G - 1, it.t1) / AT_KT + 1 : nt;
         }
+        if (mt >= n_mt) my_nt = 0;
         ++n_it;
         if (nt == 0) continue;
-        mbar_wait(&bar.qfull, n_q & 1);
-        fence_proxy_async_smem();
-        tc_fence_after_sync();
-        auto issue_s = [&](int j) {
-          mbar_wait(&bar.kfull[k_s], k_ph);
+        if (!role_pv) {
+          mbar_wait(&bar.qfull, n_q & 1);
           fence_proxy_async_smem();
           tc_fence_after_sync();
-          const uint64_t kd = kdesc0 + (uint64_t)((k_s * KV_TILE) >> 4);
-#pragma unroll
-          for (int mt = 0; mt < 2; ++mt) {
-            if (mt >= n_mt || j >= nt_mt[mt]) continue;
-            const uint32_t b = cs[mt] & 1, n = cs[mt] >> 1;
-            if (!WITH_O && n > 0) {  // with PV the buffer is released by the (ordered) PV that consumed its P
-              mbar_wait(&bar.sdone[mt][b], (n - 1) & 1);
-              tc_fence_after_sync();
-            }
-            if (leader) {
-              const uint32_t d_s = tmem + TM_S + mt * 128 + b * 64;
-              const uint64_t qd = qdesc0 + (uint64_t)((mt * 16384) >> 4);
-#pragma unroll
-              for (int kk = 0; kk < D / 16; ++kk) {
-                umma_ss(d_s, qd + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
-                        kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
+          for (int j = 0; j < nt; ++j) {
+            mbar_wait(&bar.kfull[r_s], r_ph);
+            if (j < my_nt) {
+              fence_proxy_async_smem();
+              const uint32_t b = ct & 1, n = ct >> 1;
+              if (n > 0) {  // the buffer's previous tile: its P has been consumed (PV) / its S has been read
+                if (WITH_O) mbar_wait(&bar.pfree[mt][b], (n - 1) & 1);
+                else mbar_wait(&bar.sdone[mt][b], (n - 1) & 1);
               }
-              umma_commit(&bar.sfull[mt][b]);
-            }
-            ++cs[mt];
-          }
-          if (leader) umma_commit(&bar.kempty[k_s]);
-          if (++k_s == (uint32_t)NS) {
-            k_s = 0;
-            k_ph ^= 1;
-          }
-        };
-        auto issue_pv = [&](int j) {
-          mbar_wait(&bar.vfull[v_s], v_ph);
-          fence_proxy_async_smem();
-          const uint64_t vd = vdesc0 + (uint64_t)((v_s * KV_TILE) >> 4);
+              tc_fence_after_sync();
+              if (leader) {
+                const uint32_t d_s = tmem + TM_S + mt * 128 + b * 64;
+                const uint64_t kd = kdesc0 + (uint64_t)((r_s * KV_TILE) >> 4);
 #pragma unroll
-          for (int mt = 0; mt < 2; ++mt) {
-            if (mt >= n_mt || j >= nt_mt[mt]) continue;
-            const uint32_t b = cp[mt] & 1, n = cp[mt] >> 1;
-            mbar_wait(&bar.sdone[mt][b], n & 1);
-            if (j == 0 && n_o[mt] > 0) mbar_wait(&bar.oempty[mt], (n_o[mt] - 1) & 1);
-            tc_fence_after_sync();
-            if (leader) {
-              const uint32_t d_o = tmem + TM_O + mt * D, a_p = tmem + TM_S + mt * 128 + b * 64;
-#pragma unroll
-              for (int kk = 0; kk < AT_KT / 16; ++kk)
-                umma_ts(d_o, a_p + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_o, (j | kk) != 0);
-              umma_commit(&bar.ofull[mt]);
-              if (j == nt_mt[mt] - 1) umma_commit(&bar.ofin[mt]);
+                for (int kk = 0; kk < D / 16; ++kk) {
+                  umma_ss(d_s, qdesc0 + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
+                          kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
+                }
+                umma_commit(&bar.sfull[mt][b]);
+                umma_commit(&bar.kempty[r_s]);
+              }
+              ++ct;
+            } else if (leader) {
+              mbar_arrive(&bar.kempty[r_s]);
             }
-            ++cp[mt];
+            if (++r_s == (uint32_t)NS) {
+              r_s = 0;
+              r_ph ^= 1;
+            }
           }
-          if (leader) umma_commit(&bar.vempty[v_s]);
-          if (++v_s == (uint32_t)NS) {
-            v_s = 0;
-            v_ph ^= 1;
+          if (leader) {  // every S MMA of the item has been issued: Q is free when they finish
+            if (my_nt > 0) umma_commit(&bar.qempty);
+            else mbar_arrive(&bar.qempty);
           }
-        };
-        issue_s(0);
-        for (int j = 0; j < nt; ++j) {
-          if (j + 1 < nt) issue_s(j + 1);
-          else if (leader) umma_commit(&bar.qempty);  // every S MMA of the item is issued: Q is free when they finish
-          if (WITH_O) issue_pv(j);
-        }
-        if (WITH_O) {
-          for (int mt = 0; mt < n_mt; ++mt) ++n_o[mt];
         } else {
-          for (int mt = 0; mt < n_mt; ++mt) cp[mt] = cs[mt];
+          for (int j = 0; j < nt; ++j) {
+            mbar_wait(&bar.vfull[r_s], r_ph);
+            if (j < my_nt) {
+              fence_proxy_async_smem();
+              const uint32_t b = ct & 1, n = ct >> 1;
+              mbar_wait(&bar.sdone[mt][b], n & 1);  // softmax(j) has written P over S
+              if (j == 0 && n_o > 0) mbar_wait(&bar.oempty[mt], (n_o - 1) & 1);
+              tc_fence_after_sync();
+              if (leader) {
+                const uint64_t vd = vdesc0 + (uint64_t)((r_s * KV_TILE) >> 4);
+                const uint32_t d_o = tmem + TM_O + mt * D, a_p = tmem + TM_S + mt * 128 + b * 64;
+#pragma unroll
+                for (int kk = 0; kk < AT_KT / 16; ++kk)
+                  umma_ts(d_o, a_p + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_o, (j | kk) != 0);
+                umma_commit(&bar.pfree[mt][b]);
+                umma_commit(&bar.ofull[mt]);
+                if (j == my_nt - 1) umma_commit(&bar.ofin[mt]);
+                umma_commit(&bar.vempty[r_s]);
+              }
+              ++ct;
+            } else if (leader) {
+              mbar_arrive(&bar.vempty[r_s]);
+            }
+            if (++r_s == (uint32_t)NS) {
+              r_s = 0;
+              r_ph ^= 1;
+            }
+          }
+          if (my_nt > 0) ++n_o;
         }
         ++n_q;
       }

@@ -98,7 +98,7 @@ def oracle_sample_rate(cfg, inp, budget_rows=None):
                       d_idx=cfg.d_idx, local_window=cfg.local_window, local_bias=cfg.local_bias,
                       cu_seqlens=cfg.cu_seqlens)
     n_rows = orc.num_rows(pbo)
-    nsel = budget_rows or (8 if cfg.b_sel > 1 else 256)
+    nsel = budget_rows or (96 if cfg.b_sel > 1 else 2048)  # ~10-20 s of host work at the bench workloads
     rows = np.unique(np.linspace(0, n_rows - 1, nsel).astype(np.int64))
     pos = []
     for r in rows:
@@ -169,6 +169,41 @@ def workload_config(cfg):
 # GPU leg
 # ------------------------------------------------------------------------------------------------
 
+def measure_layer_only(cfg, B, torch, gen, steps):
+    """Layer latency of another workload (device-resident inputs, CUDA events, 3 warm-up steps) next to the dense
+    GQA layer of the same library on the same tensors."""
+    inp = gen.make_inputs(cfg)
+    indexer = cfg.mode != "oracle"
+    gmode = B.SP_MODE_INDEXER if indexer else B.SP_MODE_ORACLE
+    names = ("X", "Wqi", "Wki", "Q", "K", "V") if indexer else ("Q", "K", "V")
+    devt = {n: B.bf16_tensor(inp[n]) for n in names}
+    pb = B.Problem.from_config(cfg)
+    O = torch.empty(cfg.L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+    idx = torch.empty(pb.num_rows, cfg.k, dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(pb, B.SP_STAGE_LAYER_INDEXER if indexer else B.SP_STAGE_LAYER_ORACLE)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps, warm):
+        for _ in range(warm):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    ms = timed(lambda: B.sp_prefill_layer(pb, gmode, devt.get("X"), devt.get("Wqi"), devt.get("Wki"), devt["Q"],
+                                          devt["K"], devt["V"], O, idx, ws), steps, 3)
+    dense_ms = timed(lambda: B.sp_dense_gqa_attn(pb, devt["Q"], devt["K"], devt["V"], O, None), 2, 1)
+    causal = cfg.L * (cfg.L + 1) // 2
+    return {"config": workload_config(cfg), "ms_per_step": ms, "tokens_per_s": cfg.L / (ms * 1e-3), "steps": steps,
+            "dense_layer_ms": dense_ms, "dense_tflops": 4.0 * cfg.d * cfg.Hq * causal / (dense_ms * 1e-3) / 1e12,
+            "speedup_sparse_vs_dense": dense_ms / ms}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -177,6 +212,7 @@ def main():
     ap.add_argument("--workload", default="c3")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-long", action="store_true", help="skip the 128K (c5) layer line inside the c3 run")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -370,6 +406,19 @@ def main():
         "paper_context": "TTFT ratios in the paper (whole model, other hardware): 1.93x Qwen3.5-9B GPU-80G vs FA2 @256K; "
                          "1.71x Qwen3.5-0.8B NPU-64G vs vLLM-Ascend FA @256K (PAPER.md:434-440); not comparable to a layer",
     }
+    # measured DRAM traffic of the dominant kernel (ncu --set full capture summarised under profiles/)
+    tr_path = os.path.join(ROOT, "profiles", "kernel_traffic.txt")
+    if os.path.exists(tr_path):
+        with open(tr_path) as f:
+            tr = json.load(f).get(cfg.name, {}).get(dom)
+        if tr is not None:
+            line["roofline"]["traffic"] = tr["dram_bytes_per_launch"]
+            line["roofline"]["traffic_source"] = tr["source"]
+    if cfg.name == "c3" and not args.no_long and world == 1:
+        # the metric is quoted at 32K and 128K: the 128K layer (BASELINE.json configs[4]) timed in the same run
+        del devt, host, O, O_dense, idx, ws, arena, scores
+        torch.cuda.empty_cache()
+        line["long_context_128k"] = measure_layer_only(gen.ALL["c5"], B, torch, gen, steps=min(args.steps, 5))
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         cb = oracle_sample_rate(cfg, inp)
         cb.pop("seconds", None)

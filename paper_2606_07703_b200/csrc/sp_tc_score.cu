@@ -4,11 +4,12 @@
 // The KEY index is the MMA M dimension (TMEM lane = key, column = query), so the max over a selection block's
 // queries is a per-thread running max over columns and global writes are coalesced along s.
 //
-// One CTA per SM.  A query SUPER TILE (512 consecutive local positions of one sequence = two MMA N = 256
-// halves) stays resident in shared memory while 128-key tiles stream through a TMA ring; each half owns one
-// 256-column TMEM accumulator and one epilogue warpgroup (tcgen05.ld -> block max -> coalesced stores), so
-// each epilogue overlaps the MMAs of the other half.  Only lower-triangular (key tile, half) pairs are computed.  The
-// linear sequence of key-tile steps (weight = active halves) is cut into equal contiguous ranges, one per
+// One CTA per SM.  A query SUPER TILE (512 consecutive local positions of one sequence = four MMA N = 128
+// parts) stays resident in shared memory while 128-key tiles stream through a TMA ring; each part owns one
+// 128-column TMEM accumulator, two epilogue warpgroups (tcgen05.ld -> block max -> coalesced stores) serve
+// parts {0,2} and {1,3}, and a part's accumulator is reused only after the other three parts' MMAs, so the
+// epilogues hide behind the tensor pipe.  Only lower-triangular (key tile, part) pairs are computed.  The
+// linear sequence of key-tile steps (weight = active parts) is cut into equal contiguous ranges, one per
 // CTA, so a CTA reloads Q only when its range crosses a super-tile boundary.
 #include "sp_common.cuh"
 #include "sp_tc.cuh"
@@ -17,7 +18,8 @@ using namespace sptc;
 
 namespace {
 
-constexpr int SC_NQ = 256;     // queries per half (MMA N)
+constexpr int SC_NQ = 128;     // queries per part (MMA N); a super tile has SC_PARTS parts
+constexpr int SC_PARTS = 4;
 constexpr int SC_SUPER = 512;  // queries per resident super tile
 constexpr int SC_KT = 128;     // keys per tile (MMA M)
 constexpr int SC_THREADS = 320;  // warp 0: TMA, warp 1: MMA, warps 2-5 / 6-9: epilogue of half 0 / 1
@@ -55,13 +57,22 @@ __device__ __forceinline__ ScSuper sc_super_info(const SpGeom& g, int st) {
   return ScSuper{0, 0, 0, 0};
 }
 
-// Key-tile steps of one super tile: kt in [0, nkt); steps kt < k2 feed both halves (weight 2), the rest only
-// half 1 (weight 1).
+// Key-tile steps of one super tile: kt in [0, nkt).  Part p (queries q0 + 128 p ...) needs key tile kt iff
+// kt * 128 <= its last query: steps kt < jfull feed every existing part (weight np), step jfull + m (m >= 0)
+// only parts p > m (weight np - 1 - m).
 struct ScSteps {
-  int nkt, k2;
-  __device__ __forceinline__ int weight() const { return nkt + k2; }
-  __device__ __forceinline__ int first_at(int x) const {  // smallest kt whose weight prefix is >= x
-    return x <= 2 * k2 ? (x + 1) / 2 : k2 + (x - 2 * k2);
+  int nkt, jfull, np;
+  __device__ __forceinline__ int w_before(int kt) const {  // weight of steps [0, kt)
+    if (kt <= jfull) return np * kt;
+    const int m = kt - jfull;  // tail steps taken: weights np-1, np-2, ...
+    return np * jfull + m * np - m * (m + 1) / 2;
+  }
+  __device__ __forceinline__ int weight() const { return w_before(nkt); }
+  __device__ __forceinline__ int first_at(int x) const {  // smallest kt with w_before(kt) >= x
+    if (x <= np * jfull) return (x + np - 1) / np;
+    int kt = jfull;
+    while (kt < nkt && w_before(kt) < x) ++kt;
+    return kt;
   }
 };
 
@@ -69,17 +80,17 @@ __device__ __forceinline__ ScSteps sc_steps(const ScSuper& su) {
   const int q_last = min(su.q0 + SC_SUPER, su.n) - 1;
   ScSteps s;
   s.nkt = q_last / SC_KT + 1;
-  if (su.q0 + SC_NQ <= q_last) s.k2 = (su.q0 + SC_NQ - 1) / SC_KT + 1;  // half 1 exists: half 0 ends at q0 + 255
-  else s.k2 = 0;                                                        // only half 0: weight 1 per step
+  s.np = (q_last - su.q0) / SC_NQ + 1;
+  s.jfull = min(su.q0 / SC_KT + 1, s.nkt);
   return s;
 }
 
-// is (kt, half h) a computed pair?  (identical in the MMA and the epilogue role)
-__device__ __forceinline__ bool sc_half_active(const ScSuper& su, int kt, int h) {
-  const int qh0 = su.q0 + h * SC_NQ;
-  if (qh0 >= su.n) return false;
-  const int qh_last = min(qh0 + SC_NQ, su.n) - 1;
-  return kt * SC_KT <= qh_last;
+// is (kt, part p) a computed pair?  (identical in the MMA and the epilogue role)
+__device__ __forceinline__ bool sc_part_active(const ScSuper& su, int kt, int p) {
+  const int qp0 = su.q0 + p * SC_NQ;
+  if (qp0 >= su.n) return false;
+  const int qp_last = min(qp0 + SC_NQ, su.n) - 1;
+  return kt * SC_KT <= qp_last;
 }
 
 // This CTA's contiguous range [lo, hi) of the global weight axis.
@@ -110,7 +121,7 @@ __device__ __forceinline__ void sc_segment(const ScSteps& s, long long B, const 
 struct ScBarriers {
   uint64_t qfull, qempty;
   uint64_t kfull[SC_MAX_STAGES], kempty[SC_MAX_STAGES];
-  uint64_t accfull[2], accempty[2];
+  uint64_t accfull[SC_PARTS], accempty[SC_PARTS];
 };
 
 // Epilogue of one (key tile, half): thread = key (TMEM lane), columns = the half's 256 queries.
@@ -198,14 +209,14 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                    int st_count, int n_stages, float* __restrict__ scores, int64_t ld) {
   constexpr int KB = DI / 64;
   constexpr uint32_t A_BYTES = SC_KT * 128;  // per 64-wide K block: 128 keys
-  constexpr uint32_t B_BYTES = SC_NQ * 128;  // per 64-wide K block: 256 queries
+  constexpr uint32_t B_BYTES = SC_NQ * 128;  // per 64-wide K block: the 128 queries of one part
   constexpr uint32_t K_STAGE = KB * A_BYTES;
   extern __shared__ uint8_t smem_raw[];
   __shared__ ScBarriers bar;
   __shared__ uint32_t tmem_slot;
   uint8_t* smem = sc_align1024(smem_raw);
-  uint8_t* sQ = smem;                       // [half][kb] boxes of 256 rows x 128 B
-  uint8_t* sK = smem + 2 * KB * B_BYTES;    // [stage][kb] boxes of 128 rows x 128 B
+  uint8_t* sQ = smem;                             // [part][kb] boxes of 128 rows x 128 B
+  uint8_t* sK = smem + SC_PARTS * KB * B_BYTES;   // [stage][kb] boxes of 128 rows x 128 B
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int NS = n_stages;
   const int b = g.b_sel;
@@ -217,7 +228,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
       mbar_init(&bar.kfull[s], 1);
       mbar_init(&bar.kempty[s], 1);
     }
-    for (int h = 0; h < 2; ++h) {
+    for (int h = 0; h < SC_PARTS; ++h) {
       mbar_init(&bar.accfull[h], 1);
       mbar_init(&bar.accempty[h], 128);
     }
@@ -245,7 +256,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         B += ss.weight();
         if (kt_lo >= kt_hi) continue;
         if (n_seg > 0) mbar_wait(&bar.qempty, (n_seg - 1) & 1);
-        const int nh = (su.q0 + SC_NQ < su.n) ? 2 : 1;
+        const int nh = ss.np;
         mbar_expect_tx(&bar.qfull, nh * KB * B_BYTES);
         for (int h = 0; h < nh; ++h)
 #pragma unroll
@@ -272,7 +283,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ), 16, 1024);
     const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
     uint32_t k_s = 0, k_ph = 0, n_seg = 0;
-    uint32_t use[2] = {0, 0};  // accumulator uses so far
+    uint32_t use[SC_PARTS] = {0, 0, 0, 0};  // accumulator uses so far
     long long B = 0;
     for (int i = 0; i < st_count; ++i) {
       const ScSuper su = sc_super_info(g, st_begin + i);
@@ -288,8 +299,8 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         tc_fence_after_sync();
         const uint64_t kd = kdesc0 + (uint64_t)((k_s * K_STAGE) >> 4);
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          if (!sc_half_active(su, kt, h)) continue;
+        for (int h = 0; h < SC_PARTS; ++h) {
+          if (!sc_part_active(su, kt, h)) continue;
           if (use[h] > 0) {
             mbar_wait(&bar.accempty[h], (use[h] - 1) & 1);
             tc_fence_after_sync();
@@ -315,12 +326,13 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     __syncwarp();
   } else {
     // =========================================== epilogue ===========================================
-    // warps 2-5 serve half 0, warps 6-9 half 1: each warpgroup has the MMA time of BOTH halves for its own.
-    const int h = (warp - 2) >> 2;
+    // warps 2-5 serve parts 0 and 2, warps 6-9 parts 1 and 3.  A part's accumulator is needed again only after
+    // the MMAs of the other three parts, so the epilogue has ~3x its MMA time of slack.
+    const int e = (warp - 2) >> 2;
     const int wq = warp & 3;  // TMEM lane quarter this warp may access
-    const uint32_t trow = tmem + ((uint32_t)(wq * 32) << 16) + h * SC_NQ;
+    const uint32_t trow0 = tmem + ((uint32_t)(wq * 32) << 16);
     const int lb = 31 - __clz(b);
-    uint32_t use = 0;
+    uint32_t use[2] = {0, 0};
     long long B = 0;
     for (int i = 0; i < st_count; ++i) {
       const ScSuper su = sc_super_info(g, st_begin + i);
@@ -328,18 +340,21 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
       int kt_lo, kt_hi;
       sc_segment(ss, B, rg, kt_lo, kt_hi);
       B += ss.weight();
-      const int hq0 = su.q0 + h * SC_NQ;
-      const int q_last = min(hq0 + SC_NQ, su.n) - 1;
-      const int hrow0 = su.row0 + ((h * SC_NQ) >> lb);
       for (int kt = kt_lo; kt < kt_hi; ++kt) {
-        if (!sc_half_active(su, kt, h)) continue;
-        mbar_wait(&bar.accfull[h], use & 1);
-        tc_fence_after_sync();
-        sc_epilogue(trow, wq, lane, kt * SC_KT, hq0, hrow0, q_last, b, lb, idx_scale, local_window, local_bias,
-                    row_begin, row_count, scores, ld);
-        tc_fence_before_sync();
-        mbar_arrive(&bar.accempty[h]);
-        ++use;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int p = e + 2 * u;
+          if (!sc_part_active(su, kt, p)) continue;
+          const int pq0 = su.q0 + p * SC_NQ;
+          const int q_last = min(pq0 + SC_NQ, su.n) - 1;
+          mbar_wait(&bar.accfull[p], use[u] & 1);
+          tc_fence_after_sync();
+          sc_epilogue(trow0 + p * SC_NQ, wq, lane, kt * SC_KT, pq0, su.row0 + ((p * SC_NQ) >> lb), q_last, b, lb,
+                      idx_scale, local_window, local_bias, row_begin, row_count, scores, ld);
+          tc_fence_before_sync();
+          mbar_arrive(&bar.accempty[p]);
+          ++use[u];
+        }
       }
     }
   }
@@ -353,7 +368,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
 // ---------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------
-bool sp_tc_scores_supported(int b_sel) { return b_sel == 1 || b_sel == 32 || b_sel == 64 || b_sel == 128 || b_sel == 256; }
+bool sp_tc_scores_supported(int b_sel) { return b_sel == 1 || b_sel == 32 || b_sel == 64 || b_sel == 128; }
 
 static int sc_sm_count() {
   static int n = 0;
@@ -374,7 +389,7 @@ static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const vo
   if ((e = sp_make_tmap_bf16(&tmQ, q_idx, g.L, DI, DI, SC_NQ)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmK, k_idx, g.L, DI, DI, SC_KT)) != cudaSuccess) return e;
   constexpr int stages = DI == 128 ? 3 : 4;
-  constexpr size_t smem = (size_t)(DI / 64) * (2 * SC_NQ * 128 + stages * SC_KT * 128) + 1024;
+  constexpr size_t smem = (size_t)(DI / 64) * (SC_PARTS * SC_NQ * 128 + stages * SC_KT * 128) + 1024;
   static bool attr_done = false;
   if (!attr_done) {
     e = cudaFuncSetAttribute(sp_tc_score_kernel<DI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -6,9 +6,9 @@
 //
 // One CTA per SM.  A query SUPER TILE (512 consecutive local positions of one sequence = four MMA N = 128
 // parts) stays resident in shared memory while 128-key tiles stream through a TMA ring; each part owns one
-// 128-column TMEM accumulator, two epilogue warpgroups (tcgen05.ld -> block max -> coalesced stores) serve
-// parts {0,2} and {1,3}, and a part's accumulator is reused only after the other three parts' MMAs, so the
-// epilogues hide behind the tensor pipe.  Only lower-triangular (key tile, part) pairs are computed.  The
+// 128-column TMEM accumulator and one epilogue warpgroup (tcgen05.ld -> block max -> coalesced stores); a
+// part's accumulator is reused only after the other three parts' MMAs, so the epilogues hide behind the
+// tensor pipe.  Only lower-triangular (key tile, part) pairs are computed.  The
 // linear sequence of key-tile steps (weight = active parts) is cut into equal contiguous ranges, one per
 // CTA, so a CTA reloads Q only when its range crosses a super-tile boundary.
 #include "sp_common.cuh"
@@ -22,7 +22,7 @@ constexpr int SC_NQ = 128;     // queries per part (MMA N); a super tile has SC_
 constexpr int SC_PARTS = 4;
 constexpr int SC_SUPER = 512;  // queries per resident super tile
 constexpr int SC_KT = 128;     // keys per tile (MMA M)
-constexpr int SC_THREADS = 320;  // warp 0: TMA, warp 1: MMA, warps 2-5 / 6-9: epilogue of half 0 / 1
+constexpr int SC_THREADS = 576;  // warp 0: TMA, warp 1: MMA, warps 2-17: one epilogue warpgroup per part
 constexpr int SC_MAX_STAGES = 4;
 
 __device__ __forceinline__ uint8_t* sc_align1024(uint8_t* p) {
@@ -60,18 +60,24 @@ __device__ __forceinline__ ScSuper sc_super_info(const SpGeom& g, int st) {
 // Key-tile steps of one super tile: kt in [0, nkt).  Part p (queries q0 + 128 p ...) needs key tile kt iff
 // kt * 128 <= its last query: steps kt < jfull feed every existing part (weight np), step jfull + m (m >= 0)
 // only parts p > m (weight np - 1 - m).
+constexpr int SC_FIXED_W = 8;  // weight units (one unit = one 128 x 128 x d_idx MMA tile) charged per super tile
+                               // for draining the pipeline and reloading the resident Q tile
 struct ScSteps {
   int nkt, jfull, np;
-  __device__ __forceinline__ int w_before(int kt) const {  // weight of steps [0, kt)
+  __device__ __forceinline__ int w_steps(int kt) const {  // MMA weight of steps [0, kt)
     if (kt <= jfull) return np * kt;
     const int m = kt - jfull;  // tail steps taken: weights np-1, np-2, ...
     return np * jfull + m * np - m * (m + 1) / 2;
   }
+  __device__ __forceinline__ int w_before(int kt) const { return kt == 0 ? 0 : SC_FIXED_W + w_steps(kt); }
   __device__ __forceinline__ int weight() const { return w_before(nkt); }
   __device__ __forceinline__ int first_at(int x) const {  // smallest kt with w_before(kt) >= x
-    if (x <= np * jfull) return (x + np - 1) / np;
+    if (x <= 0) return 0;
+    const int y = x - SC_FIXED_W;
+    if (y <= np) return 1;
+    if (y <= np * jfull) return (y + np - 1) / np;
     int kt = jfull;
-    while (kt < nkt && w_before(kt) < x) ++kt;
+    while (kt < nkt && w_steps(kt) < y) ++kt;
     return kt;
   }
 };
@@ -96,6 +102,8 @@ __device__ __forceinline__ bool sc_part_active(const ScSuper& su, int kt, int p)
 // This CTA's contiguous range [lo, hi) of the global weight axis.
 struct ScRange {
   long long lo, hi;
+  int i_first;        // first super tile (relative to st_begin) that intersects [lo, hi)
+  long long b_first;  // its weight base
 };
 __device__ __forceinline__ ScRange sc_cta_range(const SpGeom& g, int st_begin, int st_count, int cta, int P) {
   long long U = 0;
@@ -103,6 +111,18 @@ __device__ __forceinline__ ScRange sc_cta_range(const SpGeom& g, int st_begin, i
   ScRange r;
   r.lo = (U * cta + P - 1) / P;
   r.hi = (U * (cta + 1) + P - 1) / P;
+  r.i_first = st_count;
+  r.b_first = U;
+  long long B = 0;
+  for (int i = 0; i < st_count; ++i) {
+    const long long W = sc_steps(sc_super_info(g, st_begin + i)).weight();
+    if (B + W > r.lo) {
+      r.i_first = i;
+      r.b_first = B;
+      break;
+    }
+    B += W;
+  }
   return r;
 }
 // key-tile segment [kt_lo, kt_hi) of super tile with weight base B that falls into range r
@@ -124,7 +144,22 @@ struct ScBarriers {
   uint64_t accfull[SC_PARTS], accempty[SC_PARTS];
 };
 
-// Epilogue of one (key tile, half): thread = key (TMEM lane), columns = the half's 256 queries.
+__device__ __forceinline__ float sc_max32(const uint32_t* v) {
+  float m0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1]));
+  float m1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
+  float m2 = fmaxf(__uint_as_float(v[4]), __uint_as_float(v[5]));
+  float m3 = fmaxf(__uint_as_float(v[6]), __uint_as_float(v[7]));
+#pragma unroll
+  for (int j = 8; j < 32; j += 8) {
+    m0 = fmaxf(m0, fmaxf(__uint_as_float(v[j]), __uint_as_float(v[j + 1])));
+    m1 = fmaxf(m1, fmaxf(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3])));
+    m2 = fmaxf(m2, fmaxf(__uint_as_float(v[j + 4]), __uint_as_float(v[j + 5])));
+    m3 = fmaxf(m3, fmaxf(__uint_as_float(v[j + 6]), __uint_as_float(v[j + 7])));
+  }
+  return fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
+}
+
+// Epilogue of one (key tile, part): thread = key (TMEM lane), columns = the part's 128 queries.
 // b == 1 writes every causal (t, s); b > 1 (a power of two, 2^lb) keeps the max of each selection block.
 __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane, int s0, int hq0, int hrow0, int q_last,
                                             int b, int lb, float idx_scale, int local_window, float local_bias,
@@ -156,6 +191,33 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
   }
   const bool fast_ok = idx_scale > 0.f;  // max commutes with a positive scale
   const int nblk = SC_NQ >> lb;
+  if (fast_ok && hq0 + SC_NQ - 1 <= q_last && hq0 - s_hi >= (local_window > 0 ? local_window : 0)) {
+    // interior (key warp, part): all 32 x 128 pairs are causal, inside the sequence and outside the local
+    // window -> no per-element work, no inner branches: chunk maxima, then one store per selection block
+    float cm[4];
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      uint32_t v0[32], v1[32];
+      tmem_ld_x32(trow + hh * 64, v0);
+      tmem_ld_x32(trow + hh * 64 + 32, v1);
+      tmem_ld_wait();
+      cm[2 * hh] = sc_max32(v0);
+      cm[2 * hh + 1] = sc_max32(v1);
+    }
+    if (lb == 6) {
+      cm[0] = fmaxf(cm[0], cm[1]);
+      cm[1] = fmaxf(cm[2], cm[3]);
+    } else if (lb == 7) {
+      cm[0] = fmaxf(fmaxf(cm[0], cm[1]), fmaxf(cm[2], cm[3]));
+    }
+#pragma unroll
+    for (int blk = 0; blk < 4; ++blk) {
+      const int row = hrow0 + blk;
+      if (blk < nblk && row >= row_begin && row < row_begin + row_count)
+        scores[(size_t)(row - row_begin) * ld + s] = cm[blk] * idx_scale;
+    }
+    return;
+  }
   for (int blk = 0; blk < nblk; ++blk) {
     const int bq0 = hq0 + (blk << lb);  // first local query of the selection block
     if (bq0 > q_last) break;
@@ -185,15 +247,18 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
         }
         best = fmaxf(best, fmaxf(fmaxf(m0, m1), fmaxf(m2, m3)) * idx_scale);
       } else {
+        // diagonal / local-window chunk: branch-free per element, four independent max chains
+        const int d0 = t0 - s;          // t - s of column j is d0 + j
+        const int jmax = q_last - t0;   // warp-uniform: columns j > jmax lie beyond the sequence end
+        float m4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
         for (int j = 0; j < 32; ++j) {
-          const int t = t0 + j;
-          if (t <= q_last && s <= t) {
-            float z = __uint_as_float(v[j]) * idx_scale;
-            if (local_window > 0 && t - s < local_window) z += local_bias;
-            best = fmaxf(best, z);
-          }
+          float z = __uint_as_float(v[j]) * idx_scale;
+          if (local_window > 0) z = (d0 + j < local_window) ? z + local_bias : z;
+          z = (d0 + j >= 0 && j <= jmax) ? z : -INFINITY;
+          m4[j & 3] = fmaxf(m4[j & 3], z);
         }
+        best = fmaxf(best, fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3])));
       }
     }
     const int row = hrow0 + blk;
@@ -247,8 +312,8 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     // =========================================== TMA producer ===========================================
     if (lane == 0) {
       uint32_t k_s = 0, k_ph = 0, n_seg = 0;
-      long long B = 0;
-      for (int i = 0; i < st_count; ++i) {
+      long long B = rg.b_first;
+      for (int i = rg.i_first; i < st_count && B < rg.hi; ++i) {
         const ScSuper su = sc_super_info(g, st_begin + i);
         const ScSteps ss = sc_steps(su);
         int kt_lo, kt_hi;
@@ -284,8 +349,8 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
     uint32_t k_s = 0, k_ph = 0, n_seg = 0;
     uint32_t use[SC_PARTS] = {0, 0, 0, 0};  // accumulator uses so far
-    long long B = 0;
-    for (int i = 0; i < st_count; ++i) {
+    long long B = rg.b_first;
+    for (int i = rg.i_first; i < st_count && B < rg.hi; ++i) {
       const ScSuper su = sc_super_info(g, st_begin + i);
       const ScSteps ss = sc_steps(su);
       int kt_lo, kt_hi;
@@ -326,35 +391,32 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     __syncwarp();
   } else {
     // =========================================== epilogue ===========================================
-    // warps 2-5 serve parts 0 and 2, warps 6-9 parts 1 and 3.  A part's accumulator is needed again only after
-    // the MMAs of the other three parts, so the epilogue has ~3x its MMA time of slack.
-    const int e = (warp - 2) >> 2;
+    // one epilogue warpgroup per part (warps 2-5, 6-9, 10-13, 14-17).  A part's accumulator is needed again
+    // only after the MMAs of the other three parts, so each epilogue has ~3x its MMA time of slack.
+    const int p = (warp - 2) >> 2;
     const int wq = warp & 3;  // TMEM lane quarter this warp may access
-    const uint32_t trow0 = tmem + ((uint32_t)(wq * 32) << 16);
+    const uint32_t trow = tmem + ((uint32_t)(wq * 32) << 16) + p * SC_NQ;
     const int lb = 31 - __clz(b);
-    uint32_t use[2] = {0, 0};
-    long long B = 0;
-    for (int i = 0; i < st_count; ++i) {
+    uint32_t use = 0;
+    long long B = rg.b_first;
+    for (int i = rg.i_first; i < st_count && B < rg.hi; ++i) {
       const ScSuper su = sc_super_info(g, st_begin + i);
       const ScSteps ss = sc_steps(su);
       int kt_lo, kt_hi;
       sc_segment(ss, B, rg, kt_lo, kt_hi);
       B += ss.weight();
+      const int pq0 = su.q0 + p * SC_NQ;
+      const int q_last = min(pq0 + SC_NQ, su.n) - 1;
+      const int prow0 = su.row0 + ((p * SC_NQ) >> lb);
       for (int kt = kt_lo; kt < kt_hi; ++kt) {
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          const int p = e + 2 * u;
-          if (!sc_part_active(su, kt, p)) continue;
-          const int pq0 = su.q0 + p * SC_NQ;
-          const int q_last = min(pq0 + SC_NQ, su.n) - 1;
-          mbar_wait(&bar.accfull[p], use[u] & 1);
-          tc_fence_after_sync();
-          sc_epilogue(trow0 + p * SC_NQ, wq, lane, kt * SC_KT, pq0, su.row0 + ((p * SC_NQ) >> lb), q_last, b, lb,
-                      idx_scale, local_window, local_bias, row_begin, row_count, scores, ld);
-          tc_fence_before_sync();
-          mbar_arrive(&bar.accempty[p]);
-          ++use[u];
-        }
+        if (!sc_part_active(su, kt, p)) continue;
+        mbar_wait(&bar.accfull[p], use & 1);
+        tc_fence_after_sync();
+        sc_epilogue(trow, wq, lane, kt * SC_KT, pq0, prow0, q_last, b, lb, idx_scale, local_window, local_bias,
+                    row_begin, row_count, scores, ld);
+        tc_fence_before_sync();
+        mbar_arrive(&bar.accempty[p]);
+        ++use;
       }
     }
   }

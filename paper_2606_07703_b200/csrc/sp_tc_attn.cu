@@ -38,6 +38,21 @@ __device__ __forceinline__ bool elect_one() {
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
   return pred != 0;
 }
+__device__ __forceinline__ void mbar_wait_addr(uint32_t addr, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive_addr(uint32_t addr) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
+}
 __device__ __forceinline__ void loader_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 // D[tmem] (+)= A[tmem] * B[smem]: A = 128 lanes x (K/2) 32-bit columns of packed bf16 pairs (K-major).
@@ -74,6 +89,32 @@ __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+// exp2 of two fp32 values on the FMA / ALU pipes: round-to-nearest split x = n + f (magic-number add), degree-4
+// minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 2.7e-6 in fp32 Horner form), exponent patched
+// in with an integer add.  Inputs are clamped to >= -125 (result ~2^-125, i.e. 0 for every use here).
+#ifndef AT_POLY_EVERY
+#define AT_POLY_EVERY 8  // one pair in AT_POLY_EVERY takes the polynomial path (0 = never)
+#endif
+__device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  f2_unpack(x2, x0, x1);
+  x0 = fmaxf(x0, -125.f);
+  x1 = fmaxf(x1, -125.f);
+  const uint64_t xc = f2_pack(x0, x1);
+  const uint64_t magic = f2_pack(12582912.f, 12582912.f);  // 1.5 * 2^23
+  const uint64_t t = f2_add(xc, magic);
+  const uint64_t nf = f2_add(t, f2_pack(-12582912.f, -12582912.f));
+  const uint64_t f = f2_fma(nf, f2_pack(-1.f, -1.f), xc);
+  uint64_t q = f2_fma(f, f2_pack(0.009570099413394928f, 0.009570099413394928f), f2_pack(0.05591785907745361f, 0.05591785907745361f));
+  q = f2_fma(q, f, f2_pack(0.240247443318367f, 0.240247443318367f));
+  q = f2_fma(q, f, f2_pack(0.6931217908859253f, 0.6931217908859253f));
+  q = f2_fma(q, f, f2_pack(0.9999992847442627f, 0.9999992847442627f));
+  float q0, q1, t0, t1;
+  f2_unpack(q, q0, q1);
+  f2_unpack(t, t0, t1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
 }
 __device__ __forceinline__ uint32_t bf16x2_rn(float lo, float hi) {
   uint32_t r;
@@ -153,7 +194,9 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   const int NS = n_stages;
   const int P = gridDim.x, cta = blockIdx.x;
 
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  // 1024-byte alignment as an OFFSET from the shared array, so the compiler keeps the shared address space
+  // (LDS / STS instead of generic loads) for everything carved from it
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint8_t* sQ = smem;
   uint8_t* sK = sQ + KB * Q_BLK;
   uint8_t* sV = sK + NS * KV_TILE;
@@ -304,25 +347,26 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     cp_async_wait<0>();
   } else if (warp == AT_MMA_WARP || warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS) {
     // =========================================== MMA issuers ===========================================
-    // Four issuing warps: S = Q K^T of M tile 0 / 1 (warps 8, 13) and O += P V of M tile 0 / 1 (warps 14, 15).
-    // One warp issuing everything needs ~200 dependent uniform-datapath instructions per key tile (~2000
-    // cycles) and paces the whole CTA; split four ways every issuer stays well under the 1024 cycles the
-    // tensor pipe needs per tile.  The whole warp runs the (warp-uniform) control flow and the mbarrier waits;
-    // one elected lane issues tcgen05.mma / tcgen05.commit.  K / V stages and the Q buffer are released by
-    // BOTH M tiles (barrier count 2; an M tile without work for a tile arrives without MMAs).
+    // One issuing warp per M tile (warps 8 and 13; 14, 15 idle).  Per key tile j it waits for softmax(j), issues
+    // O += P V (j) and then S(j+2) = Q K^T into the S buffer that PV(j) just consumed: both come from the same
+    // thread, so the tensor pipe orders them and no completion round trip sits between "P(j) written" and
+    // "S(j+2) ready".  A single warp issuing for BOTH M tiles (~200 dependent uniform-datapath instructions per
+    // tile) paced the whole CTA; split per M tile it stays under the ~1000 cycles a tile occupies the tensor pipe.
+    // The whole warp runs the (warp-uniform) control flow and the mbarrier waits; one elected lane issues
+    // tcgen05.mma / tcgen05.commit.  K / V stages and the Q buffer are released by BOTH M tiles (barrier count 2;
+    // an M tile without work for a tile arrives without MMAs).
     asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
     const bool leader = elect_one();
-    const int role_pv = warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS + 1;  // warps 14, 15
-    const int mt = (warp == AT_MMA_WARP || warp == AT_LOAD_WARP0 + AT_LOAD_WARPS + 1) ? 0 : 1;
-    if (!(role_pv && !WITH_O)) {
+    const int mt = warp == AT_MMA_WARP ? 0 : 1;
+    if (warp == AT_MMA_WARP || warp == AT_LOAD_WARP0 + AT_LOAD_WARPS) {
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, AT_KT, 0, 0);  // S = Q K^T : both K-major
       constexpr uint32_t idesc_o = umma_idesc_bf16(128, D, 0, 1);      // O += P V : P from TMEM, V MN-major
       const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ) + mt * 16384, 16, 1024);
       const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
       const uint64_t vdesc0 = umma_desc_sw128(smem_u32(sV), KV_BLK, 1024);
-      uint32_t r_s = 0, r_ph = 0;            // K (S role) or V (PV role) ring position of the next tile
-      uint32_t n_q = 0, n_it = 0, n_o = 0;   // items with work / items seen / items this M tile was active in
-      uint32_t ct = 0;                       // tiles issued by this warp (S buffer = ct & 1)
+      uint32_t k_s = 0, k_ph = 0, v_s = 0, v_ph = 0;  // K / V ring positions of the next tile this warp consumes
+      uint32_t n_q = 0, n_it = 0, n_o = 0;            // items with work / items seen / items this M tile was active in
+      uint32_t cs = 0, cp = 0;                        // S tiles issued / PV tiles issued by this warp (buffer = & 1)
       for (int i = 0; i * P < n_items; ++i) {
         const int id = at_item_id(i, cta, P, n_items);
         AtItem it;
@@ -342,75 +386,78 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
         if (mt >= n_mt) my_nt = 0;
         ++n_it;
         if (nt == 0) continue;
-        if (!role_pv) {
-          mbar_wait(&bar.qfull, n_q & 1);
+        auto adv_k = [&]() {
+          if (++k_s == (uint32_t)NS) {
+            k_s = 0;
+            k_ph ^= 1;
+          }
+        };
+        auto adv_v = [&]() {
+          if (++v_s == (uint32_t)NS) {
+            v_s = 0;
+            v_ph ^= 1;
+          }
+        };
+        auto issue_s = [&](int j) {  // S(j) into buffer cs & 1 (free: its previous tile's PV was issued by this thread)
+          mbar_wait(&bar.kfull[k_s], k_ph);
           fence_proxy_async_smem();
           tc_fence_after_sync();
-          for (int j = 0; j < nt; ++j) {
-            mbar_wait(&bar.kfull[r_s], r_ph);
-            if (j < my_nt) {
-              fence_proxy_async_smem();
-              const uint32_t b = ct & 1, n = ct >> 1;
-              if (n > 0) {  // the buffer's previous tile: its P has been consumed (PV) / its S has been read
-                if (WITH_O) mbar_wait(&bar.pfree[mt][b], (n - 1) & 1);
-                else mbar_wait(&bar.sdone[mt][b], (n - 1) & 1);
-              }
-              tc_fence_after_sync();
-              if (leader) {
-                const uint32_t d_s = tmem + TM_S + mt * 128 + b * 64;
-                const uint64_t kd = kdesc0 + (uint64_t)((r_s * KV_TILE) >> 4);
+          if (leader) {
+            const uint32_t d_s = tmem + TM_S + mt * 128 + (cs & 1) * 64;
+            const uint64_t kd = kdesc0 + (uint64_t)((k_s * KV_TILE) >> 4);
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk) {
-                  umma_ss(d_s, qdesc0 + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
-                          kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
-                }
-                umma_commit(&bar.sfull[mt][b]);
-                umma_commit(&bar.kempty[r_s]);
-              }
-              ++ct;
-            } else if (leader) {
-              mbar_arrive(&bar.kempty[r_s]);
+            for (int kk = 0; kk < D / 16; ++kk) {
+              umma_ss(d_s, qdesc0 + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
+                      kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
             }
-            if (++r_s == (uint32_t)NS) {
-              r_s = 0;
-              r_ph ^= 1;
-            }
+            umma_commit(&bar.sfull[mt][cs & 1]);
+            umma_commit(&bar.kempty[k_s]);
+            if (j == my_nt - 1) umma_commit(&bar.qempty);  // every S MMA of the item is issued: Q is free when they finish
           }
-          if (leader) {  // every S MMA of the item has been issued: Q is free when they finish
-            if (my_nt > 0) umma_commit(&bar.qempty);
-            else mbar_arrive(&bar.qempty);
+          ++cs;
+          adv_k();
+        };
+        mbar_wait(&bar.qfull, n_q & 1);
+        fence_proxy_async_smem();
+        tc_fence_after_sync();
+        if (my_nt == 0 && leader) mbar_arrive(&bar.qempty);
+        for (int j = 0; j < 2 && j < my_nt; ++j) issue_s(j);
+        for (int j = 0; j < my_nt; ++j) {
+          const uint32_t b = cp & 1, n = cp >> 1;
+          if (WITH_O) {
+            mbar_wait(&bar.vfull[v_s], v_ph);
+            fence_proxy_async_smem();
           }
-        } else {
-          for (int j = 0; j < nt; ++j) {
-            mbar_wait(&bar.vfull[r_s], r_ph);
-            if (j < my_nt) {
-              fence_proxy_async_smem();
-              const uint32_t b = ct & 1, n = ct >> 1;
-              mbar_wait(&bar.sdone[mt][b], n & 1);  // softmax(j) has written P over S
-              if (j == 0 && n_o > 0) mbar_wait(&bar.oempty[mt], (n_o - 1) & 1);
-              tc_fence_after_sync();
-              if (leader) {
-                const uint64_t vd = vdesc0 + (uint64_t)((r_s * KV_TILE) >> 4);
-                const uint32_t d_o = tmem + TM_O + mt * D, a_p = tmem + TM_S + mt * 128 + b * 64;
+          mbar_wait(&bar.sdone[mt][b], n & 1);  // softmax(j) has read S (and written P over it)
+          if (WITH_O) {
+            if (j == 0 && n_o > 0) mbar_wait(&bar.oempty[mt], (n_o - 1) & 1);
+            tc_fence_after_sync();
+            if (leader) {
+              const uint64_t vd = vdesc0 + (uint64_t)((v_s * KV_TILE) >> 4);
+              const uint32_t d_o = tmem + TM_O + mt * D, a_p = tmem + TM_S + mt * 128 + b * 64;
 #pragma unroll
-                for (int kk = 0; kk < AT_KT / 16; ++kk)
-                  umma_ts(d_o, a_p + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_o, (j | kk) != 0);
-                umma_commit(&bar.pfree[mt][b]);
-                umma_commit(&bar.ofull[mt]);
-                if (j == my_nt - 1) umma_commit(&bar.ofin[mt]);
-                umma_commit(&bar.vempty[r_s]);
-              }
-              ++ct;
-            } else if (leader) {
-              mbar_arrive(&bar.vempty[r_s]);
+              for (int kk = 0; kk < AT_KT / 16; ++kk)
+                umma_ts(d_o, a_p + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_o, (j | kk) != 0);
+              umma_commit(&bar.ofull[mt]);
+              if (j == my_nt - 1) umma_commit(&bar.ofin[mt]);
+              umma_commit(&bar.vempty[v_s]);
             }
-            if (++r_s == (uint32_t)NS) {
-              r_s = 0;
-              r_ph ^= 1;
-            }
+            adv_v();
           }
-          if (my_nt > 0) ++n_o;
+          ++cp;
+          if (j + 2 < my_nt) issue_s(j + 2);
         }
+        for (int j = my_nt; j < nt; ++j) {  // tiles only the other M tile reads: keep the ring counts in step
+          mbar_wait(&bar.kfull[k_s], k_ph);
+          if (leader) mbar_arrive(&bar.kempty[k_s]);
+          adv_k();
+          if (WITH_O) {
+            mbar_wait(&bar.vfull[v_s], v_ph);
+            if (leader) mbar_arrive(&bar.vempty[v_s]);
+            adv_v();
+          }
+        }
+        if (WITH_O && my_nt > 0) ++n_o;
         ++n_q;
       }
     }
@@ -425,6 +472,8 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     const uint32_t lane_base = (uint32_t)((warp % 4) * 32) << 16;
     const uint32_t t_o = tmem + lane_base + TM_O + mt * D;
     const uint64_t sl2_2 = f2_pack(sl2, sl2);
+    const uint32_t t_s0 = tmem + lane_base + TM_S + mt * 128;
+    const uint32_t a_sfull = smem_u32(&bar.sfull[mt][0]), a_sdone = smem_u32(&bar.sdone[mt][0]);  // 32-bit barrier addresses
     uint32_t cs = 0, n_it = 0, n_ep = 0;  // S tiles consumed by this M tile (== PVs issued for it), items seen, epilogues
     for (int i = 0; i * P < n_items; ++i) {
       const int id = at_item_id(i, cta, P, n_items);
@@ -453,8 +502,8 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
         float m_run = -INFINITY, l_run = 0.f;
         for (int j = 0; j < my_nt; ++j, ++cs) {
           const uint32_t b = cs & 1;
-          const uint32_t t_s = tmem + lane_base + TM_S + mt * 128 + b * 64;
-          mbar_wait(&bar.sfull[mt][b], (cs >> 1) & 1);
+          const uint32_t t_s = t_s0 + b * 64;
+          mbar_wait_addr(a_sfull + b * 8, (cs >> 1) & 1);
           tc_fence_after_sync();
           uint32_t v[AT_KT];
           tmem_ld_x32(t_s, v);
@@ -466,6 +515,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
           else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
           flagged = flagged || !scale_pos;
           float mx;
+          float xs[AT_KT];  // flagged tiles only: scaled, biased, masked logits (v itself is never written)
           if (!flagged) {
             float a0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1]));
             float a1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
@@ -496,7 +546,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
               }
               float x = -INFINITY;
               if (ok) x = fmaf(__uint_as_float(v[cc]), sl2, (win > 0 && dist < win) ? lb2 : 0.f);
-              v[cc] = __float_as_uint(x);  // already scaled
+              xs[cc] = x;
               mx = fmaxf(mx, x);
             }
           }
@@ -529,17 +579,24 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
             const uint64_t nm2 = f2_pack(-m_off, -m_off);
 #pragma unroll
             for (int cc = 0; cc < AT_KT; cc += 2) {
-              float x0, x1;
-              f2_unpack(f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2), x0, x1);
-              const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+              const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2);
+              float p0, p1;
+              if (WITH_O && AT_POLY_EVERY > 0 && (cc / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
+                ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
+              } else {
+                float x0, x1;
+                f2_unpack(x2, x0, x1);
+                p0 = ex2_approx(x0);
+                p1 = ex2_approx(x1);
+              }
               sum2 = f2_add(sum2, f2_pack(p0, p1));
               pk[cc / 2] = bf16x2_rn(p0, p1);
             }
           } else {
 #pragma unroll
             for (int cc = 0; cc < AT_KT; cc += 2) {
-              const float p0 = ex2_approx(__uint_as_float(v[cc]) - m_off);
-              const float p1 = ex2_approx(__uint_as_float(v[cc + 1]) - m_off);
+              const float p0 = ex2_approx(xs[cc] - m_off);
+              const float p1 = ex2_approx(xs[cc + 1] - m_off);
               sum2 = f2_add(sum2, f2_pack(p0, p1));
               pk[cc / 2] = bf16x2_rn(p0, p1);
             }
@@ -554,7 +611,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
             tmem_st_wait();
           }
           tc_fence_before_sync();
-          mbar_arrive(&bar.sdone[mt][b]);
+          mbar_arrive_addr(a_sdone + b * 8);
         }
         // ---- epilogue ----
         if (WITH_O) {

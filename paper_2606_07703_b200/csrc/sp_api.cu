@@ -149,19 +149,36 @@ cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const flo
                         row_count, max_nv, mass, ld, st);
 }
 
-// idx == nullptr -> dense.  [q_begin, q_begin + q_count) must be the whole pack for the tcgen05 kernel.
+// idx == nullptr -> dense.  The tcgen05 kernel covers the whole pack, or -- dense and LSE-only (O == nullptr,
+// the oracle's pass 1 of a row panel) -- the query chunks that intersect [q_begin, q_begin + q_count): rows of a
+// boundary chunk outside the range get their lse too, which is harmless.
 cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
                      int q_count, void* O, float* lse, cudaStream_t st) {
   const SpGeom g = dev_geom(p);
   const int G = p->Hq / p->Hkv;
   const bool whole = q_begin == 0 && q_count == p->L;
-  if (whole && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k, p->d)) {
+  const bool dense_lse_range = idx == nullptr && O == nullptr && q_count > 0;
+  if ((whole || dense_lse_range) && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k, p->d)) {
     const HostGeom hg = host_geom(p);
     const int QT = 256 / G;
-    long long chunks = 0;
-    for (int i = 0; i < hg.batch; ++i) chunks += (hg.seq_len(i) + QT - 1) / QT;
-    return sp_launch_attn_tc(g, hg.num_rows(), chunks, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p),
-                             p->local_window, p->local_bias, O, lse, st);
+    long long chunks = 0, c_lo = -1, c_hi = -1;
+    const long long q_lo = q_begin, q_hi = (long long)q_begin + q_count - 1;
+    for (int i = 0; i < hg.batch; ++i) {
+      const long long s0 = hg.seq_start(i), n = hg.seq_len(i);
+      const long long lo = q_lo > s0 ? q_lo : s0, hi = q_hi < s0 + n - 1 ? q_hi : s0 + n - 1;
+      if (lo <= hi) {
+        if (c_lo < 0) c_lo = chunks + (lo - s0) / QT;
+        c_hi = chunks + (hi - s0) / QT;
+      }
+      chunks += (n + QT - 1) / QT;
+    }
+    if (idx != nullptr || whole) {
+      c_lo = 0;
+      c_hi = chunks - 1;
+    }
+    if (c_lo < 0) return cudaSuccess;
+    return sp_launch_attn_tc(g, hg.num_rows(), c_hi - c_lo + 1, c_lo, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d,
+                             attn_scale(p), p->local_window, p->local_bias, O, lse, st);
   }
   return sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
                         q_begin, q_count, O, lse, st);

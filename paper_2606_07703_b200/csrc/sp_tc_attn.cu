@@ -141,7 +141,7 @@ struct AtItem {
 
 // Work item `id` -> queries and KV head.  Identical in every warp role.
 template <int G, bool SPARSE>
-__device__ __forceinline__ bool at_item(const SpGeom& g, int id, int Hkv, int cpr, int n_chunks, AtItem& it) {
+__device__ __forceinline__ bool at_item(const SpGeom& g, int id, int Hkv, int cpr, int n_chunks, int chunk_base, AtItem& it) {
   constexpr int QT = 256 / G;
   it.kvh = id % Hkv;
   const int x = id / Hkv;
@@ -155,7 +155,7 @@ __device__ __forceinline__ bool at_item(const SpGeom& g, int id, int Hkv, int cp
   } else {
     SpGeom g2 = g;
     g2.b_sel = QT;
-    it.row = n_chunks - 1 - x;  // heavy (late) chunks first
+    it.row = chunk_base + n_chunks - 1 - x;  // heavy (late) chunks first
     const SpRow ri = sp_row_info(g2, it.row);
     it.seq_start = ri.seq_start;
     it.t0 = ri.t_first;
@@ -175,8 +175,8 @@ template <int D, int G, bool SPARSE, bool WITH_O>
 __global__ void __launch_bounds__(AT_THREADS, 1)
 sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
-                  int local_window, float local_bias, int chunks_per_row, int n_chunks, int n_items, int n_stages,
-                  int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
+                  int local_window, float local_bias, int chunks_per_row, int n_chunks, int chunk_base, int n_items,
+                  int n_stages, int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
   constexpr int KB = D / 64;              // 64-wide column blocks of a row
   constexpr int CPR = D / 8;              // 16-byte chunks per row
   constexpr uint32_t Q_BLK = 256 * 128;   // bytes of one column block of the Q tile (256 rows)
@@ -254,7 +254,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     for (int i = 0; i * P < n_items; ++i) {
       const int id = at_item_id(i, cta, P, n_items);
       AtItem it;
-      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, chunk_base, it)) continue;
       const int nq = it.t1 - it.t0 + 1;
       const int n_mt = (nq * G > 128) ? 2 : 1;
       int nt;
@@ -370,7 +370,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       for (int i = 0; i * P < n_items; ++i) {
         const int id = at_item_id(i, cta, P, n_items);
         AtItem it;
-        if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+        if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, chunk_base, it)) continue;
         const int nq = it.t1 - it.t0 + 1;
         const int n_mt = (nq * G > 128) ? 2 : 1;
         int nt, my_nt;
@@ -478,7 +478,7 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     for (int i = 0; i * P < n_items; ++i) {
       const int id = at_item_id(i, cta, P, n_items);
       AtItem it;
-      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, it)) continue;
+      if (id < 0 || !at_item<G, SPARSE>(g, id, Hkv, chunks_per_row, n_chunks, chunk_base, it)) continue;
       const int nq = it.t1 - it.t0 + 1;
       const int n_mt = (nq * G > 128) ? 2 : 1;
       int my_nt;
@@ -686,7 +686,7 @@ int at_sm_count() {
 template <int D, int G, bool SPARSE, bool WITH_O>
 cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
                        const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks,
-                       int n_items, void* O, float* lse) {
+                       int chunk_base, int n_items, void* O, float* lse) {
   const int kpad = SPARSE ? (k + AT_KT - 1) / AT_KT * AT_KT : 0;
   const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O);
   if (stages < 2) return cudaErrorInvalidValue;
@@ -701,31 +701,31 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
   const int grid = n_items < at_sm_count() ? n_items : at_sm_count();
   sp_tc_attn_kernel<D, G, SPARSE, WITH_O><<<grid, AT_THREADS, smem, st>>>(
       g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, cpr,
-      n_chunks, n_items, stages, kpad, (__nv_bfloat16*)O, lse);
+      n_chunks, chunk_base, n_items, stages, kpad, (__nv_bfloat16*)O, lse);
   return cudaGetLastError();
 }
 
 template <int D, int G>
 cudaError_t launch_dg(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V, const int32_t* idx,
-                      int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks, int n_items, void* O,
+                      int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks, int chunk_base, int n_items, void* O,
                       float* lse) {
   if (idx != nullptr) {
-    if (O) return launch_one<D, G, true, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
-    return launch_one<D, G, true, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    if (O) return launch_one<D, G, true, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
+    return launch_one<D, G, true, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
   }
-  if (O) return launch_one<D, G, false, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
-  return launch_one<D, G, false, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+  if (O) return launch_one<D, G, false, true>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
+  return launch_one<D, G, false, false>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
 }
 
 template <int D>
 cudaError_t launch_d(int G, const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
                      const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks,
-                     int n_items, void* O, float* lse) {
+                     int chunk_base, int n_items, void* O, float* lse) {
   switch (G) {
-    case 1: return launch_dg<D, 1>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
-    case 2: return launch_dg<D, 2>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
-    case 4: return launch_dg<D, 4>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
-    case 8: return launch_dg<D, 8>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, n_items, O, lse);
+    case 1: return launch_dg<D, 1>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
+    case 2: return launch_dg<D, 2>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
+    case 4: return launch_dg<D, 4>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
+    case 8: return launch_dg<D, 8>(g, st, Q, K, V, idx, k, Hkv, scale, lw, lb, cpr, n_chunks, chunk_base, n_items, O, lse);
   }
   return cudaErrorInvalidValue;
 }
@@ -741,10 +741,12 @@ bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d) {
   return (d == 128 ? attn_pick_stages<128>(kpad, true, true) : attn_pick_stages<64>(kpad, true, true)) >= 2;
 }
 
-// idx == nullptr -> dense causal attention over the whole pack.  n_chunks_dense = sum_i ceil(n_i / (256/G)).
-cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, const void* Q, const void* K,
-                              const void* V, const int32_t* idx, int k, int Hq, int Hkv, int d, float scale,
-                              int local_window, float local_bias, void* O, float* lse, cudaStream_t st) {
+// idx == nullptr -> dense causal attention over the query chunks [chunk_base, chunk_base + n_chunks_dense) of the
+// pack (a chunk = 256/G consecutive queries of one sequence; the whole pack has sum_i ceil(n_i / (256/G)) chunks).
+cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, long long chunk_base,
+                              const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hq, int Hkv,
+                              int d, float scale, int local_window, float local_bias, void* O, float* lse,
+                              cudaStream_t st) {
   const int G = Hq / Hkv;
   const int QT = 256 / G;
   const bool sparse = idx != nullptr;
@@ -754,9 +756,9 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
   if (nx * Hkv > 0x7fffffffLL) return cudaErrorInvalidValue;
   const int n_items = (int)(nx * Hkv);
   cudaError_t e = d == 128 ? launch_d<128>(G, g, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr,
-                                           (int)nx, n_items, O, lse)
+                                           (int)nx, sparse ? 0 : (int)chunk_base, n_items, O, lse)
                            : launch_d<64>(G, g, st, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, cpr,
-                                          (int)nx, n_items, O, lse);
+                                          (int)nx, sparse ? 0 : (int)chunk_base, n_items, O, lse);
   sp_count_launch();
   return e;
 }

@@ -190,6 +190,32 @@ def test_mass_matches_oracle(cfg, b, lw):
         assert np.allclose(sums, 1.0, atol=1e-4)
 
 
+@pytest.mark.parametrize("cfg,b", [(SMALL_ORC, 1), (SMALL_ORC128, 1), (SMALL_ORC128, 64)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_mass_row_panel_matches_oracle(cfg, b):
+    """A row PANEL through sp_oracle_mass with the normalisers computed inside the call: pass 1 then runs over the
+    query chunks that intersect the panel only (tcgen05 dense kernel, LSE only), pass 2 over the panel's rows."""
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(b_sel=b, local_window=16, local_bias=0.75)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    rows = pbg.num_rows
+    r0, cnt = rows // 3, max(1, rows // 2)
+    R, nv = orc.support_scores(pbo, orc.MODE_ORACLE, inp["Q"], inp["K"], np.arange(r0, r0 + cnt))
+    mass = torch.full((cnt, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
+    lse = torch.full((cfg.L, cfg.Hq), float("nan"), dtype=torch.float32, device=DEV)
+    B.sp_oracle_mass(pbg, dev(inp["Q"]), dev(inp["K"]), lse, False, r0, cnt, mass)
+    got = to_f64(mass)
+    for i in range(cnt):
+        n = int(nv[i])
+        assert np.all(np.abs(got[i, :n] - R[i, :n]) <= 1e-4 * R[i, :n] + 1e-12), (r0 + i)
+    # the panel's queries got their normalisers
+    q_lo, q_hi = r0 * b, min(cfg.L, (r0 + cnt) * b)
+    pos = np.arange(q_lo, q_hi, 5)
+    _, lse_o = orc.dense_attn(pbo, inp["Q"], inp["K"], inp["V"], pos, want_lse=True)
+    assert np.allclose(to_f64(lse)[pos], lse_o, rtol=0, atol=2e-5)
+
+
 # ------------------------------------------------------------------ a6/a7 attention: stage-isolated
 
 @pytest.mark.parametrize("cfg,b,k", [(SMALL_ORC, 1, 96), (SMALL_ORC, 64, 96), (SMALL_ORC128, 1, 64),

@@ -1,6 +1,6 @@
 // sp_tc_mass.cu -- oracle attention mass, pass 2, on tcgen05 / TMEM / TMA (Alg.1 step 3 :143):
 //   P[t,s] = (1/Hq) sum_h exp(z[t,h,s] - lse[t,h]),  z = scale <q_{t,h}, k_{s,g(h)}> (+ local term),  s <= t
-// for per-query supports (b_sel == 1; block-shared oracle rows stay on the CUDA-core kernel of sp_simt.cu).
+// and, for block-shared rows (b_sel in {32, 64, 128}), R_B(s) = max over the block's queries.
 //
 // Persistent, warp specialised.  A work item = 128 consecutive queries of one sequence (MMA M, TMEM lane =
 // query, so lse[t,h] is a per-thread scalar) x 256 consecutive keys (MMA N); only lower-triangular items exist.
@@ -20,7 +20,7 @@ namespace {
 constexpr int MS_MQ = 128;        // queries per item (MMA M)
 constexpr int MS_NK = 256;        // keys per item (MMA N)
 constexpr int MS_THREADS = 384;   // warps 0-3 / 4-7: epilogue of key columns 0-127 / 128-255; 8: TMA; 9: MMA; 10-11 idle
-constexpr int MS_QSTAGES = 3;
+constexpr int MS_QSTAGES = 2;
 
 __device__ __forceinline__ uint8_t* ms_align1024(uint8_t* p) {
   return reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(p) + 1023) & ~(uintptr_t)1023);
@@ -56,19 +56,22 @@ __device__ __forceinline__ float ms_ex2(float x) {
 
 struct MsTile {
   int seq_start, n, q0;  // sequence start (packed), sequence length, first LOCAL query of the 128-query tile
+  int row0;              // support row of the tile's first query
 };
 
 // linear query-tile index over the pack -> geometry
 __device__ __forceinline__ MsTile ms_tile_info(const SpGeom& g, int qt) {
-  if (g.cu == nullptr) return MsTile{0, g.L, qt * MS_MQ};
-  int t0 = 0;
+  const int b = g.b_sel;
+  if (g.cu == nullptr) return MsTile{0, g.L, qt * MS_MQ, qt * MS_MQ / b};
+  int t0 = 0, r0 = 0;
   for (int i = 0; i < g.batch; ++i) {
     const int s = g.cu[i], n = g.cu[i + 1] - s;
     const int nt = (n + MS_MQ - 1) / MS_MQ;
-    if (qt < t0 + nt) return MsTile{s, n, (qt - t0) * MS_MQ};
+    if (qt < t0 + nt) return MsTile{s, n, (qt - t0) * MS_MQ, r0 + (qt - t0) * MS_MQ / b};
     t0 += nt;
+    r0 += (n + b - 1) / b;
   }
-  return MsTile{0, 0, 0};
+  return MsTile{0, 0, 0, 0};
 }
 // key tiles of a query tile: every 256-key tile that starts at or below the tile's last query
 __device__ __forceinline__ int ms_nkt(const MsTile& t) { return (min(t.q0 + MS_MQ, t.n) - 1) / MS_NK + 1; }
@@ -90,6 +93,35 @@ __device__ __forceinline__ void ms_segment(int nkt, long long B, const MsRange& 
   kt_hi = z > a ? (int)z : (int)a;
 }
 
+// Max over the 32 lanes of a warp for 32 columns at once (reduce-scatter butterfly, 31 shuffles): on return lane l
+// holds the maximum of column l.
+__device__ __forceinline__ float ms_warp_colmax32(const float* x, int lane) {
+  float y16[16], y8[8], y4[4], y2[2];
+  const bool b16 = lane & 16, b8 = lane & 8, b4 = lane & 4, b2 = lane & 2, b1 = lane & 1;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const float mine = b16 ? x[16 + i] : x[i], other = b16 ? x[i] : x[16 + i];
+    y16[i] = fmaxf(mine, __shfl_xor_sync(0xffffffffu, other, 16));
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float mine = b8 ? y16[8 + i] : y16[i], other = b8 ? y16[i] : y16[8 + i];
+    y8[i] = fmaxf(mine, __shfl_xor_sync(0xffffffffu, other, 8));
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float mine = b4 ? y8[4 + i] : y8[i], other = b4 ? y8[i] : y8[4 + i];
+    y4[i] = fmaxf(mine, __shfl_xor_sync(0xffffffffu, other, 4));
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const float mine = b2 ? y4[2 + i] : y4[i], other = b2 ? y4[i] : y4[2 + i];
+    y2[i] = fmaxf(mine, __shfl_xor_sync(0xffffffffu, other, 2));
+  }
+  const float mine = b1 ? y2[1] : y2[0], other = b1 ? y2[0] : y2[1];
+  return fmaxf(mine, __shfl_xor_sync(0xffffffffu, other, 1));
+}
+
 struct MsBarriers {
   uint64_t qfull[MS_QSTAGES], qempty[MS_QSTAGES];
   uint64_t kfull[2], kempty[2];
@@ -108,11 +140,13 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   extern __shared__ uint8_t smem_raw[];
   __shared__ MsBarriers bar;
   __shared__ uint32_t tmem_slot;
+  __shared__ float ms_x[2][4][128];  // block-shared rows: per-warp column maxima of one warpgroup's 128 key columns
   uint8_t* smem = ms_align1024(smem_raw);
   uint8_t* sQ = smem;                         // [stage][kb] boxes of 128 rows x 128 B
   uint8_t* sK = smem + MS_QSTAGES * Q_STAGE;  // [buf][kb] boxes of 256 rows x 128 B
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int G = Hq / Hkv;
+  const int b_sel = g.b_sel;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < MS_QSTAGES; ++s) {
@@ -297,25 +331,67 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             }
           }
         }
-        // ---- mean over heads, write this thread's row segment ----
-        const int row = ti.seq_start + tl;  // b_sel == 1: support row == packed position
-        if (t_ok && row >= row_begin && row < row_begin + row_count && sc0 <= tl) {
-          float* dst = mass + (size_t)(row - row_begin) * ld + sc0;
-          if (vec_ok && sc0 + 127 <= tl) {
+        if (b_sel == 1) {
+          // ---- mean over heads, write this thread's row segment ----
+          const int row = ti.seq_start + tl;  // b_sel == 1: support row == packed position
+          if (t_ok && row >= row_begin && row < row_begin + row_count && sc0 <= tl) {
+            float* dst = mass + (size_t)(row - row_begin) * ld + sc0;
+            if (vec_ok && sc0 + 127 <= tl) {
 #pragma unroll
-            for (int c = 0; c < 64; c += 2) {
-              float a0, a1, a2, a3;
-              ms_unpack(acc[c], a0, a1);
-              ms_unpack(acc[c + 1], a2, a3);
-              reinterpret_cast<float4*>(dst)[c >> 1] = make_float4(a0 * inv_hq, a1 * inv_hq, a2 * inv_hq, a3 * inv_hq);
+              for (int c = 0; c < 64; c += 2) {
+                float a0, a1, a2, a3;
+                ms_unpack(acc[c], a0, a1);
+                ms_unpack(acc[c + 1], a2, a3);
+                reinterpret_cast<float4*>(dst)[c >> 1] = make_float4(a0 * inv_hq, a1 * inv_hq, a2 * inv_hq, a3 * inv_hq);
+              }
+            } else {
+#pragma unroll
+              for (int c = 0; c < 64; ++c) {
+                float a0, a1;
+                ms_unpack(acc[c], a0, a1);
+                if (sc0 + 2 * c <= tl) dst[2 * c] = a0 * inv_hq;
+                if (sc0 + 2 * c + 1 <= tl) dst[2 * c + 1] = a1 * inv_hq;
+              }
             }
-          } else {
+          }
+        } else {
+          // ---- block-shared rows: R_B(s) = max over the block's queries of the head mean.  Masked
+          // (s > t) and out-of-sequence pairs contributed exactly 0, below every valid mass.  Lanes of a warp are 32
+          // consecutive queries: reduce-scatter over the lanes, then over the warps of the block through shared memory.
+          float red[4];
 #pragma unroll
-            for (int c = 0; c < 64; ++c) {
+          for (int gq = 0; gq < 4; ++gq) {
+            float x[32];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
               float a0, a1;
-              ms_unpack(acc[c], a0, a1);
-              if (sc0 + 2 * c <= tl) dst[2 * c] = a0 * inv_hq;
-              if (sc0 + 2 * c + 1 <= tl) dst[2 * c + 1] = a1 * inv_hq;
+              ms_unpack(acc[16 * gq + c], a0, a1);
+              x[2 * c] = a0 * inv_hq;
+              x[2 * c + 1] = a1 * inv_hq;
+            }
+            red[gq] = ms_warp_colmax32(x, lane);
+          }
+          const int wpb = b_sel >> 5;  // warps per block: 1, 2 or 4
+          if (wpb > 1) {
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");  // previous item's readers are done
+#pragma unroll
+            for (int gq = 0; gq < 4; ++gq) ms_x[e][wq][32 * gq + lane] = red[gq];
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");
+          }
+          if ((wq & (wpb - 1)) == 0) {  // first warp of its block writes
+            const int bq0 = ti.q0 + 32 * wq;
+            if (bq0 < ti.n) {
+              const int blk_last = min(bq0 + b_sel - 1, ti.n - 1);
+              const int row = ti.row0 + (32 * wq) / b_sel;
+              if (row >= row_begin && row < row_begin + row_count) {
+#pragma unroll
+                for (int gq = 0; gq < 4; ++gq) {
+                  float v = red[gq];
+                  for (int w = 1; w < wpb; ++w) v = fmaxf(v, ms_x[e][wq + w][32 * gq + lane]);
+                  const int s = sc0 + 32 * gq + lane;
+                  if (s <= blk_last) mass[(size_t)(row - row_begin) * ld + s] = v;
+                }
+              }
             }
           }
         }
@@ -362,24 +438,29 @@ cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const 
 
 }  // namespace
 
-bool sp_tc_mass_supported(int b_sel, int d) { return b_sel == 1 && (d == 64 || d == 128); }
+bool sp_tc_mass_supported(int b_sel, int d) {
+  return (b_sel == 1 || b_sel == 32 || b_sel == 64 || b_sel == 128) && (d == 64 || d == 128);
+}
 
-// cu_host: HOST copy of cu_seqlens (nullptr = one sequence).  b_sel == 1: support rows are packed positions.
+// cu_host: HOST copy of cu_seqlens (nullptr = one sequence).
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
                               int row_count, float* mass, int64_t ld, cudaStream_t st) {
   if (row_count <= 0) return cudaSuccess;
-  // 128-query tiles (per sequence) that intersect the packed query range [row_begin, row_begin + row_count)
-  long long t0 = 0, items = 0;
+  // 128-query tiles (per sequence) that intersect the support-row panel [row_begin, row_begin + row_count)
+  const int b = g.b_sel;
+  long long t0 = 0, r0 = 0, items = 0;
   long long qlo = -1, qhi = -1;
-  const long long p_lo = row_begin, p_hi = (long long)row_begin + row_count - 1;
   for (int i = 0; i < g.batch; ++i) {
-    const long long s = cu_host ? cu_host[i] : 0;
     const int n = cu_host ? cu_host[i + 1] - cu_host[i] : g.L;
-    const long long nt = (n + MS_MQ - 1) / MS_MQ;
-    const long long lo = p_lo > s ? p_lo : s, hi = p_hi < s + n - 1 ? p_hi : s + n - 1;
+    const long long nr = (n + b - 1) / b, nt = (n + MS_MQ - 1) / MS_MQ;
+    const long long lo = row_begin > r0 ? row_begin : r0;
+    const long long hi = ((long long)row_begin + row_count < r0 + nr ? (long long)row_begin + row_count : r0 + nr) - 1;
     if (lo <= hi) {
-      const long long a = (lo - s) / MS_MQ, z = (hi - s) / MS_MQ;
+      const long long a = (lo - r0) * b / MS_MQ;
+      long long last_q = (hi - r0 + 1) * b - 1;
+      if (last_q > n - 1) last_q = n - 1;
+      const long long z = last_q / MS_MQ;
       if (qlo < 0) qlo = t0 + a;
       qhi = t0 + z;
       for (long long j = a; j <= z; ++j) {
@@ -388,6 +469,7 @@ cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const voi
       }
     }
     t0 += nt;
+    r0 += nr;
   }
   if (qlo < 0) return cudaSuccess;
   const int cnt = (int)(qhi - qlo + 1);

@@ -109,7 +109,7 @@ def oracle_sample_rate(cfg, inp, budget_rows=None):
     kw = {}
     t0 = time.perf_counter()
     if cfg.mode != "oracle":
-        ki = orc.project(pbo, inp["X"], inp["Wki"])
+        ki = orc.project(pbo, inp["X"], inp["Wki"], key=True)
         t_shared = time.perf_counter() - t0
         t1 = time.perf_counter()
         qi = np.zeros((cfg.L, cfg.d_idx), np.uint16)

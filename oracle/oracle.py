@@ -41,7 +41,7 @@ class _Params(C.Structure):
         ("Hq", C.c_int32), ("Hkv", C.c_int32), ("d", C.c_int32), ("k", C.c_int32),
         ("b_sel", C.c_int32), ("hidden", C.c_int32), ("d_idx", C.c_int32),
         ("scale", C.c_double), ("idx_scale", C.c_double),
-        ("local_window", C.c_int32), ("local_bias", C.c_double),
+        ("local_window", C.c_int32), ("local_bias", C.c_double), ("flags", C.c_int32),
     ]
 
 
@@ -61,6 +61,7 @@ class Problem:
     local_window: int = 0
     local_bias: float = 0.0
     cu_seqlens: Optional[Sequence[int]] = None
+    flags: int = 0                       # F_RELU | F_KEY_LN | F_ROPE: the served scorer
 
     def c_params(self):
         cu = None
@@ -74,7 +75,7 @@ class Problem:
             batch, self.L, cu, self.Hq, self.Hkv, self.d, self.k, self.b_sel, self.hidden, self.d_idx,
             self.scale if self.scale is not None else 1.0 / math.sqrt(self.d),
             self.idx_scale if self.idx_scale is not None else (1.0 / math.sqrt(self.d_idx) if self.d_idx else 0.0),
-            self.local_window, self.local_bias,
+            self.local_window, self.local_bias, self.flags,
         )
         p._keep = keep
         return p
@@ -144,14 +145,27 @@ def row_of_pos(pb: Problem, pos: int) -> int:
     return int(lib().orc_row_of_pos(C.byref(p), C.c_int32(pos)))
 
 
-def project(pb: Problem, X, W, rows=None) -> np.ndarray:
-    """O3' projection: bf16_rne(X[rows] @ W) with an fp64 sum (A14)."""
+F_RELU, F_KEY_LN, F_ROPE = 1, 2, 4
+
+
+def project(pb: Problem, X, W, rows=None, key: bool = False) -> np.ndarray:
+    """O3' projection: bf16_rne(T(X[rows] @ W)) with an fp64 sum (A14); T = key LayerNorm
+    (key side only) and RoPE when pb.flags asks for them (A27, A28), else the identity."""
     X, W = _u16(X), _u16(W)
     rows = _i32(np.arange(X.shape[0]) if rows is None else rows)
     out = np.empty((len(rows), pb.d_idx), dtype=np.uint16)
-    lib().orc_project(_ptr(X, C.c_uint16), _ptr(W, C.c_uint16), C.c_int32(pb.hidden), C.c_int32(pb.d_idx),
+    cp = pb.c_params()
+    lib().orc_project(C.byref(cp), _ptr(X, C.c_uint16), _ptr(W, C.c_uint16), C.c_int32(1 if key else 0),
                       _ptr(rows, C.c_int32), C.c_int32(len(rows)), _ptr(out, C.c_uint16))
     return out
+
+
+def transform(y, pos_local: int, flags: int, key: bool) -> np.ndarray:
+    """The fp64 core of the served scorer's per-token transform (LayerNorm then RoPE), for the pins."""
+    y = np.ascontiguousarray(np.asarray(y, dtype=np.float64)).copy()
+    lib().orc_transform(y.ctypes.data_as(C.POINTER(C.c_double)), C.c_int32(y.shape[0]), C.c_int32(pos_local),
+                        C.c_int32(flags), C.c_int32(1 if key else 0))
+    return y
 
 
 def query_scores(pb: Problem, mode: int, A, B, pos, ld: Optional[int] = None) -> np.ndarray:
@@ -262,7 +276,7 @@ def prefill_layer(pb: Problem, mode: int, Q, K, V, X=None, Wqi=None, Wki=None,
         if q_idx is None:
             q_idx = project(pb, X, Wqi)
         if k_idx is None:
-            k_idx = project(pb, X, Wki)
+            k_idx = project(pb, X, Wki, key=True)
         A, B = q_idx, k_idx
     else:
         A, B = Q, K

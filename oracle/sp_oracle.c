@@ -58,7 +58,16 @@ typedef struct orc_params {
   double idx_scale;          /* indexer scale (1/sqrt(d_idx))                           */
   int32_t local_window;      /* 0 = off                                                 */
   double local_bias;         /* added to the scaled logit when 0 <= t-s < local_window  */
+  int32_t flags;             /* ORC_F_* : the served scorer's ReLU / key LayerNorm / RoPE */
 } orc_params;
+
+/* The served scorer (Alg.2 steps 3-4): k_idx = LN(W_K x), RoPE on q and k_idx, ReLU on the scaled
+ * similarity.  Readings where the paper is silent (A26-A28): LayerNorm over the d_idx channels of one
+ * token, no affine, biased variance, eps = 1e-6; RoPE in the rotate-half pairing (i, i + d_idx/2) with
+ * theta_i = pos * 10000^(-2i/d_idx), pos = position LOCAL to the sequence; ReLU applied to the final logit
+ * (scaled similarity + the local term of A20).  The transforms run in fp64 on the fp64 projection sum and the
+ * result is rounded ONCE to bf16 (A14). */
+enum { ORC_F_RELU = 1, ORC_F_KEY_LN = 2, ORC_F_ROPE = 4 };
 
 enum { ORC_MODE_ORACLE = 0, ORC_MODE_INDEXER = 1 };
 
@@ -159,9 +168,34 @@ static inline double local_term(const orc_params *p, int32_t t, int32_t s) {    
 
 /* ---------- O3': indexer projection, PAPER.md:270, :297 ---------- */
 
-/* out[r,:] = bf16_rne( sum_j X[rows[r],j] * W[j,:] ), fp64 sum in index order j = 0..hidden-1. */
-void orc_project(const uint16_t *X, const uint16_t *W, int32_t hidden, int32_t d_idx,
+/* LayerNorm (key side only) then RoPE of one token's d channels, in place, fp64 (A27, A28). */
+void orc_transform(double *y, int32_t d, int32_t pos_local, int32_t flags, int32_t is_key) {
+  if (is_key && (flags & ORC_F_KEY_LN)) {
+    double mean = 0.0, var = 0.0;
+    for (int32_t c = 0; c < d; ++c) mean += y[c];
+    mean /= d;
+    for (int32_t c = 0; c < d; ++c) var += (y[c] - mean) * (y[c] - mean);
+    var /= d;
+    const double rstd = 1.0 / sqrt(var + 1e-6);
+    for (int32_t c = 0; c < d; ++c) y[c] = (y[c] - mean) * rstd;
+  }
+  if (flags & ORC_F_ROPE) {
+    const int32_t h = d / 2;
+    for (int32_t i = 0; i < h; ++i) {
+      const double theta = (double)pos_local * pow(10000.0, -2.0 * i / d);
+      const double c = cos(theta), sn = sin(theta);
+      const double a = y[i], b = y[i + h];
+      y[i] = a * c - b * sn;
+      y[i + h] = b * c + a * sn;
+    }
+  }
+}
+
+/* out[r,:] = bf16_rne( T( sum_j X[rows[r],j] * W[j,:] ) ), fp64 sum in index order j = 0..hidden-1; T = orc_transform
+ * with p->flags (identity when flags == 0). */
+void orc_project(const orc_params *p, const uint16_t *X, const uint16_t *W, int32_t is_key,
                  const int32_t *rows, int32_t nrows, uint16_t *out) {
+  const int32_t hidden = p->hidden, d_idx = p->d_idx;
 #pragma omp parallel
   {
     double *acc = (double *)malloc(sizeof(double) * (size_t)d_idx);
@@ -174,6 +208,11 @@ void orc_project(const uint16_t *X, const uint16_t *W, int32_t hidden, int32_t d
         const uint16_t *w = W + (size_t)j * d_idx;
         for (int32_t c = 0; c < d_idx; ++c) acc[c] += xv * bf16_to_f64(w[c]);
       }
+      if (p->flags & (ORC_F_KEY_LN | ORC_F_ROPE)) {
+        int32_t s0, n;
+        seq_of_pos(p, rows[r], &s0, &n);
+        orc_transform(acc, d_idx, rows[r] - s0, p->flags, is_key);
+      }
       for (int32_t c = 0; c < d_idx; ++c) out[(size_t)r * d_idx + c] = f64_to_bf16_rne(acc[c]);
     }
     free(acc);
@@ -183,7 +222,8 @@ void orc_project(const uint16_t *X, const uint16_t *W, int32_t hidden, int32_t d
 /* ---------- per-query score rows ---------- */
 
 /* O3' scoring: z[s] = idx_scale*<q_idx[t],k_idx[s]> (+local term) for local s = 0..tl
- * (without LN/RoPE/ReLU, as BASELINE.json configs 2-5 define the logits). q_idx,k_idx are packed [L,d_idx]. */
+ * (BASELINE.json configs 2-5 define the logits without LN/RoPE/ReLU: flags == 0; ORC_F_RELU clips at 0).
+ * q_idx,k_idx are packed [L,d_idx], already transformed by orc_project. */
 static void indexer_row(const orc_params *p, const uint16_t *q_idx, const uint16_t *k_idx,
                         int32_t s0, int32_t tl, double *z) {
   const uint16_t *q = q_idx + (size_t)(s0 + tl) * p->d_idx;
@@ -192,6 +232,7 @@ static void indexer_row(const orc_params *p, const uint16_t *q_idx, const uint16
     double acc = 0.0;
     for (int32_t c = 0; c < p->d_idx; ++c) acc += bf16_to_f64(q[c]) * bf16_to_f64(kk[c]);
     z[s] = p->idx_scale * acc + local_term(p, tl, s);
+    if ((p->flags & ORC_F_RELU) && z[s] < 0.0) z[s] = 0.0; /* PAPER.md:274; A26 */
   }
 }
 

@@ -115,7 +115,7 @@ def test_projection_matches_oracle(cfg):
     pbo = orc_problem(cfg)
     pbg = B.Problem.from_config(cfg)
     want_q = orc.project(pbo, inp["X"], inp["Wqi"])
-    want_k = orc.project(pbo, inp["X"], inp["Wki"])
+    want_k = orc.project(pbo, inp["X"], inp["Wki"], key=True)
     q = torch.empty(cfg.L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
     k = torch.empty_like(q)
     rows = pbg.num_rows
@@ -141,7 +141,7 @@ def test_indexer_scores_match_oracle(cfg, b):
     pbo = orc_problem(cfg, b_sel=b)
     pbg = B.Problem.from_config(cfg, b_sel=b)
     q_idx = orc.project(pbo, inp["X"], inp["Wqi"])
-    k_idx = orc.project(pbo, inp["X"], inp["Wki"])
+    k_idx = orc.project(pbo, inp["X"], inp["Wki"], key=True)
     rows = pbg.num_rows
     R, nv = orc.support_scores(pbo, orc.MODE_INDEXER, q_idx, k_idx, np.arange(rows))
     sc = torch.full((rows, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
@@ -304,7 +304,7 @@ def run_layer_and_compare(cfg, rows, n_queries, mode=None, seed=0, inputs=None):
         qi[need_q] = orc.project(pbo, inp["X"], inp["Wqi"], rows=need_q)
         ki = np.zeros((cfg.L, cfg.d_idx), np.uint16)
         need_k = np.arange(0, int(need_q.max()) + 1)
-        ki[need_k] = orc.project(pbo, inp["X"], inp["Wki"], rows=need_k)
+        ki[need_k] = orc.project(pbo, inp["X"], inp["Wki"], rows=need_k, key=True)
         kw["q_idx"], kw["k_idx"] = qi, ki
     res = orc.prefill_layer(pbo, omode, inp["Q"], inp["K"], inp["V"], rows=rows, pos=pos, **kw)
 

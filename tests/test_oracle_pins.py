@@ -400,3 +400,88 @@ def test_empty_effective_support_gives_zero_output():
     sup = np.full((1, 1), 9, np.int32)
     o, lse = orc.sparse_attn(pb, Q, K, V, [3], sup, want_lse=True)
     assert np.all(o == 0) and np.all(np.isneginf(lse))
+
+
+# ------------------------------------------------------------------ served scorer: key LayerNorm, RoPE, ReLU
+# (readings A26-A28 of DESIGN.md).  Pins on the fp64 core orc_transform and on the chain.
+
+def test_served_scorer_layernorm_closed_form():
+    rng = np.random.Generator(np.random.Philox(77))
+    y = rng.standard_normal(64) * 3.0 + 1.5
+    z = orc.transform(y, pos_local=5, flags=orc.F_KEY_LN, key=True)
+    assert abs(z.mean()) < 1e-12
+    assert abs(z.var() - y.var() / (y.var() + 1e-6)) < 1e-12          # biased variance, eps = 1e-6, no affine
+    assert np.allclose(z, (y - y.mean()) / np.sqrt(y.var() + 1e-6), rtol=0, atol=1e-12)
+    # the query side is never normalised; a constant key row maps to 0
+    assert np.array_equal(orc.transform(y, 5, orc.F_KEY_LN, key=False), y)
+    assert np.allclose(orc.transform(np.full(16, 2.5), 3, orc.F_KEY_LN, key=True), 0.0, atol=1e-9)
+
+
+def test_served_scorer_rope_closed_forms():
+    rng = np.random.Generator(np.random.Philox(78))
+    d = 32
+    q, k = rng.standard_normal(d), rng.standard_normal(d)
+    # position 0 is the identity; every position preserves the norm of each (i, i + d/2) pair
+    assert np.array_equal(orc.transform(q, 0, orc.F_ROPE, key=False), q)
+    for pos in (1, 17, 4096, 131071):
+        r = orc.transform(q, pos, orc.F_ROPE, key=False)
+        assert np.allclose(r[:d // 2] ** 2 + r[d // 2:] ** 2, q[:d // 2] ** 2 + q[d // 2:] ** 2, rtol=1e-12)
+    # d = 2: theta_0 = pos, (1, 0) -> (cos pos, sin pos)
+    for pos in (1, 2, 100):
+        assert np.allclose(orc.transform(np.array([1.0, 0.0]), pos, orc.F_ROPE, key=True), [math.cos(pos), math.sin(pos)],
+                           atol=1e-12)
+    # frequencies: pair i turns by pos * 10000^(-2i/d)
+    e = np.zeros(d); e[3] = 1.0
+    r = orc.transform(e, 7, orc.F_ROPE, key=False)
+    th = 7 * 10000.0 ** (-2 * 3 / d)
+    assert np.allclose([r[3], r[3 + d // 2]], [math.cos(th), math.sin(th)], atol=1e-12)
+    # relative-position property: <R_t q, R_s k> depends on t - s only
+    a = orc.transform(q, 900, orc.F_ROPE, False) @ orc.transform(k, 650, orc.F_ROPE, True)
+    b = orc.transform(q, 300, orc.F_ROPE, False) @ orc.transform(k, 50, orc.F_ROPE, True)
+    assert abs(a - b) < 1e-9
+    # LayerNorm is applied BEFORE the rotation on the key side
+    both = orc.transform(k, 11, orc.F_KEY_LN | orc.F_ROPE, key=True)
+    assert np.allclose(both, orc.transform(orc.transform(k, 11, orc.F_KEY_LN, True), 11, orc.F_ROPE, True), atol=1e-12)
+
+
+def test_served_scorer_projection_uses_local_positions_and_rounds_once():
+    rng = np.random.Generator(np.random.Philox(79))
+    L, hid, di = 24, 32, 16
+    X = orc.f64_to_bf16(rng.standard_normal((L, hid)))
+    W = orc.f64_to_bf16(rng.standard_normal((hid, di)) / math.sqrt(hid))
+    cu = (0, 10, 24)
+    pb = orc.Problem(L=L, Hq=2, Hkv=1, d=8, k=4, hidden=hid, d_idx=di, cu_seqlens=cu,
+                     flags=orc.F_KEY_LN | orc.F_ROPE)
+    got = orc.project(pb, X, W, key=True)
+    y = orc.bf16_to_f64(X) @ orc.bf16_to_f64(W)                        # exact products, fp64 sum
+    for t in range(L):
+        local = t - (0 if t < 10 else 10)
+        want = orc.f64_to_bf16(orc.transform(y[t], local, pb.flags, key=True))
+        assert np.array_equal(got[t], want), t
+    # flags == 0 is the plain projection
+    pb0 = orc.Problem(L=L, Hq=2, Hkv=1, d=8, k=4, hidden=hid, d_idx=di)
+    assert np.array_equal(orc.project(pb0, X, W, key=True), orc.f64_to_bf16(y))
+
+
+def test_served_scorer_relu_and_zero_ties():
+    rng = np.random.Generator(np.random.Philox(80))
+    L, di, k = 40, 8, 6
+    q = orc.f64_to_bf16(rng.standard_normal((L, di)))
+    kk = orc.f64_to_bf16(rng.standard_normal((L, di)))
+    pb0 = orc.Problem(L=L, Hq=2, Hkv=1, d=8, k=k, hidden=16, d_idx=di, local_window=3, local_bias=-0.25)
+    pb1 = orc.Problem(L=L, Hq=2, Hkv=1, d=8, k=k, hidden=16, d_idx=di, local_window=3, local_bias=-0.25,
+                      flags=orc.F_RELU)
+    pos = np.arange(L)
+    z0 = orc.query_scores(pb0, orc.MODE_INDEXER, q, kk, pos)
+    z1 = orc.query_scores(pb1, orc.MODE_INDEXER, q, kk, pos)
+    fin = np.isfinite(z0)
+    assert np.array_equal(np.isfinite(z1), fin)
+    assert np.array_equal(z1[fin], np.maximum(z0[fin], 0.0))          # ReLU on the final logit (A26)
+    # a query whose logits are all negative: every score is 0, ties -> the lowest indices fill the budget (A11)
+    qn = q.copy(); kn = kk.copy()
+    qn[:] = orc.f64_to_bf16(np.ones((L, di))); kn[:] = orc.f64_to_bf16(-np.ones((L, di)))
+    pb2 = orc.Problem(L=L, Hq=2, Hkv=1, d=8, k=k, hidden=16, d_idx=di, flags=orc.F_RELU)
+    R, nv = orc.support_scores(pb2, orc.MODE_INDEXER, qn, kn, np.arange(L))
+    idx, cnt = orc.topk(R, nv, k)
+    for t in range(k, L):
+        assert np.array_equal(idx[t], np.arange(k)), t

@@ -41,7 +41,7 @@ extern "C" {
 typedef enum sp_status {
   SP_OK = 0,
   SP_ERR_INVALID_ARG = -1, /* null / misaligned pointer, nonpositive size, Hq % Hkv, bad cu_seqlens, bad panel */
-  SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}, Hq/Hkv not in {1,2,4,8}, flags != 0 ...) */
+  SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}, Hq/Hkv not in {1,2,4,8}, unknown flag bits ...) */
   SP_ERR_WORKSPACE = -3,   /* workspace too small (see sp_workspace_bytes)                                      */
   SP_ERR_CUDA = -4         /* a CUDA launch / API error; text via sp_strerror                                   */
 } sp_status;
@@ -76,8 +76,18 @@ typedef struct sp_params {
   float idx_scale;                /* indexer scale;   0 -> 1/sqrt(d_idx) */
   int32_t local_window;           /* 0 = off                                                              */
   float local_bias;               /* added to the scaled logit when 0 <= t-s < local_window               */
-  uint32_t flags;                 /* reserved (ReLU / key LayerNorm / RoPE of PAPER.md:270-274): must be 0 */
+  uint32_t flags;                 /* SP_F_* below; 0 = the plain scorer BASELINE.json configs 2-5 define       */
 } sp_params;
+
+/* The served scorer of PAPER.md:268-274 / Alg.2 steps 3-4 (indexer mode only; needs the tcgen05 paths, i.e.
+ * b_sel in {1,32,64,128}, else SP_ERR_UNSUPPORTED).  Readings where the paper is silent: DESIGN.md A26-A28.
+ *   SP_F_KEY_LN : k_idx = LayerNorm(X Wki) over the d_idx channels of a token (no affine, biased variance, eps 1e-6)
+ *   SP_F_ROPE   : rotary embedding of q_idx and (after the LayerNorm) k_idx, rotate-half pairing (i, i + d_idx/2),
+ *                 theta_i = pos * 10000^(-2i/d_idx), pos local to the sequence
+ *   SP_F_RELU   : z = max(idx_scale <q_idx, k_idx> + local term, 0)
+ * KEY_LN and ROPE act in the projection (q_idx / k_idx come out transformed, rounded once to bf16; with
+ * preprojected = 1 the caller's tensors are taken as already transformed); RELU acts in the score epilogue. */
+enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u };
 
 /* Number of support rows of the whole pack (host arithmetic only). Returns < 0 on invalid params. */
 int64_t sp_num_rows(const sp_params *p);

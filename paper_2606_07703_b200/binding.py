@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libsp.so")
 
 SP_OK, SP_ERR_INVALID_ARG, SP_ERR_UNSUPPORTED, SP_ERR_WORKSPACE, SP_ERR_CUDA = 0, -1, -2, -3, -4
 SP_MODE_ORACLE, SP_MODE_INDEXER = 0, 1
+SP_F_RELU, SP_F_KEY_LN, SP_F_ROPE = 1, 2, 4   # sp_params.flags: the served scorer of PAPER.md:270-274
 (SP_STAGE_INDEXER_SCORES, SP_STAGE_ORACLE_MASS, SP_STAGE_TOPK, SP_STAGE_SPARSE_ATTN, SP_STAGE_DENSE_ATTN,
  SP_STAGE_LAYER_ORACLE, SP_STAGE_LAYER_INDEXER) = range(7)
 
@@ -125,7 +126,7 @@ class Problem:
     def from_config(cls, cfg, device="cuda", **over):
         kw = dict(L=cfg.L, Hq=cfg.Hq, Hkv=cfg.Hkv, d=cfg.d, k=cfg.k, b_sel=cfg.b_sel, hidden=cfg.hidden,
                   d_idx=cfg.d_idx, local_window=cfg.local_window, local_bias=cfg.local_bias,
-                  cu_seqlens=cfg.cu_seqlens, device=device)
+                  cu_seqlens=cfg.cu_seqlens, flags=getattr(cfg, "flags", 0), device=device)
         kw.update(over)
         return cls(**kw)
 

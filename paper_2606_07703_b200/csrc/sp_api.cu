@@ -90,7 +90,8 @@ int validate_common(const sp_params* p, bool need_attn, bool need_indexer) {
   } else if (p->batch != 1) {
     return SP_ERR_INVALID_ARG;
   }
-  if (p->flags != 0) return SP_ERR_UNSUPPORTED;
+  if (p->flags & ~(uint32_t)(SP_F_RELU | SP_F_KEY_LN | SP_F_ROPE)) return SP_ERR_UNSUPPORTED;
+  if (p->flags != 0 && (!sp_tc_scores_supported(p->b_sel) || debug_simt())) return SP_ERR_UNSUPPORTED;
   if (p->local_window < 0) return SP_ERR_INVALID_ARG;
   if (need_attn) {
     if (p->Hq < 1 || p->Hkv < 1 || p->d < 1 || p->Hq % p->Hkv != 0) return SP_ERR_INVALID_ARG;
@@ -124,7 +125,8 @@ int validate_panel(const sp_params* p, int32_t row_begin, int32_t row_count, int
 // ---- stage dispatch: tcgen05 kernels where the shape is in their built set, CUDA-core kernels otherwise ----
 cudaError_t run_project(const sp_params* p, const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx,
                         void* ws, cudaStream_t st) {
-  if (!(debug_simt() & 1)) return sp_launch_project_tc(X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, st);
+  if (!(debug_simt() & 1))
+    return sp_launch_project_tc(dev_geom(p), p->flags, X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, st);
   return sp_launch_project(X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, ws, st);
 }
 
@@ -133,8 +135,8 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
   const SpGeom g = dev_geom(p);
   if (sp_tc_scores_supported(p->b_sel) && !(debug_simt() & 2))
     return sp_launch_indexer_scores_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, q_idx, k_idx, p->d_idx,
-                                       index_scale(p), p->local_window, p->local_bias, row_begin, row_count, max_nv,
-                                       scores, ld, st);
+                                       index_scale(p), p->local_window, p->local_bias, (p->flags & SP_F_RELU) ? 1 : 0,
+                                       row_begin, row_count, max_nv, scores, ld, st);
   return sp_launch_indexer_scores(g, q_idx, k_idx, p->d_idx, index_scale(p), p->local_window, p->local_bias, row_begin,
                                   row_count, max_nv, scores, ld, st);
 }
@@ -233,7 +235,7 @@ const char* sp_strerror(int code) {
   switch (code) {
     case SP_OK: return "SP_OK";
     case SP_ERR_INVALID_ARG: return "SP_ERR_INVALID_ARG: null/misaligned pointer, bad size, bad cu_seqlens or bad panel";
-    case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED: shape outside the built set (d in {64,128}, Hq/Hkv in {1,2,4,8}, d_idx in {64,128}, hidden % 64 == 0, flags == 0)";
+    case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED: shape outside the built set (d in {64,128}, Hq/Hkv in {1,2,4,8}, d_idx in {64,128}, hidden % 64 == 0, known flags; flags need b_sel in {1,32,64,128})";
     case SP_ERR_WORKSPACE: return "SP_ERR_WORKSPACE: workspace too small, see sp_workspace_bytes";
     case SP_ERR_CUDA: return g_err_text;
   }

@@ -107,12 +107,13 @@ cudaError_t sp_launch_attn(const SpGeom& g, const void* Q, const void* K, const 
                            int q_count, void* O, float* lse, cudaStream_t st);
 
 // tcgen05 paths (sp_tc_gemm.cu, sp_tc_attn.cu)
-cudaError_t sp_launch_project_tc(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
-                                 int hidden, int d_idx, cudaStream_t st);
+cudaError_t sp_launch_project_tc(const SpGeom& g, uint32_t flags, const void* X, const void* Wq, const void* Wk,
+                                 void* q_idx, void* k_idx, int L, int hidden, int d_idx, cudaStream_t st);
 bool sp_tc_scores_supported(int b_sel);
 cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host, const void* q_idx, const void* k_idx,
-                                        int d_idx, float idx_scale, int local_window, float local_bias, int row_begin,
-                                        int row_count, int max_n_valid, float* scores, int64_t ld, cudaStream_t st);
+                                        int d_idx, float idx_scale, int local_window, float local_bias, int relu,
+                                        int row_begin, int row_count, int max_n_valid, float* scores, int64_t ld,
+                                        cudaStream_t st);
 
 bool sp_tc_mass_supported(int b_sel, int d);
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,

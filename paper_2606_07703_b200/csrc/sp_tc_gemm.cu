@@ -55,7 +55,7 @@ template <int DI>
 __global__ void __launch_bounds__(128, 1)
 sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmWq,
                      const __grid_constant__ CUtensorMap tmWk, __nv_bfloat16* __restrict__ q_idx,
-                     __nv_bfloat16* __restrict__ k_idx, int L, int hidden) {
+                     __nv_bfloat16* __restrict__ k_idx, int L, int hidden, SpGeom g, uint32_t flags) {
   constexpr int N = 2 * DI;
   constexpr int NG = N / 64;                  // 64-column groups of B
   constexpr uint32_t A_BYTES = 128 * 128;     // 128 rows x 64 k
@@ -125,21 +125,109 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
   // epilogue: thread = output row
   const int m = m0 + warp * 32 + lane;
   const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  if ((flags & (SP_F_KEY_LN | SP_F_ROPE)) == 0) {
 #pragma unroll
-  for (int c0 = 0; c0 < N; c0 += 32) {
-    uint32_t v[32];
-    tmem_ld_x32(trow + c0, v);
-    tmem_ld_wait();
-    if (m < L) {
-      __nv_bfloat16* dst = (c0 < DI ? q_idx + (size_t)m * DI + c0 : k_idx + (size_t)m * DI + (c0 - DI));
+    for (int c0 = 0; c0 < N; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld_x32(trow + c0, v);
+      tmem_ld_wait();
+      if (m < L) {
+        __nv_bfloat16* dst = (c0 < DI ? q_idx + (size_t)m * DI + c0 : k_idx + (size_t)m * DI + (c0 - DI));
 #pragma unroll
-      for (int j = 0; j < 32; j += 8) {
-        uint4 o;
-        o.x = sp_pack_bf16(__uint_as_float(v[j]), __uint_as_float(v[j + 1]));
-        o.y = sp_pack_bf16(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
-        o.z = sp_pack_bf16(__uint_as_float(v[j + 4]), __uint_as_float(v[j + 5]));
-        o.w = sp_pack_bf16(__uint_as_float(v[j + 6]), __uint_as_float(v[j + 7]));
-        *reinterpret_cast<uint4*>(dst + j) = o;
+        for (int j = 0; j < 32; j += 8) {
+          uint4 o;
+          o.x = sp_pack_bf16(__uint_as_float(v[j]), __uint_as_float(v[j + 1]));
+          o.y = sp_pack_bf16(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+          o.z = sp_pack_bf16(__uint_as_float(v[j + 4]), __uint_as_float(v[j + 5]));
+          o.w = sp_pack_bf16(__uint_as_float(v[j + 6]), __uint_as_float(v[j + 7]));
+          *reinterpret_cast<uint4*>(dst + j) = o;
+        }
+      }
+    }
+  } else {
+    // The served scorer (readings A27/A28): LayerNorm of the KEY row over its DI channels (no
+    // affine, biased variance, eps 1e-6), then RoPE of both rows in the rotate-half pairing (i, i + DI/2) at the
+    // token's LOCAL position; everything in fp32 on the fp32 accumulator, ONE rounding to bf16.
+    const int mm = min(m, L - 1);
+    const int pos = mm - sp_pos_info(g, mm).seq_start;
+    float mean = 0.f, rstd = 1.f;
+    if (flags & SP_F_KEY_LN) {
+      float sum = 0.f;
+#pragma unroll
+      for (int c0 = 0; c0 < DI; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld_x32(trow + DI + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 32; ++j) sum += __uint_as_float(v[j]);
+      }
+      mean = sum * (1.f / DI);
+      float ss = 0.f;
+#pragma unroll
+      for (int c0 = 0; c0 < DI; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld_x32(trow + DI + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const float dlt = __uint_as_float(v[j]) - mean;
+          ss = fmaf(dlt, dlt, ss);
+        }
+      }
+      rstd = rsqrtf(ss * (1.f / DI) + 1e-6f);
+    }
+    constexpr int H = DI / 2;
+#pragma unroll
+    for (int c0 = 0; c0 < H; c0 += 32) {
+      float cs[32], sn[32];
+      if (flags & SP_F_ROPE) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          // theta = pos * 10000^(-2i/DI), reduced to [-pi, pi] in double before the fp32 sin / cos
+          const double inv_freq = exp2(-(double)(2 * (c0 + j)) / DI * 13.287712379549449);  // log2(10000)
+          const double th = (double)pos * inv_freq;
+          const float r = (float)(th - 6.283185307179586 * rint(th * 0.15915494309189535));
+          cs[j] = cosf(r);
+          sn[j] = sinf(r);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          cs[j] = 1.f;
+          sn[j] = 0.f;
+        }
+      }
+#pragma unroll
+      for (int side = 0; side < 2; ++side) {
+        uint32_t a[32], b2[32];
+        tmem_ld_x32(trow + side * DI + c0, a);
+        tmem_ld_x32(trow + side * DI + H + c0, b2);
+        tmem_ld_wait();
+        const float mu = side ? mean : 0.f, rs = side ? rstd : 1.f;
+        float lo[32], hi[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const float x = (__uint_as_float(a[j]) - mu) * rs, y = (__uint_as_float(b2[j]) - mu) * rs;
+          lo[j] = x * cs[j] - y * sn[j];
+          hi[j] = y * cs[j] + x * sn[j];
+        }
+        if (m < L) {
+          __nv_bfloat16* dst = (side ? k_idx : q_idx) + (size_t)m * DI;
+#pragma unroll
+          for (int j = 0; j < 32; j += 8) {
+            uint4 o;
+            o.x = sp_pack_bf16(lo[j], lo[j + 1]);
+            o.y = sp_pack_bf16(lo[j + 2], lo[j + 3]);
+            o.z = sp_pack_bf16(lo[j + 4], lo[j + 5]);
+            o.w = sp_pack_bf16(lo[j + 6], lo[j + 7]);
+            *reinterpret_cast<uint4*>(dst + c0 + j) = o;
+            o.x = sp_pack_bf16(hi[j], hi[j + 1]);
+            o.y = sp_pack_bf16(hi[j + 2], hi[j + 3]);
+            o.z = sp_pack_bf16(hi[j + 4], hi[j + 5]);
+            o.w = sp_pack_bf16(hi[j + 6], hi[j + 7]);
+            *reinterpret_cast<uint4*>(dst + H + c0 + j) = o;
+          }
+        }
       }
     }
   }
@@ -154,8 +242,8 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
 // launchers
 // ---------------------------------------------------------------------------------------------------
 template <int DI>
-static cudaError_t launch_project_tc(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
-                                     int hidden, cudaStream_t st) {
+static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void* X, const void* Wq, const void* Wk,
+                                     void* q_idx, void* k_idx, int L, int hidden, cudaStream_t st) {
   CUtensorMap tmX, tmWq, tmWk;
   cudaError_t e;
   if ((e = sp_make_tmap_bf16(&tmX, X, L, hidden, hidden, 128)) != cudaSuccess) return e;
@@ -169,13 +257,13 @@ static cudaError_t launch_project_tc(const void* X, const void* Wq, const void* 
     attr_done = true;
   }
   sp_tc_project_kernel<DI><<<(L + 127) / 128, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
-                                                               (__nv_bfloat16*)k_idx, L, hidden);
+                                                               (__nv_bfloat16*)k_idx, L, hidden, g, flags);
   sp_count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t sp_launch_project_tc(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
-                                 int hidden, int d_idx, cudaStream_t st) {
-  return d_idx == 128 ? launch_project_tc<128>(X, Wq, Wk, q_idx, k_idx, L, hidden, st)
-                      : launch_project_tc<64>(X, Wq, Wk, q_idx, k_idx, L, hidden, st);
+cudaError_t sp_launch_project_tc(const SpGeom& g, uint32_t flags, const void* X, const void* Wq, const void* Wk,
+                                 void* q_idx, void* k_idx, int L, int hidden, int d_idx, cudaStream_t st) {
+  return d_idx == 128 ? launch_project_tc<128>(g, flags, X, Wq, Wk, q_idx, k_idx, L, hidden, st)
+                      : launch_project_tc<64>(g, flags, X, Wq, Wk, q_idx, k_idx, L, hidden, st);
 }

@@ -162,7 +162,7 @@ __device__ __forceinline__ float sc_max32(const uint32_t* v) {
 // Epilogue of one (key tile, part): thread = key (TMEM lane), columns = the part's 128 queries.
 // b == 1 writes every causal (t, s); b > 1 (a power of two, 2^lb) keeps the max of each selection block.
 __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane, int s0, int hq0, int hrow0, int q_last,
-                                            int b, int lb, float idx_scale, int local_window, float local_bias,
+                                            int b, int lb, float idx_scale, int local_window, float local_bias, bool relu,
                                             int row_begin, int row_count, float* __restrict__ scores, int64_t ld) {
   const int s = s0 + warp_q * 32 + lane;  // this thread's local key
   const int s_lo = s0 + warp_q * 32;      // warp-uniform: smallest / largest key of the warp
@@ -183,6 +183,7 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
         if (t <= q_last && s <= t && row >= row_begin && row < row_begin + row_count) {
           float z = __uint_as_float(v[j]) * idx_scale;
           if (local_window > 0 && t - s < local_window) z += local_bias;
+          if (relu) z = fmaxf(z, 0.f);  // PAPER.md:274 (A26): ReLU on the final logit
           scores[(size_t)(row - row_begin) * ld + s] = z;
         }
       }
@@ -214,7 +215,7 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
     for (int blk = 0; blk < 4; ++blk) {
       const int row = hrow0 + blk;
       if (blk < nblk && row >= row_begin && row < row_begin + row_count)
-        scores[(size_t)(row - row_begin) * ld + s] = cm[blk] * idx_scale;
+        scores[(size_t)(row - row_begin) * ld + s] = relu ? fmaxf(cm[blk] * idx_scale, 0.f) : cm[blk] * idx_scale;
     }
     return;
   }
@@ -262,6 +263,7 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
       }
     }
     const int row = hrow0 + blk;
+    if (relu) best = fmaxf(best, 0.f);  // max and ReLU commute; a block row always has a valid (t >= s) pair here
     if (row >= row_begin && row < row_begin + row_count && s <= blk_last)
       scores[(size_t)(row - row_begin) * ld + s] = best;
   }
@@ -270,8 +272,8 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
 template <int DI>
 __global__ void __launch_bounds__(SC_THREADS, 1)
 sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK, SpGeom g,
-                   float idx_scale, int local_window, float local_bias, int row_begin, int row_count, int st_begin,
-                   int st_count, int n_stages, float* __restrict__ scores, int64_t ld) {
+                   float idx_scale, int local_window, float local_bias, int relu, int row_begin, int row_count,
+                   int st_begin, int st_count, int n_stages, float* __restrict__ scores, int64_t ld) {
   constexpr int KB = DI / 64;
   constexpr uint32_t A_BYTES = SC_KT * 128;  // per 64-wide K block: 128 keys
   constexpr uint32_t B_BYTES = SC_NQ * 128;  // per 64-wide K block: the 128 queries of one part
@@ -413,7 +415,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         mbar_wait(&bar.accfull[p], use & 1);
         tc_fence_after_sync();
         sc_epilogue(trow, wq, lane, kt * SC_KT, pq0, prow0, q_last, b, lb, idx_scale, local_window, local_bias,
-                    row_begin, row_count, scores, ld);
+                    relu != 0, row_begin, row_count, scores, ld);
         tc_fence_before_sync();
         mbar_arrive(&bar.accempty[p]);
         ++use;
@@ -444,7 +446,7 @@ static int sc_sm_count() {
 
 template <int DI>
 static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const void* k_idx, float idx_scale, int lw,
-                                    float lb, int row_begin, int row_count, int st_begin, int st_count, long long units,
+                                    float lb, int relu, int row_begin, int row_count, int st_begin, int st_count, long long units,
                                     float* scores, int64_t ld, cudaStream_t st) {
   CUtensorMap tmQ, tmK;
   cudaError_t e;
@@ -460,7 +462,7 @@ static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const vo
   }
   long long grid = units < sc_sm_count() ? units : sc_sm_count();
   if (grid < 1) grid = 1;
-  sp_tc_score_kernel<DI><<<(unsigned)grid, SC_THREADS, smem, st>>>(tmQ, tmK, g, idx_scale, lw, lb, row_begin, row_count,
+  sp_tc_score_kernel<DI><<<(unsigned)grid, SC_THREADS, smem, st>>>(tmQ, tmK, g, idx_scale, lw, lb, relu, row_begin, row_count,
                                                                   st_begin, st_count, stages, scores, ld);
   sp_count_launch();
   return cudaGetLastError();
@@ -468,8 +470,9 @@ static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const vo
 
 // cu_host: HOST copy of cu_seqlens (nullptr = one sequence).
 cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host, const void* q_idx, const void* k_idx,
-                                        int d_idx, float idx_scale, int local_window, float local_bias, int row_begin,
-                                        int row_count, int max_n_valid, float* scores, int64_t ld, cudaStream_t st) {
+                                        int d_idx, float idx_scale, int local_window, float local_bias, int relu,
+                                        int row_begin, int row_count, int max_n_valid, float* scores, int64_t ld,
+                                        cudaStream_t st) {
   (void)max_n_valid;
   if (row_count <= 0) return cudaSuccess;
   // query super tiles (512 local positions of one sequence) that intersect the row panel, and their step count
@@ -509,8 +512,8 @@ cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host,
     }
   }
   const int cnt = (int)(qhi - qlo + 1);
-  return d_idx == 128 ? launch_scores_tc<128>(g, q_idx, k_idx, idx_scale, local_window, local_bias, row_begin, row_count,
+  return d_idx == 128 ? launch_scores_tc<128>(g, q_idx, k_idx, idx_scale, local_window, local_bias, relu, row_begin, row_count,
                                               (int)qlo, cnt, units, scores, ld, st)
-                      : launch_scores_tc<64>(g, q_idx, k_idx, idx_scale, local_window, local_bias, row_begin, row_count,
+                      : launch_scores_tc<64>(g, q_idx, k_idx, idx_scale, local_window, local_bias, relu, row_begin, row_count,
                                              (int)qlo, cnt, units, scores, ld, st);
 }

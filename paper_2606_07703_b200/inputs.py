@@ -42,6 +42,7 @@ class Config:
     local_bias: float = 0.0
     cu_seqlens: Optional[Tuple[int, ...]] = None
     seed_extra: int = 0
+    flags: int = 0            # served-scorer switches: 1 ReLU, 2 key LayerNorm, 4 RoPE
 
     @property
     def scale(self) -> float:

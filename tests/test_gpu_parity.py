@@ -34,7 +34,7 @@ def cached_inputs(cfg, with_indexer):
 def orc_problem(cfg, **over):
     kw = dict(L=cfg.L, Hq=cfg.Hq, Hkv=cfg.Hkv, d=cfg.d, k=cfg.k, b_sel=cfg.b_sel, hidden=cfg.hidden,
               d_idx=cfg.d_idx, local_window=cfg.local_window, local_bias=cfg.local_bias,
-              cu_seqlens=cfg.cu_seqlens)
+              cu_seqlens=cfg.cu_seqlens, flags=getattr(cfg, "flags", 0))
     kw.update(over)
     return orc.Problem(**kw)
 
@@ -158,6 +158,71 @@ def test_indexer_scores_match_oracle(cfg, b):
     for i in range(rc):
         n = int(nv[r0 + i])
         assert np.array_equal(got2[i, :n], got[r0 + i, :n])
+
+
+# ------------------------------------------------------------------ served scorer: f1
+
+SERVED = B.SP_F_RELU | B.SP_F_KEY_LN | B.SP_F_ROPE
+SMALL_SERVED = gen.shrink(gen.C2, 1500, flags=SERVED)                                    # d_idx 64
+SMALL_SERVED128 = gen.shrink(gen.C3, 1100, hidden=512, flags=SERVED)                     # d_idx 128, local window
+SMALL_SERVED_VARLEN = gen.shrink(gen.C5_VARLEN, 1000, cu_seqlens=(0, 300, 301, 690, 1000), hidden=256, k=100,
+                                 b_sel=32, flags=SERVED)
+
+
+@pytest.mark.parametrize("cfg", [SMALL_SERVED, SMALL_SERVED128, SMALL_SERVED_VARLEN], ids=lambda c: c.name)
+def test_served_projection_matches_oracle(cfg):
+    """key LayerNorm + RoPE fused into the projection epilogue: bf16 outputs vs the oracle's single rounding."""
+    inp = gen.make_inputs(cfg)
+    pbo = orc_problem(cfg)
+    pbg = B.Problem.from_config(cfg)
+    want_q = orc.project(pbo, inp["X"], inp["Wqi"])
+    want_k = orc.project(pbo, inp["X"], inp["Wki"], key=True)
+    q = torch.empty(cfg.L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
+    k = torch.empty_like(q)
+    rows = pbg.num_rows
+    sc = torch.empty(rows, pbg.max_seqlen, dtype=torch.float32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
+    B.sp_indexer_scores(pbg, dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"]), q, k, False, 0, rows, sc, ws)
+    torch.cuda.synchronize()
+    for got, want in ((bf16_bits(q), want_q), (bf16_bits(k), want_k)):
+        diff = got != want
+        # fp32 (tensor-core sum, LayerNorm, sin/cos.approx after a double-precision range reduction) vs fp64: a value
+        # close to a bf16 rounding boundary may land on the other side -- rare, and never by more than one ulp
+        assert diff.mean() < 1e-2, diff.mean()
+        a = orc.bf16_to_f64(got[diff])
+        b = orc.bf16_to_f64(want[diff])
+        assert np.all(np.abs(a - b) <= np.abs(b) * 2.0 ** -7 + 2e-5)
+    # the key rows are normalised: zero mean, unit variance over d_idx (up to bf16 rounding), rotation keeps that norm
+    kf = to_f64(k)
+    assert np.allclose((kf ** 2).sum(1), cfg.d_idx, rtol=2e-2)
+
+
+@pytest.mark.parametrize("cfg,b", [(SMALL_SERVED, 64), (SMALL_SERVED128, 128), (SMALL_SERVED128, 1)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_served_scores_relu_match_oracle(cfg, b):
+    inp = gen.make_inputs(cfg)
+    pbo = orc_problem(cfg, b_sel=b)
+    pbg = B.Problem.from_config(cfg, b_sel=b)
+    q_idx = orc.project(pbo, inp["X"], inp["Wqi"])
+    k_idx = orc.project(pbo, inp["X"], inp["Wki"], key=True)
+    rows = pbg.num_rows
+    R, nv = orc.support_scores(pbo, orc.MODE_INDEXER, q_idx, k_idx, np.arange(rows))
+    sc = torch.full((rows, cfg.L), float("nan"), dtype=torch.float32, device=DEV)
+    B.sp_indexer_scores(pbg, None, None, None, dev(q_idx), dev(k_idx), True, 0, rows, sc)
+    got = to_f64(sc)
+    zeros = 0
+    for r in range(rows):
+        n = int(nv[r])
+        assert np.all(got[r, :n] >= 0.0)
+        assert np.all(np.abs(got[r, :n] - R[r, :n]) <= 1e-5 * np.maximum(1.0, np.abs(R[r, :n]))), r
+        zeros += int((R[r, :n] == 0.0).sum())
+    assert zeros > 0 or b > 1        # per-query rows of a random scorer do hit the clipped branch
+
+
+def test_served_scorer_layer_chained():
+    """The whole layer with the served scorer on a small varlen pack: supports and outputs vs the oracle."""
+    st = run_layer_and_compare(SMALL_SERVED_VARLEN, rows=None, n_queries=None)
+    assert st["strict"] + st["fuzzy"] == SMALL_SERVED_VARLEN.num_rows
 
 
 # ------------------------------------------------------------------ a4 attention mass: stage-isolated

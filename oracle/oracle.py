@@ -291,3 +291,32 @@ def prefill_layer(pb: Problem, mode: int, Q, K, V, X=None, Wqi=None, Wki=None,
     sup = np.stack([idx[row_index[row_of_pos(pb, int(t))]] for t in pos]) if len(pos) else np.empty((0, pb.k), np.int32)
     out = sparse_attn(pb, Q, K, V, pos, sup)
     return LayerResult(rows, R, nv, idx, cnt, pos, out, q_idx, k_idx)
+
+
+# ---------------------------------------------------------------- support-level diagnostics
+
+def support_overlap(idx_a, idx_b) -> np.ndarray:
+    """|S_a(r) & S_b(r)| per support row: how much of one support (e.g. the oracle's) the other
+    (e.g. the indexer's, :300) recovers -- the "support-level diagnostic" of :478.  Entries < 0 are padding."""
+    idx_a, idx_b = np.asarray(idx_a), np.asarray(idx_b)
+    out = np.zeros(idx_a.shape[0], dtype=np.int32)
+    for r in range(idx_a.shape[0]):
+        a = idx_a[r][idx_a[r] >= 0]
+        b = idx_b[r][idx_b[r] >= 0]
+        out[r] = len(set(a.tolist()) & set(b.tolist()))
+    return out
+
+
+def row_kl(P, z, n_valid) -> np.ndarray:
+    """KL(P_t || softmax(z_t)) over the valid causal keys s < n_valid[t] of each per-query row:
+    sum_s P[s] (log P[s] - log softmax(z)[s]), terms with P[s] = 0 contribute 0.  fp64, log-sum-exp form."""
+    P, z = np.asarray(P, dtype=np.float64), np.asarray(z, dtype=np.float64)
+    out = np.zeros(P.shape[0])
+    for r in range(P.shape[0]):
+        n = int(n_valid[r])
+        p, x = P[r, :n], z[r, :n]
+        m = x.max()
+        lse = m + math.log(np.exp(x - m).sum())
+        nz = p > 0
+        out[r] = float((p[nz] * (np.log(p[nz]) - (x[nz] - lse))).sum())
+    return out

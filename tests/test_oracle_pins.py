@@ -485,3 +485,35 @@ def test_served_scorer_relu_and_zero_ties():
     idx, cnt = orc.topk(R, nv, k)
     for t in range(k, L):
         assert np.array_equal(idx[t], np.arange(k)), t
+
+
+# ------------------------------------------------------------------ support-level diagnostics
+
+def test_support_overlap_pins():
+    a = np.array([[0, 2, 5, 9], [1, 3, -1, -1], [4, 5, 6, 7]], dtype=np.int32)
+    b = np.array([[2, 3, 9, 11], [0, 2, 4, -1], [4, 5, 6, 7]], dtype=np.int32)
+    assert orc.support_overlap(a, b).tolist() == [2, 0, 4]
+    assert orc.support_overlap(a, a).tolist() == [4, 2, 4]            # a support recovers itself; padding is ignored
+    rng = np.random.Generator(np.random.Philox(5))
+    x = np.sort(rng.permutation(200)[:50]); y = np.sort(rng.permutation(200)[:70])
+    assert orc.support_overlap(x[None], y[None])[0] == len(np.intersect1d(x, y))
+
+
+def test_row_kl_pins():
+    rng = np.random.Generator(np.random.Philox(6))
+    n = 37
+    z = rng.standard_normal((3, 64))
+    nv = np.array([n, 5, 64])
+    sm = np.zeros_like(z)
+    for r in range(3):
+        e = np.exp(z[r, :nv[r]] - z[r, :nv[r]].max()); sm[r, :nv[r]] = e / e.sum()
+    assert np.allclose(orc.row_kl(sm, z, nv), 0.0, atol=1e-12)         # KL(p || p) = 0
+    assert np.allclose(orc.row_kl(sm, z + 3.25, nv), 0.0, atol=1e-12)  # softmax is shift invariant
+    # uniform student: KL(P || U_n) = log n - H(P)
+    P = sm[0:1]; H = -(P[0, :n] * np.log(P[0, :n])).sum()
+    assert abs(orc.row_kl(P, np.zeros((1, 64)), nv[:1])[0] - (math.log(n) - H)) < 1e-12
+    # one-hot teacher: KL = -log softmax(z)[j]; non-negative in general (Gibbs)
+    oh = np.zeros((1, 64)); oh[0, 3] = 1.0
+    assert abs(orc.row_kl(oh, z[0:1], nv[:1])[0] + math.log(sm[0, 3])) < 1e-12
+    Q = rng.random((4, 64)); Q[:, 40:] = 0; Q /= Q.sum(1, keepdims=True)
+    assert np.all(orc.row_kl(Q, rng.standard_normal((4, 64)), np.full(4, 40)) >= 0)

@@ -143,6 +143,17 @@ int sp_sparse_gqa_attn(const sp_params *p, const void *Q, const void *K, const v
 int sp_dense_gqa_attn(const sp_params *p, const void *Q, const void *K, const void *V, void *O, float *lse,
                       void *ws, size_t ws_bytes, void *stream);
 
+/* Support-level diagnostics (PAPER.md:478: "which part of the oracle support the indexer recovers"; :262 the
+ * distillation objective evaluated forward only).  Not on the serving path; both are single bandwidth-bound passes.
+ *   sp_support_overlap: inter[r] = |S_a(r) & S_b(r)| for two index tensors [sp_num_rows(p), k] in the layout
+ *     sp_topk_support emits (ascending, -1 padded), e.g. the oracle-mode and the indexer-mode supports.
+ *   sp_row_kl: kl[r - row_begin] = KL(P_t || softmax(z_t)) over the valid causal keys of per-query row r
+ *     (b_sel must be 1: a block-max row is not a distribution); P = a mass panel, z = an indexer score panel of the
+ *     SAME rows, fp32 with their own leading dimensions; terms with P = 0 contribute 0. */
+int sp_support_overlap(const sp_params *p, const int32_t *idx_a, const int32_t *idx_b, int32_t *inter, void *stream);
+int sp_row_kl(const sp_params *p, const float *mass, int64_t ld_mass, const float *scores, int64_t ld_scores,
+              int32_t row_begin, int32_t row_count, float *kl, void *stream);
+
 /* One patched layer on one stream (PAPER.md:292 five-stage path without the paged-cache stage; Alg.1 steps
  * 2-5 in SP_MODE_ORACLE, Alg.2 steps 2,4,5 in SP_MODE_INDEXER).  Support rows are processed in panels so the
  * score workspace stays bounded.

@@ -223,6 +223,17 @@ def sp_prefill_layer_host(pb: Problem, mode: int, X, Wqi, Wki, Q, K, V, O, arena
                                        _ptr(V), _ptr(O), wp, wb, _stream()))
 
 
+def sp_support_overlap(pb: Problem, idx_a: torch.Tensor, idx_b: torch.Tensor, inter: torch.Tensor):
+    p = pb.c()
+    _check(lib().sp_support_overlap(C.byref(p), _ptr(idx_a), _ptr(idx_b), _ptr(inter), _stream()))
+
+
+def sp_row_kl(pb: Problem, mass: torch.Tensor, scores: torch.Tensor, row_begin: int, row_count: int, kl: torch.Tensor):
+    p = pb.c()
+    _check(lib().sp_row_kl(C.byref(p), _ptr(mass), C.c_int64(mass.stride(0)), _ptr(scores), C.c_int64(scores.stride(0)),
+                           C.c_int32(row_begin), C.c_int32(row_count), _ptr(kl), _stream()))
+
+
 def launch_count() -> int:
     return int(lib().sp_launch_count())
 

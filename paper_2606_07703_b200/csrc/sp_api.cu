@@ -340,6 +340,29 @@ int sp_topk_support(const sp_params* p, const float* scores, int64_t ld_scores, 
   return SP_OK;
 }
 
+int sp_support_overlap(const sp_params* p, const int32_t* idx_a, const int32_t* idx_b, int32_t* inter, void* stream) {
+  const int rc = validate_common(p, false, false);
+  if (rc != SP_OK) return rc;
+  if (!idx_a || !idx_b || !inter) return SP_ERR_INVALID_ARG;
+  SP_CUDA(sp_launch_overlap(idx_a, idx_b, host_geom(p).num_rows(), p->k, inter, (cudaStream_t)stream), "support overlap");
+  return SP_OK;
+}
+
+int sp_row_kl(const sp_params* p, const float* mass, int64_t ld_mass, const float* scores, int64_t ld_scores,
+              int32_t row_begin, int32_t row_count, float* kl, void* stream) {
+  int rc = validate_common(p, false, false);
+  if (rc != SP_OK) return rc;
+  if (p->b_sel != 1) return SP_ERR_UNSUPPORTED;
+  if (!mass || !scores || !kl) return SP_ERR_INVALID_ARG;
+  int max_nv = 0;
+  rc = validate_panel(p, row_begin, row_count, ld_mass, &max_nv);
+  if (rc != SP_OK) return rc;
+  if (ld_scores < max_nv) return SP_ERR_INVALID_ARG;
+  SP_CUDA(sp_launch_row_kl(dev_geom(p), mass, ld_mass, scores, ld_scores, row_begin, row_count, kl, (cudaStream_t)stream),
+          "row KL");
+  return SP_OK;
+}
+
 int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
                        float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
   const int rc = validate_common(p, true, false);

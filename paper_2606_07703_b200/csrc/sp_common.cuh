@@ -126,4 +126,10 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
                               int d, float scale, int local_window, float local_bias, void* O, float* lse,
                               cudaStream_t st);
 
+// diagnostics (sp_diag.cu)
+cudaError_t sp_launch_overlap(const int32_t* a, const int32_t* b, long long n_rows, int k, int32_t* inter,
+                              cudaStream_t st);
+cudaError_t sp_launch_row_kl(const SpGeom& g, const float* P, int64_t ldp, const float* z, int64_t ldz, int row_begin,
+                             int row_count, float* kl, cudaStream_t st);
+
 void sp_count_launch(int n = 1);

@@ -441,3 +441,54 @@ def test_config5_varlen_pack_sampled():
 def test_degenerate_shapes(L, k, b):
     cfg = gen.shrink(gen.C1, L, k=k, b_sel=b)
     run_layer_and_compare(cfg, rows=None, n_queries=None)
+
+
+# ------------------------------------------------------------------ support-level diagnostics
+
+def test_support_overlap_matches_oracle():
+    rng = np.random.Generator(np.random.Philox(91))
+    L, k, b = 3000, 257, 1
+    pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
+    rows = pbg.num_rows
+    def make():
+        out = np.full((rows, k), -1, np.int32)
+        for r in range(rows):
+            n = min(k, r + 1)
+            m = n if r % 7 else max(1, n // 2)          # some rows shorter than the budget
+            out[r, :m] = np.sort(rng.permutation(r + 1)[:m])
+        return out
+    a, c = make(), make()
+    inter = torch.full((rows,), -7, dtype=torch.int32, device=DEV)
+    B.sp_support_overlap(pbg, torch.from_numpy(a).to(DEV), torch.from_numpy(c).to(DEV), inter)
+    assert np.array_equal(inter.cpu().numpy(), orc.support_overlap(a, c))
+    B.sp_support_overlap(pbg, torch.from_numpy(a).to(DEV), torch.from_numpy(a).to(DEV), inter)
+    assert np.array_equal(inter.cpu().numpy(), (a >= 0).sum(1))
+
+
+def test_row_kl_matches_oracle():
+    cfg = gen.shrink(gen.C4_SWEEP[0], 900, Hq=8, Hkv=2, hidden=256, k=64)
+    inp = gen.make_inputs(cfg, with_indexer=True)
+    pbo = orc_problem(cfg)
+    pbg = B.Problem.from_config(cfg)
+    rows = pbg.num_rows
+    r0, cnt = 100, 700
+    mass = torch.zeros(cnt, cfg.L, dtype=torch.float32, device=DEV)
+    sc = torch.zeros(cnt, cfg.L + 4, dtype=torch.float32, device=DEV)        # a different leading dimension
+    q = torch.empty(cfg.L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
+    k = torch.empty_like(q)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    B.sp_oracle_mass(pbg, dev(inp["Q"]), dev(inp["K"]), lse, False, r0, cnt, mass)
+    B.sp_indexer_scores(pbg, dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"]), q, k, False, r0, cnt, sc, ws)
+    kl = torch.empty(cnt, dtype=torch.float32, device=DEV)
+    B.sp_row_kl(pbg, mass, sc, r0, cnt, kl)
+    nv = np.arange(r0, r0 + cnt) + 1
+    want = orc.row_kl(to_f64(mass), to_f64(sc), nv)                           # same (GPU) rows, fp64 arithmetic
+    got = to_f64(kl)
+    assert np.all(got >= -1e-5)
+    assert np.allclose(got, want, rtol=1e-4, atol=1e-5)
+    # and against the oracle's own rows end to end (looser: fp32 mass / scores feed the GPU number)
+    Ro, nvo = orc.support_scores(pbo, orc.MODE_ORACLE, inp["Q"], inp["K"], np.arange(r0, r0 + 50))
+    qi = orc.project(pbo, inp["X"], inp["Wqi"]); ki = orc.project(pbo, inp["X"], inp["Wki"], key=True)
+    Zo, _ = orc.support_scores(pbo, orc.MODE_INDEXER, qi, ki, np.arange(r0, r0 + 50))
+    assert np.allclose(got[:50], orc.row_kl(Ro, Zo, nvo), rtol=1e-3, atol=1e-5)

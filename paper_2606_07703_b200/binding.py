@@ -26,7 +26,7 @@ SP_F_RELU, SP_F_KEY_LN, SP_F_ROPE = 1, 2, 4   # sp_params.flags: the served scor
 EXPORTS = (
     "sp_num_rows", "sp_workspace_bytes", "sp_indexer_scores", "sp_oracle_mass", "sp_topk_support",
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
-    "sp_prefill_layer_host", "sp_strerror", "sp_launch_count",
+    "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
 )
 
 

@@ -8,7 +8,8 @@ the metric is quoted on (`--workload c5` runs the 128K one).  `value` = tokens/s
 in HBM; `e2e` = the same through sp_prefill_layer_host with pinned HOST buffers (copies inside the
 timed region).  The dense GQA layer of the same library is timed in the same run.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c2|c1] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c2|c1|c4] [--impl reference]
+  (--workload c4 prints the oracle-vs-indexer length sweep of BASELINE.json configs[3]: overlap + stage split)
 
 N > 1 (torchrun): the path does not shard (one GPU per layer call, no collectives) -> N independent
 replicas, value = N * L / max-over-ranks time ("replicas only").
@@ -169,6 +170,102 @@ def workload_config(cfg):
 # GPU leg
 # ------------------------------------------------------------------------------------------------
 
+def run_c4_sweep(args, B, torch, gen, peaks):
+    """BASELINE.json configs[3]: oracle-vs-indexer length sweep, per-query supports.  For every (L, k) of the sweep:
+    the layer in both modes (CUDA events, device-resident inputs), the stage split of each mode (staged C-ABI calls on
+    the MIDDLE row panel, scaled by rows / panel rows: per-row cost is linear in the row's prefix length), the support
+    overlap |S_oracle & S_indexer| / |S_oracle| (sp_support_overlap) and the mean forward KL(P || softmax(z)) of the
+    panel's rows (sp_row_kl).  X is drawn independently of Q/K/V and the indexer weights are random, so the overlap is
+    the paper's "untrained indexer" regime (A21): near chance by construction, reported as measured."""
+    import numpy as np
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps, warm=1):
+        for _ in range(warm):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    out = []
+    l0 = B.launch_count()
+    reps = max(1, min(args.steps, 3))
+    for cfg in gen.C4_SWEEP:
+        inp = gen.make_inputs(cfg, with_indexer=True)
+        dv = {n: B.bf16_tensor(inp[n]) for n in ("X", "Wqi", "Wki", "Q", "K", "V")}
+        pb = B.Problem.from_config(cfg)
+        L, k, n_rows = cfg.L, cfg.k, pb.num_rows
+        O = torch.empty(L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+        idx_i = torch.empty(n_rows, k, dtype=torch.int32, device="cuda")
+        idx_o = torch.empty_like(idx_i)
+        ws = B.alloc_workspace(pb, B.SP_STAGE_LAYER_ORACLE)
+        ws_i = B.alloc_workspace(pb, B.SP_STAGE_LAYER_INDEXER)
+        t_idx = timed(lambda: B.sp_prefill_layer(pb, B.SP_MODE_INDEXER, dv["X"], dv["Wqi"], dv["Wki"], dv["Q"], dv["K"],
+                                                 dv["V"], O, idx_i, ws_i), reps)
+        t_orc = timed(lambda: B.sp_prefill_layer(pb, B.SP_MODE_ORACLE, None, None, None, dv["Q"], dv["K"], dv["V"], O,
+                                                 idx_o, ws), reps)
+        del ws, ws_i
+        # ---- support overlap ----
+        inter = torch.empty(n_rows, dtype=torch.int32, device="cuda")
+        B.sp_support_overlap(pb, idx_o, idx_i, inter)
+        cnt = (idx_o >= 0).sum(1)
+        beyond = cnt.new_tensor(np.arange(n_rows) + 1 > k, dtype=torch.bool)
+        pooled = float(inter.sum().item()) / float(cnt.sum().item())
+        pooled_beyond = float(inter[beyond].sum().item()) / max(1.0, float(cnt[beyond].sum().item()))
+        chance = float((k / (torch.arange(n_rows, device="cuda")[beyond] + 1).double()).mean().item()) if bool(beyond.any()) else 1.0
+        # ---- stage split on the middle panel ----
+        ld = (L + 3) // 4 * 4
+        panel = min(n_rows, max(1, (1 << 30) // (ld * 4)))
+        r0 = (n_rows - panel) // 2
+        f = n_rows / panel
+        sc = torch.empty(panel, ld, dtype=torch.float32, device="cuda")
+        ms = torch.empty(panel, ld, dtype=torch.float32, device="cuda")
+        q_idx = torch.empty(L, cfg.d_idx, dtype=torch.bfloat16, device="cuda")
+        k_idx = torch.empty_like(q_idx)
+        lse = torch.empty(L, cfg.Hq, dtype=torch.float32, device="cuda")
+        idx_p = torch.empty(panel, k, dtype=torch.int32, device="cuda")
+        wsx = B.alloc_workspace(pb, B.SP_STAGE_INDEXER_SCORES)
+        t_both = timed(lambda: B.sp_indexer_scores(pb, dv["X"], dv["Wqi"], dv["Wki"], q_idx, k_idx, False, r0, panel, sc, wsx), reps)
+        t_sc = timed(lambda: B.sp_indexer_scores(pb, None, None, None, q_idx, k_idx, True, r0, panel, sc), reps)
+        t_p1 = timed(lambda: B.sp_dense_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], None, lse), reps)
+        t_p2 = timed(lambda: B.sp_oracle_mass(pb, dv["Q"], dv["K"], lse, True, r0, panel, ms), reps)
+        t_tk = timed(lambda: B.sp_topk_support(pb, sc, r0, panel, idx_p), reps)
+        t_at = timed(lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_i, O), reps)
+        kl = torch.empty(panel, dtype=torch.float32, device="cuda")
+        B.sp_row_kl(pb, ms, sc, r0, panel, kl)
+        pairs = k * L - k * (k - 1) // 2
+        out.append({
+            "L": L, "k": k, "indexer_layer_ms": t_idx, "oracle_layer_ms": t_orc,
+            "overlap_pooled": pooled, "overlap_pooled_rows_beyond_budget": pooled_beyond, "overlap_chance_level": chance,
+            "mean_forward_kl_nats_middle_panel": float(kl.double().mean().item()),
+            "stages_ms": {"projection": max(t_both - t_sc, 0.0), "scoring": t_sc * f, "mass_pass1_lse": t_p1,
+                          "mass_pass2": t_p2 * f, "topk": t_tk * f, "sparse_attention_per_query": t_at},
+            "gather_GBps": 4.0 * cfg.Hkv * cfg.d * pairs / (t_at * 1e-3) / 1e9,
+            "mass_pass2_TFLOPs": 2.0 * cfg.d * cfg.Hq * (L * (L + 1) // 2) / (t_p2 * f * 1e-3) / 1e12,
+            "panel_rows": [r0, r0 + panel],
+        })
+        del dv, O, idx_i, idx_o, sc, ms, inp
+        torch.cuda.empty_cache()
+    ref = next(e for e in out if e["L"] == 32768)
+    line = {"metric": METRIC, "value": 32768 / (ref["indexer_layer_ms"] * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": reps, "warmup": 1, "ms_per_step": ref["indexer_layer_ms"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[3] (c4): oracle-vs-indexer length sweep, per-query supports; "
+                                   "value = the L=32768 indexer-mode layer", "Hq": 32, "Hkv": 8, "d": 128, "d_idx": 128,
+                       "b_sel": 1, "parallelism": "replicas only (no sharding, no collectives)"},
+            "gpu_launches": int(B.launch_count() - l0), "sweep": out,
+            "roofline": {"bound": "hbm", "achieved": ref["gather_GBps"], "peak": peaks["hbm"], "unit": "GB/s",
+                         "frac": ref["gather_GBps"] / peaks["hbm"], "traffic": None,
+                         "kernel": "sparse_attention_per_query (gathered K/V rows, mostly L2 hits)",
+                         "peak_source": peaks["source"]}}
+    print(json.dumps(line))
+
+
 def measure_layer_only(cfg, B, torch, gen, steps):
     """Layer latency of another workload (device-resident inputs, CUDA events, 3 warm-up steps) next to the dense
     GQA layer of the same library on the same tensors."""
@@ -217,6 +314,12 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
     from paper_2606_07703_b200 import inputs as gen
+    if args.workload == "c4" and args.impl != "reference":
+        import torch
+        from paper_2606_07703_b200 import binding as B
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        B.lib()
+        return run_c4_sweep(args, B, torch, gen, load_peaks())
     cfg = gen.ALL[args.workload]
     if args.impl == "reference":
         return run_reference(args, cfg)

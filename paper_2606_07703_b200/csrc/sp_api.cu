@@ -182,6 +182,9 @@ cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const voi
     return sp_launch_attn_tc(g, hg.num_rows(), c_hi - c_lo + 1, c_lo, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d,
                              attn_scale(p), p->local_window, p->local_bias, O, lse, st);
   }
+  if (idx != nullptr && !(debug_simt() & 4))  // per-query / small-block supports: warp-level mma.sync + cp.async gathers
+    return sp_launch_attn_pq(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
+                             q_begin, q_count, O, lse, st);
   return sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
                         q_begin, q_count, O, lse, st);
 }

@@ -126,6 +126,11 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
                               int d, float scale, int local_window, float local_bias, void* O, float* lse,
                               cudaStream_t st);
 
+// per-query gather-sparse attention on mma.sync (sp_mma_attn.cu)
+cudaError_t sp_launch_attn_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,
+                              int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int q_begin,
+                              int q_count, void* O, float* lse, cudaStream_t st);
+
 // diagnostics (sp_diag.cu)
 cudaError_t sp_launch_overlap(const int32_t* a, const int32_t* b, long long n_rows, int k, int32_t* inter,
                               cudaStream_t st);

@@ -103,6 +103,43 @@ def test_topk_exact(L, b, k, cu, quant):
         assert np.array_equal(idx.cpu().numpy(), want_idx)
 
 
+@pytest.mark.parametrize("pattern", ["ramp_up", "ramp_down", "two_level", "spike_tail", "neg_inf_mix"])
+@pytest.mark.parametrize("k", [1, 300, 1999, 2048])
+def test_topk_adversarial_rows(pattern, k):
+    """Rows built to defeat the sampled bracket of the selector: monotone ramps put every bracketed candidate into ONE
+    warp's segment (list overflow -> exact radix fallback), two-level rows are one giant tie around the threshold,
+    spike_tail hides the top values where a strided sample is sparse, neg_inf_mix has -inf entries."""
+    L, b = 33000, 3000                                     # 11 block rows with n = 3000 ... 33000
+    pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
+    pbo = orc.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
+    rows = pbg.num_rows
+    rng = np.random.Generator(np.random.Philox(4242 + k))
+    x = np.zeros((rows, L), np.float32)
+    t = np.arange(L, dtype=np.float32)
+    for r in range(rows):
+        if pattern == "ramp_up":
+            x[r] = t * 1e-3
+        elif pattern == "ramp_down":
+            x[r] = -t * 1e-3
+        elif pattern == "two_level":
+            x[r] = np.where(rng.random(L) < 0.5, 1.0, 2.0)
+        elif pattern == "spike_tail":
+            x[r] = rng.standard_normal(L) * 0.01
+            n = min(L, (r + 1) * b)
+            x[r, n - 40:n] += 5.0
+        else:
+            x[r] = rng.standard_normal(L)
+            x[r, rng.random(L) < 0.7] = -np.inf
+    info = [orc.row_info(pbo, i) for i in range(rows)]
+    nv = np.array([t1 + 1 for _, _, t1 in info], np.int32)
+    want_idx, want_cnt = orc.topk(x.astype(np.float64), nv, k)
+    idx = torch.full((rows, k), -7, dtype=torch.int32, device=DEV)
+    cnt = torch.full((rows,), -7, dtype=torch.int32, device=DEV)
+    B.sp_topk_support(pbg, torch.from_numpy(x).to(DEV), 0, rows, idx, cnt)
+    assert np.array_equal(cnt.cpu().numpy(), want_cnt)
+    assert np.array_equal(idx.cpu().numpy(), want_idx)
+
+
 # ------------------------------------------------------------------ a1/a2/a3 indexer: stage-isolated
 
 SMALL_IDX = gen.shrink(gen.C2, 1500)                  # ragged vs 64 and 128, d_idx = 64, hidden = 1024

@@ -356,6 +356,33 @@ def test_dense_attention_matches_oracle(cfg):
     assert np.allclose(to_f64(lse), l, rtol=0, atol=2e-5)
 
 
+@pytest.mark.parametrize("b", [64, 1])
+def test_attention_growing_logits_rescale_path(b):
+    """Logits that keep growing along the key axis (later keys dominate by > 2^8) force the lazy O rescale of the
+    tcgen05 kernel in most tiles, and large magnitudes check that nothing overflows; dense and sparse paths."""
+    cfg = SMALL_ORC128
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    Kf = orc.bf16_to_f64(inp["K"]).reshape(cfg.L, cfg.Hkv, cfg.d)
+    Qf = orc.bf16_to_f64(inp["Q"]).reshape(cfg.L, cfg.Hq, cfg.d)
+    u = np.ones(cfg.d) / math.sqrt(cfg.d)
+    Kf = Kf + (np.arange(cfg.L)[:, None, None] * 0.25) * u          # <q, k_s> grows by ~0.25 * <q,u> per key
+    Qf = Qf + 6.0 * u
+    Kb, Qb = orc.f64_to_bf16(Kf), orc.f64_to_bf16(Qf)
+    over = dict(b_sel=b, k=200)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    res = orc.prefill_layer(pbo, orc.MODE_ORACLE, Qb, Kb, inp["V"])
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    B.sp_sparse_gqa_attn(pbg, dev(Qb), dev(Kb), dev(inp["V"]), torch.from_numpy(res.idx).to(DEV), O)
+    parity.compare_attention(to_f64(O), res.out)
+    O2 = torch.full_like(O, float("nan"))
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    B.sp_dense_gqa_attn(pbg, dev(Qb), dev(Kb), dev(inp["V"]), O2, lse)
+    o, l = orc.dense_attn(pbo, Qb, Kb, inp["V"], np.arange(cfg.L), want_lse=True)
+    parity.compare_attention(to_f64(O2), o)
+    assert np.allclose(to_f64(lse), l, rtol=1e-6, atol=2e-4)
+
+
 def test_varlen_small_pack_layer():
     cfg = gen.shrink(gen.C5_VARLEN, 1000, cu_seqlens=(0, 300, 301, 690, 1000), hidden=256, k=100, b_sel=32)
     run_layer_and_compare(cfg, rows=None, n_queries=None)

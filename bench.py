@@ -80,6 +80,20 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm), "power_w_max": max(float(s[2]) for s in self.samples)}
 
 
+def replicas_aggregate(ms_local, tokens_per_replica, dist=None, device="cpu"):
+    """"Replicas only" scaling rule: every rank runs the same layer on its own GPU with no data-path
+    collective; the job's step time is the MAX over ranks and the aggregate value is world * tokens / that time."""
+    import torch
+    world = 1
+    ms = float(ms_local)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        world = dist.get_world_size()
+    return ms, world * tokens_per_replica / (ms * 1e-3)
+
+
 def kept_pairs(L, k):
     k = min(k, L)
     return k * L - k * (k - 1) // 2
@@ -377,13 +391,7 @@ def main():
     ev1.record(stream)
     barrier()
     launches = B.launch_count() - l0
-    ms_total = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / args.steps
-    value = world * cfg.L / (ms_step * 1e-3)
+    ms_step, value = replicas_aggregate(ev0.elapsed_time(ev1) / args.steps, cfg.L, dist, "cuda")
 
     # ---- CUDA-event timing of a staged call on the launching stream ----
     def time_call(fn, reps):
@@ -485,11 +493,7 @@ def main():
         e2e_step()
     bb.record(stream)
     barrier()
-    e2e_ms = a.elapsed_time(bb) / e2e_reps
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms, _ = replicas_aggregate(a.elapsed_time(bb) / e2e_reps, cfg.L, dist, "cuda")
     sampler.stop()
     h2d = sum(host[n].numel() * 2 for n in names)
     d2h = O_host.numel() * 2

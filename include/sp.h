@@ -96,8 +96,9 @@ int64_t sp_num_rows(const sp_params *p);
  * For the two LAYER stages the figure includes the score panel and the index buffer. */
 int sp_workspace_bytes(const sp_params *p, int stage, size_t *bytes_out);
 
-/* Indexer support-row scores (PAPER.md:270 projections, :274 scaled similarity without LN/RoPE/ReLU,
- * :299 max-aggregate over each b_sel block; Alg.2 steps 2 and 4).
+/* Indexer support-row scores (PAPER.md:270 projections, :274 scaled similarity -- plain when flags == 0, with the
+ * key LayerNorm / RoPE / ReLU of the served scorer when the SP_F_* flags ask for them --, :299 max-aggregate over
+ * each b_sel block; Alg.2 steps 2-4).
  *   preprojected == 0: q_idx = bf16(X Wqi), k_idx = bf16(X Wki) are computed for ALL L tokens (fp32
  *     accumulate, one round-to-nearest-even to bf16) and written to q_idx / k_idx (outputs, [L,d_idx]).
  *   preprojected != 0: X, Wqi, Wki are ignored (may be NULL); q_idx / k_idx are inputs.

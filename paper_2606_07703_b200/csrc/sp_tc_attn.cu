@@ -128,7 +128,6 @@ struct AtBarriers {
   uint64_t sfull[2][2];  // MMA -> softmax: S tile (M tile, buffer) is in TMEM
   uint64_t sdone[2][2];  // softmax -> MMA: S has been read (and P written over it)
   uint64_t ofull[2];     // MMA -> softmax: one completion per PV of that M tile (lazy-rescale path)
-  uint64_t pfree[2][2];  // PV issuer -> S issuer: the PV that read P from S buffer (M tile, buffer) has finished
   uint64_t ofin[2];      // MMA -> softmax: one completion per ITEM, after its last PV (epilogue).  A parity wait on
                          // ofull could alias here: the softmax may be two PVs ahead of the tensor pipe.
   uint64_t oempty[2];    // softmax -> MMA: the item's O accumulator has been read out
@@ -225,8 +224,6 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       }
       mbar_init(&bar.ofull[m], 1);
       mbar_init(&bar.ofin[m], 1);
-      mbar_init(&bar.pfree[m][0], 1);
-      mbar_init(&bar.pfree[m][1], 1);
       mbar_init(&bar.oempty[m], 128);
       mbar_init(&bar.idxfull[m], 128);
       mbar_init(&bar.idxempty[m], 256);

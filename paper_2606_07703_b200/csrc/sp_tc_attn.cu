@@ -172,7 +172,8 @@ __device__ __forceinline__ int at_item_id(int i, int c, int P, int n_items) {
 
 template <int D, int G, bool SPARSE, bool WITH_O>
 __global__ void __launch_bounds__(AT_THREADS, 1)
-sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ K,
+sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_bfloat16* __restrict__ Q,
+                  const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
                   int local_window, float local_bias, int chunks_per_row, int n_chunks, int chunk_base, int n_items,
                   int n_stages, int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
@@ -209,7 +210,8 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
 
   // ---- barriers, TMEM ----
   if (threadIdx.x == 0) {
-    mbar_init(&bar.qfull, 128);
+    mbar_init(&bar.qfull, 1);
+    tma_prefetch_desc(&tmQ);
     mbar_init(&bar.qempty, 2);
     for (int s = 0; s < AT_MAX_STAGES; ++s) {
       mbar_init(&bar.kfull[s], 128);
@@ -248,6 +250,58 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     const int key0 = ptid / CPR;
     const uint32_t kv_off = (uint32_t)(c / 8) * KV_BLK;
     uint32_t gk = 0, n_q = 0, n_it = 0;
+    // ---- index-list staging runs ONE ITEM AHEAD of the K/V loads (its global loads have L2 / DRAM latency and would
+    // otherwise sit between two items): `is` / n_st walk the same item sequence as `i` / n_it ----
+    int is = 0;
+    uint32_t n_st = 0;
+    int nt_buf[2] = {0, 0};
+    auto stage_next = [&]() {  // stage the next valid item's support row into buffer n_st & 1 (SPARSE only)
+      AtItem its;
+      for (;; ++is) {
+        if (is * P >= n_items) return;
+        const int ids = at_item_id(is, cta, P, n_items);
+        if (ids >= 0 && at_item<G, SPARSE>(g, ids, Hkv, chunks_per_row, n_chunks, chunk_base, its)) break;
+      }
+      ++is;
+      const int ib = n_st & 1, iu = n_st >> 1;
+      if (iu > 0) mbar_wait(&bar.idxempty[ib], (iu - 1) & 1);  // the softmax warps are done with item n_st - 2
+      int* siw = sIdx + ib * kpad;
+      uint32_t* fl = sFlag + ib * ntmax;
+      for (int t = ptid; t < ntmax; t += 128) fl[t] = 0u;
+      if (ptid == 0) n_eff_sh[ib] = 0;
+      loader_bar_sync();
+      const int32_t* sup = idx + (size_t)its.row * k;
+      const int qa0 = its.seq_start + its.t0, qa1 = qa0 + 128 / G, plast = its.seq_start + its.t1;
+      int my_last = 0;
+      for (int e0 = ptid; e0 < kpad; e0 += 128 * 8) {  // 8 independent loads in flight per thread
+        int pv[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int e = e0 + u * 128;
+          pv[u] = e < k ? __ldg(sup + e) : -1;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int e = e0 + u * 128;
+          if (e < kpad) {
+            const int p = pv[u];
+            const bool ok = p >= its.seq_start && p <= plast;
+            siw[e] = ok ? p : -1;
+            uint32_t f = 0;
+            if (!ok || p > qa0 - win) f |= 1u;
+            if (!ok || p > qa1 - win) f |= 2u;
+            if (ok) my_last = e + 1;
+            if (f) atomicOr(&fl[e / AT_KT], f);
+          }
+        }
+      }
+      if (my_last) atomicMax(&n_eff_sh[ib], my_last);
+      loader_bar_sync();
+      nt_buf[ib] = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
+      mbar_arrive(&bar.idxfull[ib]);
+      ++n_st;
+    };
+    if (SPARSE) stage_next();
     for (int i = 0; i * P < n_items; ++i) {
       const int id = at_item_id(i, cta, P, n_items);
       AtItem it;
@@ -256,33 +310,11 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       const int n_mt = (nq * G > 128) ? 2 : 1;
       int nt;
       const int* si = nullptr;
+      bool staged_ahead = false;
       if (SPARSE) {
-        // ---- stage the support row's index list; per-tile flags; number of useful tiles ----
-        const int ib = n_it & 1, iu = n_it >> 1;
-        if (iu > 0) mbar_wait(&bar.idxempty[ib], (iu - 1) & 1);
-        int* siw = sIdx + ib * kpad;
-        uint32_t* fl = sFlag + ib * ntmax;
-        for (int t = ptid; t < ntmax; t += 128) fl[t] = 0u;
-        if (ptid == 0) n_eff_sh[ib] = 0;
-        loader_bar_sync();
-        const int32_t* sup = idx + (size_t)it.row * k;
-        const int qa0 = it.seq_start + it.t0, qa1 = qa0 + 128 / G, plast = it.seq_start + it.t1;
-        int my_last = 0;
-        for (int e = ptid; e < kpad; e += 128) {
-          const int p = e < k ? __ldg(sup + e) : -1;
-          const bool ok = p >= it.seq_start && p <= plast;
-          siw[e] = ok ? p : -1;
-          uint32_t f = 0;
-          if (!ok || p > qa0 - win) f |= 1u;
-          if (!ok || p > qa1 - win) f |= 2u;
-          if (ok) my_last = e + 1;
-          if (f) atomicOr(&fl[e / AT_KT], f);
-        }
-        if (my_last) atomicMax(&n_eff_sh[ib], my_last);
-        loader_bar_sync();
-        nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
-        mbar_arrive(&bar.idxfull[ib]);
-        si = siw;
+        nt = nt_buf[n_it & 1];
+        si = sIdx + (n_it & 1) * kpad;
+        if (nt == 0) stage_next();  // nothing to load for this item: keep the one-item lookahead
       } else {
         nt = it.t1 / AT_KT + 1;
       }
@@ -327,18 +359,26 @@ sp_tc_attn_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       // are prefetched BEFORE waiting for the Q buffer (released by that last S MMA).
       const int pre = min(nt, NS - 2);
       for (int j = 0; j < pre; ++j) load_tile(j);
-      {  // Q tile: row R = query * G + head; rows past the chunk repeat its last query (outputs never written)
+      {  // Q tile: ONE 3-D TMA box per 64-column block: [256/G queries] x [G heads] x [64 channels] lands as rows
+         // R = query * G + head of 128 bytes, SWIZZLE_128B (rows past the chunk are later queries or zero fill: their
+         // outputs are never written).  The cp.async version cost ~800 address instructions per loader warp per item.
         if (n_q > 0) mbar_wait(&bar.qempty, (n_q - 1) & 1);
-        for (int e = ptid; e < n_mt * 128 * CPR; e += 128) {
-          const int R = e / CPR, cc = e % CPR;
-          const int ql = min(R / G, nq - 1), h = R % G;
-          const __nv_bfloat16* src = Q + ((size_t)(it.seq_start + it.t0 + ql) * Hq + it.kvh * G + h) * D + cc * 8;
-          cp_async16(smem_u32(sQ + (cc / 8) * Q_BLK) + sw128_offset(R, cc % 8), src);
+        if (ptid == 0) {
+          mbar_expect_tx(&bar.qfull, KB * Q_BLK);
+#pragma unroll
+          for (int kb = 0; kb < KB; ++kb)
+            tma_load_3d(sQ + kb * Q_BLK, &tmQ, &bar.qfull, kb * 64, it.kvh * G, it.seq_start + it.t0);
         }
-        cp_async_arrive_noinc(&bar.qfull);
         ++n_q;
       }
-      for (int j = pre; j < nt; ++j) load_tile(j);
+      for (int j = pre; j < nt; ++j) {
+        load_tile(j);
+        if (SPARSE && !staged_ahead && (j >= 3 || j == nt - 1)) {  // a few tiles are in flight: now fetch the NEXT item's list
+          stage_next();
+          staged_ahead = true;
+        }
+      }
+      if (SPARSE && !staged_ahead) stage_next();
       gk += nt;
     }
     cp_async_wait<0>();
@@ -696,8 +736,14 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
     attr_smem = smem;
   }
   const int grid = n_items < at_sm_count() ? n_items : at_sm_count();
+  CUtensorMap tmQ;  // Q viewed as [L][Hq][D]: box = 256/G queries x G heads x 64 channels
+  {
+    cudaError_t e = sp_make_tmap_bf16_3d(&tmQ, Q, D, (uint64_t)Hkv * G, (uint64_t)g.L, (uint64_t)D * 2,
+                                         (uint64_t)Hkv * G * D * 2, G, 256 / G);
+    if (e != cudaSuccess) return e;
+  }
   sp_tc_attn_kernel<D, G, SPARSE, WITH_O><<<grid, AT_THREADS, smem, st>>>(
-      g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, cpr,
+      tmQ, g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, cpr,
       n_chunks, chunk_base, n_items, stages, kpad, (__nv_bfloat16*)O, lse);
   return cudaGetLastError();
 }

@@ -40,6 +40,21 @@ cudaError_t sp_make_tmap_bf16(CUtensorMap* out, const void* base, uint64_t rows,
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+// bf16 tensor [d2][d1][d0] (d0 contiguous) with byte strides s1, s2; box = [b2 x b1 x 64 elements], SWIZZLE_128B.
+cudaError_t sp_make_tmap_bf16_3d(CUtensorMap* out, const void* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t s1,
+                                 uint64_t s2, uint32_t b1, uint32_t b2) {
+  sp_encode_tiled_fn enc = sp_get_encode();
+  if (!enc) return cudaErrorNotSupported;
+  const cuuint64_t dims[3] = {d0, d1, d2};
+  const cuuint64_t strides[2] = {s1, s2};
+  const cuuint32_t box[3] = {64, b1, b2};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 namespace {
 
 __device__ __forceinline__ uint8_t* align1024(uint8_t* p) {

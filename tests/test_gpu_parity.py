@@ -383,6 +383,34 @@ def test_attention_growing_logits_rescale_path(b):
     assert np.allclose(to_f64(lse), l, rtol=1e-6, atol=2e-4)
 
 
+@pytest.mark.parametrize("Hq,Hkv", [(4, 4), (8, 4), (8, 1), (16, 2)])     # G = 1, 2, 8, 8
+@pytest.mark.parametrize("d", [64, 128])
+def test_attention_every_group_size(Hq, Hkv, d):
+    """Dense, block-shared sparse (tcgen05) and per-query sparse (mma.sync) attention for every supported GQA group
+    size and head dim, against the oracle on the oracle's own supports."""
+    L, k = 333, 40
+    rng = np.random.Generator(np.random.Philox(1000 + Hq * 10 + Hkv + d))
+    Qb = orc.f64_to_bf16(rng.standard_normal((L, Hq, d)))
+    Kb = orc.f64_to_bf16(rng.standard_normal((L, Hkv, d)))
+    Vb = orc.f64_to_bf16(rng.standard_normal((L, Hkv, d)))
+    for b in (1, 64):
+        kw = dict(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=b, local_window=5, local_bias=0.5)
+        pbo, pbg = orc.Problem(**kw), B.Problem(**kw)
+        res = orc.prefill_layer(pbo, orc.MODE_ORACLE, Qb, Kb, Vb)
+        O = torch.full((L, Hq, d), float("nan"), dtype=torch.bfloat16, device=DEV)
+        lse = torch.empty(L, Hq, dtype=torch.float32, device=DEV)
+        B.sp_sparse_gqa_attn(pbg, dev(Qb), dev(Kb), dev(Vb), torch.from_numpy(res.idx).to(DEV), O, lse)
+        parity.compare_attention(to_f64(O), res.out)
+        sup = np.stack([res.idx[orc.row_of_pos(pbo, t)] for t in range(L)])
+        _, lse_o = orc.sparse_attn(pbo, Qb, Kb, Vb, np.arange(L), sup, want_lse=True)
+        fin = np.isfinite(lse_o)
+        assert np.allclose(to_f64(lse)[fin], lse_o[fin], rtol=0, atol=2e-5)
+    O2 = torch.full((L, Hq, d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    B.sp_dense_gqa_attn(pbg, dev(Qb), dev(Kb), dev(Vb), O2, None)
+    o, _ = orc.dense_attn(pbo, Qb, Kb, Vb, np.arange(L), want_lse=True)
+    parity.compare_attention(to_f64(O2), o)
+
+
 def test_varlen_small_pack_layer():
     cfg = gen.shrink(gen.C5_VARLEN, 1000, cu_seqlens=(0, 300, 301, 690, 1000), hidden=256, k=100, b_sel=32)
     run_layer_and_compare(cfg, rows=None, n_queries=None)

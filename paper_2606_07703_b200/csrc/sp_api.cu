@@ -338,7 +338,7 @@ int sp_topk_support(const sp_params* p, const float* scores, int64_t ld_scores, 
   int max_nv = 0;
   rc = validate_panel(p, row_begin, row_count, ld_scores, &max_nv);
   if (rc != SP_OK) return rc;
-  SP_CUDA(sp_launch_topk(dev_geom(p), scores, ld_scores, row_begin, row_count, p->k, idx, cnt, (cudaStream_t)stream),
+  SP_CUDA(sp_launch_topk(dev_geom(p), scores, ld_scores, row_begin, row_count, p->k, max_nv, idx, cnt, (cudaStream_t)stream),
           "top-k");
   return SP_OK;
 }
@@ -420,7 +420,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
     } else {
       SP_CUDA(run_mass(p, Q, K, lse, (int)r0, rcnt, max_nv, scores, pl.ld, st), "mass pass 2");
     }
-    SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
+    SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, max_nv, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
   }
   SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st), "sparse attention");
   return SP_OK;

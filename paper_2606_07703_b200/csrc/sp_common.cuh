@@ -87,7 +87,7 @@ struct SpLaunch {
 };
 
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
-                           int32_t* idx, int32_t* cnt, cudaStream_t st);
+                           int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st);
 
 cudaError_t sp_launch_project(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
                               int hidden, int d_idx, void* ws, cudaStream_t st);

@@ -322,10 +322,69 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
   else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
 }
 
+// ---- short rows (n <= 1024): one WARP per support row, the whole row in registers (32 keys per lane, element
+// i = slot * 32 + lane), 32-step bisection with warp-wide counts, index-ordered compaction by ballots.  No shared
+// memory, no block barriers: the 1024-thread kernel above spends ~9 us per row on barriers regardless of n. ----
+constexpr int TKS_WARPS = 8;
+__global__ void __launch_bounds__(TKS_WARPS * 32)
+sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
+                     int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
+  const int lane = threadIdx.x & 31;
+  const int r = blockIdx.x * TKS_WARPS + (threadIdx.x >> 5);
+  if (r >= row_count) return;
+  const SpRow ri = sp_row_info(g, row_begin + r);
+  const int n = ri.t_last + 1;  // <= 1024 (checked by the launcher)
+  int32_t* out = idx + (size_t)r * k;
+  const int keep = min(n, k);
+  if (lane == 0 && cnt) cnt[r] = keep;
+  for (int j = keep + lane; j < k; j += 32) out[j] = -1;
+  if (n <= k) {
+    for (int j = lane; j < n; j += 32) out[j] = ri.seq_start + j;
+    return;
+  }
+  const float* x = scores + (size_t)r * ld;
+  uint32_t key[32];
+#pragma unroll
+  for (int s = 0; s < 32; ++s) {
+    const int i = s * 32 + lane;
+    key[s] = i < n ? order_key(__ldg(x + i)) : 0u;  // padding key 0 is below every tested threshold (>= 1)
+  }
+  uint32_t t = 0;
+  for (int bit = 31; bit >= 0; --bit) {  // T = the largest value with count(key >= T) >= k = the k-th largest key
+    const uint32_t c0 = t | (1u << bit);
+    int c = 0;
+#pragma unroll
+    for (int s = 0; s < 32; ++s) c += key[s] >= c0;
+    if (__reduce_add_sync(0xffffffffu, c) >= k) t = c0;
+  }
+  int cg = 0;
+#pragma unroll
+  for (int s = 0; s < 32; ++s) cg += key[s] > t;
+  const uint32_t need_eq = (uint32_t)(k - __reduce_add_sync(0xffffffffu, cg));
+  const uint32_t lt = (1u << lane) - 1u;
+  uint32_t run_gt = 0, run_eq = 0;
+#pragma unroll
+  for (int s = 0; s < 32; ++s) {
+    const int i = s * 32 + lane;
+    const bool gt = i < n && key[s] > t, eq = i < n && key[s] == t;
+    const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
+    const uint32_t pg = run_gt + __popc(mg & lt), pe = run_eq + __popc(me & lt);
+    if (gt || (eq && pe < need_eq)) out[pg + min(pe, need_eq)] = ri.seq_start + i;
+    run_gt += __popc(mg);
+    run_eq += __popc(me);
+  }
+}
+
 }  // namespace
 
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
-                           int32_t* idx, int32_t* cnt, cudaStream_t st) {
+                           int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st) {
+  if (row_count > 0 && max_n_valid <= 1024) {  // every row of the panel is short: warp-per-row kernel
+    sp_topk_small_kernel<<<(row_count + TKS_WARPS - 1) / TKS_WARPS, TKS_WARPS * 32, 0, st>>>(g, scores, ld, row_begin,
+                                                                                             row_count, k, idx, cnt);
+    sp_count_launch();
+    return cudaGetLastError();
+  }
   static bool attr_done = false;
   const size_t smem = (size_t)(TK_CACHE + TK_WARPS * TK_CAND_PER_WARP) * sizeof(uint32_t);
   if (!attr_done) {

@@ -75,6 +75,11 @@ def rand_scores(seed, rows, ld, quant=None):
     (4096, 64, 512, (0, 1000, 1700, 4096), 8),
     (300, 8, 512, None, None),           # k > L: every row keeps its whole prefix
     (1, 1, 4, None, None),
+    (1024, 1, 256, None, None),          # every row <= 1024 keys: the warp-per-row kernel
+    (1024, 1, 256, None, 8),
+    (1000, 1, 1, None, 4),               # k = 1 on one giant tie
+    (999, 4, 100, (0, 300, 999), 8),
+    (1024, 32, 1023, None, 2),
 ])
 def test_topk_exact(L, b, k, cu, quant):
     pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b, cu_seqlens=cu)

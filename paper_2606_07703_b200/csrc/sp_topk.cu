@@ -300,7 +300,7 @@ __device__ void topk_row(const float* __restrict__ x, uint32_t* keys, uint32_t* 
 
 __global__ void __launch_bounds__(TK_THREADS, 1)
 sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
-               int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
+               int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
   extern __shared__ uint32_t tk_smem[];
   __shared__ TkShared sh;
   uint32_t* keys = tk_smem;
@@ -309,6 +309,7 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
   const int r = row_count - 1 - (int)blockIdx.x;
   const SpRow ri = sp_row_info(g, row_begin + r);
   const int n = ri.t_last + 1;
+  if (n <= n_lo) return;  // a short row: sp_topk_small_kernel's
   int32_t* out = idx + (size_t)r * k;
   const int keep = min(n, k);
   if (threadIdx.x == 0 && cnt) cnt[r] = keep;
@@ -322,50 +323,95 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
   else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
 }
 
-// ---- short rows (n <= 1024): one WARP per support row, the whole row in registers (32 keys per lane, element
-// i = slot * 32 + lane), 32-step bisection with warp-wide counts, index-ordered compaction by ballots.  No shared
-// memory, no block barriers: the 1024-thread kernel above spends ~9 us per row on barriers regardless of n. ----
+// ---- short rows: W = 1, 2, 4 or 8 warps per support row (class W takes n <= 1024 W), the whole row in registers.
+// Warp w owns the contiguous segment [w * seg, (w + 1) * seg) of the row (seg a multiple of 32, element
+// i = w * seg + slot * 32 + lane, at most 32 slots).  32-step bisection on the order-preserving keys with
+// `redux.sync` counts (W > 1: combined through a double-buffered shared array, one named barrier of the row's W
+// warps per step), then an
+// index-ordered compaction by ballots from per-warp bases.  The 1024-thread kernel above spends ~9 us per row on
+// block barriers whatever n is; this one costs O(n) issue slots.  A row is processed iff n_lo < n <= n_hi, so that
+// a panel with mixed row lengths can be covered by one launch per class. ----
 constexpr int TKS_WARPS = 8;
+constexpr int TKS_NW = 1024;  // class W holds rows with n <= TKS_NW * W
+template <int W>
 __global__ void __launch_bounds__(TKS_WARPS * 32)
 sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
-                     int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
-  const int lane = threadIdx.x & 31;
-  const int r = blockIdx.x * TKS_WARPS + (threadIdx.x >> 5);
-  if (r >= row_count) return;
+                     int n_lo, int n_hi, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
+  constexpr int RPC = TKS_WARPS / W;  // rows per CTA
+  __shared__ int sh_cnt[2][TKS_WARPS];
+  __shared__ int sh_fin[2][TKS_WARPS];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int w = warp % W;
+  const int r = blockIdx.x * RPC + warp / W;
+  if (r >= row_count) return;  // uniform over the W warps of a row, which are the only ones that synchronise
   const SpRow ri = sp_row_info(g, row_begin + r);
-  const int n = ri.t_last + 1;  // <= 1024 (checked by the launcher)
+  const int n = ri.t_last + 1;
+  if (n <= n_lo || n > n_hi) return;
   int32_t* out = idx + (size_t)r * k;
   const int keep = min(n, k);
-  if (lane == 0 && cnt) cnt[r] = keep;
-  for (int j = keep + lane; j < k; j += 32) out[j] = -1;
+  const int tr = w * 32 + lane;  // thread index within the row's W warps
+  if (tr == 0 && cnt) cnt[r] = keep;
+  for (int j = keep + tr; j < k; j += W * 32) out[j] = -1;
   if (n <= k) {
-    for (int j = lane; j < n; j += 32) out[j] = ri.seq_start + j;
+    for (int j = tr; j < n; j += W * 32) out[j] = ri.seq_start + j;
     return;
   }
   const float* x = scores + (size_t)r * ld;
+  const int seg = (((n + W - 1) / W) + 31) & ~31;  // <= 1024
+  const int ns = seg >> 5;
+  const int i0 = w * seg + lane;
   uint32_t key[32];
 #pragma unroll
   for (int s = 0; s < 32; ++s) {
-    const int i = s * 32 + lane;
-    key[s] = i < n ? order_key(__ldg(x + i)) : 0u;  // padding key 0 is below every tested threshold (>= 1)
+    const int i = i0 + s * 32;
+    key[s] = (s < ns && i < n) ? order_key(__ldg(x + i)) : 0u;  // padding key 0 is below every tested threshold
   }
+  auto row_bar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + warp / W), "n"(W * 32) : "memory"); };
+  auto row_sum = [&](int c, int (*buf)[TKS_WARPS], int step) -> int {
+    c = __reduce_add_sync(0xffffffffu, c);
+    if (W == 1) return c;
+    if (lane == 0) buf[step & 1][warp] = c;
+    row_bar();  // the double buffer saves the second barrier
+    int v = lane < W ? buf[step & 1][warp - w + lane] : 0;
+    return __reduce_add_sync(0xffffffffu, v);
+  };
   uint32_t t = 0;
   for (int bit = 31; bit >= 0; --bit) {  // T = the largest value with count(key >= T) >= k = the k-th largest key
     const uint32_t c0 = t | (1u << bit);
-    int c = 0;
+    // key >= c0  <=>  key + (2^32 - c0) carries out (c0 >= 1): two instructions per key, four chains; slots past
+    // ns hold the padding key 0 < c0, no guard needed
+    const uint32_t nc0 = 0u - c0;
+    int c[4] = {0, 0, 0, 0};
 #pragma unroll
-    for (int s = 0; s < 32; ++s) c += key[s] >= c0;
-    if (__reduce_add_sync(0xffffffffu, c) >= k) t = c0;
+    for (int s = 0; s < 32; ++s)
+      asm("{\n\t.reg .u32 d;\n\tadd.cc.u32 d, %1, %2;\n\taddc.u32 %0, %0, 0;\n\t}" : "+r"(c[s & 3]) : "r"(key[s]), "r"(nc0));
+    if (row_sum((c[0] + c[1]) + (c[2] + c[3]), sh_cnt, bit) >= k) t = c0;
   }
-  int cg = 0;
-#pragma unroll
-  for (int s = 0; s < 32; ++s) cg += key[s] > t;
-  const uint32_t need_eq = (uint32_t)(k - __reduce_add_sync(0xffffffffu, cg));
-  const uint32_t lt = (1u << lane) - 1u;
-  uint32_t run_gt = 0, run_eq = 0;
+  int cg = 0, ce = 0;
 #pragma unroll
   for (int s = 0; s < 32; ++s) {
-    const int i = s * 32 + lane;
+    cg += key[s] > t;  // padding keys are 0 < T
+    ce += key[s] == t;
+  }
+  cg = __reduce_add_sync(0xffffffffu, cg);
+  ce = __reduce_add_sync(0xffffffffu, ce);
+  uint32_t run_gt = 0, run_eq = 0, total_gt = (uint32_t)cg;
+  if (W > 1) {
+    if (lane == 0) { sh_fin[0][warp] = cg; sh_fin[1][warp] = ce; }
+    row_bar();
+    total_gt = 0;
+    for (int j = 0; j < W; ++j) {
+      const uint32_t a = (uint32_t)sh_fin[0][warp - w + j], b = (uint32_t)sh_fin[1][warp - w + j];
+      total_gt += a;
+      if (j < w) { run_gt += a; run_eq += b; }
+    }
+  }
+  const uint32_t need_eq = (uint32_t)k - total_gt;
+  const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int s = 0; s < 32; ++s) {
+    if (s >= ns) break;
+    const int i = i0 + s * 32;
     const bool gt = i < n && key[s] > t, eq = i < n && key[s] == t;
     const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
     const uint32_t pg = run_gt + __popc(mg & lt), pe = run_eq + __popc(me & lt);
@@ -379,12 +425,7 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
 
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
                            int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st) {
-  if (row_count > 0 && max_n_valid <= 1024) {  // every row of the panel is short: warp-per-row kernel
-    sp_topk_small_kernel<<<(row_count + TKS_WARPS - 1) / TKS_WARPS, TKS_WARPS * 32, 0, st>>>(g, scores, ld, row_begin,
-                                                                                             row_count, k, idx, cnt);
-    sp_count_launch();
-    return cudaGetLastError();
-  }
+  if (row_count <= 0) return cudaSuccess;
   static bool attr_done = false;
   const size_t smem = (size_t)(TK_CACHE + TK_WARPS * TK_CAND_PER_WARP) * sizeof(uint32_t);
   if (!attr_done) {
@@ -392,8 +433,46 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  if (row_count <= 0) return cudaSuccess;
-  sp_topk_kernel<<<row_count, TK_THREADS, smem, st>>>(g, scores, ld, row_begin, row_count, k, idx, cnt);
-  sp_count_launch();
+  // Row classes by n = n_valid: W = 1, 2, 4, 8 warps per row for n <= 1024 W, the 1024-thread kernel for longer rows.
+  // One sequence (cu == nullptr): n(r) = min(L, (r + 1) b_sel) is monotone, each class is a contiguous row range and
+  // gets a launch over exactly that range (the bound (r + 1) b_sel is conservative, so no class filter is needed).
+  // Packed varlen: every class that can occur is launched over the whole panel and filters its rows by n.
+  const int end = row_begin + row_count;
+  const bool contiguous = g.cu == nullptr || max_n_valid <= TKS_NW;
+  auto launch_small = [&](int W, int rb, int rc, int nlo) {
+    const float* sc = scores + (size_t)(rb - row_begin) * ld;
+    int32_t* ix = idx + (size_t)(rb - row_begin) * k;
+    int32_t* cn = cnt ? cnt + (rb - row_begin) : nullptr;
+    const int grid = (rc + TKS_WARPS / W - 1) / (TKS_WARPS / W), nhi = TKS_NW * W;
+    if (W == 1) sp_topk_small_kernel<1><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
+    else if (W == 2) sp_topk_small_kernel<2><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
+    else if (W == 4) sp_topk_small_kernel<4><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
+    else sp_topk_small_kernel<8><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
+    sp_count_launch();
+  };
+  auto launch_big = [&](int rb, int rc, int nlo) {
+    sp_topk_kernel<<<rc, TK_THREADS, smem, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
+                                                 idx + (size_t)(rb - row_begin) * k,
+                                                 cnt ? cnt + (rb - row_begin) : nullptr);
+    sp_count_launch();
+  };
+  if (contiguous) {
+    // first row (absolute) whose bound (r + 1) b_sel exceeds the class limit; every row when the panel's longest fits
+    auto first_above = [&](int nmax) {
+      return max_n_valid <= nmax ? end : min(end, max(row_begin, nmax / g.b_sel));
+    };
+    const int r8 = first_above(TKS_NW * 8);
+    if (r8 < end) launch_big(r8, end - r8, -1);  // the longest rows first
+    int hi = r8;
+    for (int W = 8; W >= 1; W >>= 1) {
+      const int lo = W == 1 ? row_begin : first_above(TKS_NW * (W / 2));
+      if (lo < hi) launch_small(W, lo, hi - lo, -1);
+      hi = min(hi, lo);
+    }
+  } else {
+    if (max_n_valid > TKS_NW * 8) launch_big(row_begin, row_count, TKS_NW * 8);
+    for (int W = 8; W >= 1; W >>= 1)
+      if (W == 1 || max_n_valid > TKS_NW * (W / 2)) launch_small(W, row_begin, row_count, W == 1 ? -1 : TKS_NW * (W / 2));
+  }
   return cudaGetLastError();
 }

@@ -80,6 +80,9 @@ def rand_scores(seed, rows, ld, quant=None):
     (1000, 1, 1, None, 4),               # k = 1 on one giant tie
     (999, 4, 100, (0, 300, 999), 8),
     (1024, 32, 1023, None, 2),
+    (12000, 8, 256, None, 8),            # one panel crossing all three row classes (n <= 1024, <= 8192, longer)
+    (20000, 16, 128, (0, 900, 5000, 20000), 8),   # packed: the three classes interleaved, filtered per kernel
+    (8192, 1, 8191, None, None),
 ])
 def test_topk_exact(L, b, k, cu, quant):
     pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b, cu_seqlens=cu)

@@ -421,6 +421,16 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
   }
 }
 
+int g_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
+}
+
 }  // namespace
 
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
@@ -456,19 +466,32 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
                                                  cnt ? cnt + (rb - row_begin) : nullptr);
     sp_count_launch();
   };
+  // A class is launched only when it fills the machine (rows * W >= one 8-warp CTA per SM) or when it is the last
+  // one the panel needs; otherwise its rows are merged into the next larger class (which handles shorter rows too,
+  // less efficiently) and finally into the 1024-thread kernel: a near-empty extra launch costs more than it saves
+  // (c3 has 128 rows with n <= 8192: four extra launches made its top-k 0.068 -> 0.094 ms).
+  const int fill = g_sm_count() * TKS_WARPS;
   if (contiguous) {
     // first row (absolute) whose bound (r + 1) b_sel exceeds the class limit; every row when the panel's longest fits
     auto first_above = [&](int nmax) {
       return max_n_valid <= nmax ? end : min(end, max(row_begin, nmax / g.b_sel));
     };
-    const int r8 = first_above(TKS_NW * 8);
-    if (r8 < end) launch_big(r8, end - r8, -1);  // the longest rows first
-    int hi = r8;
-    for (int W = 8; W >= 1; W >>= 1) {
-      const int lo = W == 1 ? row_begin : first_above(TKS_NW * (W / 2));
-      if (lo < hi) launch_small(W, lo, hi - lo, -1);
-      hi = min(hi, lo);
+    int cls_w[4], cls_lo[4], cls_hi[4], ncls = 0;
+    int pending = row_begin;
+    for (int W = 1; W <= 8; W <<= 1) {
+      const int hi = first_above(TKS_NW * W);
+      const int rows = hi - pending;
+      if (rows > 0 && ((long long)rows * W >= fill || hi == end)) {
+        cls_w[ncls] = W; cls_lo[ncls] = pending; cls_hi[ncls] = hi; ++ncls;
+        pending = hi;
+      }
+      if (hi == end) break;
     }
+    if (pending < end) launch_big(pending, end - pending, -1);  // the longest rows first
+    for (int i = ncls - 1; i >= 0; --i) launch_small(cls_w[i], cls_lo[i], cls_hi[i] - cls_lo[i], -1);
+  } else if ((long long)row_count < fill) {  // packed, few rows: one launch
+    if (max_n_valid > TKS_NW * 8) launch_big(row_begin, row_count, -1);
+    else launch_small(max_n_valid > TKS_NW * 4 ? 8 : max_n_valid > TKS_NW * 2 ? 4 : 2, row_begin, row_count, -1);
   } else {
     if (max_n_valid > TKS_NW * 8) launch_big(row_begin, row_count, TKS_NW * 8);
     for (int W = 8; W >= 1; W >>= 1)

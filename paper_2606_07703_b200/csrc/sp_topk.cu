@@ -323,7 +323,8 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
   else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
 }
 
-// ---- short rows: W = 1, 2, 4 or 8 warps per support row (class W takes n <= 1024 W), the whole row in registers.
+// ---- rows up to 16384 keys: W = 1, 2, ... 16 warps per support row (class W takes n <= 1024 W), the whole row in
+// registers.
 // Warp w owns the contiguous segment [w * seg, (w + 1) * seg) of the row (seg a multiple of 32, element
 // i = w * seg + slot * 32 + lane, at most 32 slots).  32-step bisection on the order-preserving keys with
 // `redux.sync` counts (W > 1: combined through a double-buffered shared array, one named barrier of the row's W
@@ -331,15 +332,18 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
 // index-ordered compaction by ballots from per-warp bases.  The 1024-thread kernel above spends ~9 us per row on
 // block barriers whatever n is; this one costs O(n) issue slots.  A row is processed iff n_lo < n <= n_hi, so that
 // a panel with mixed row lengths can be covered by one launch per class. ----
-constexpr int TKS_WARPS = 8;
+constexpr int TKS_WARPS = 8;   // warps per CTA for W <= 8; W = 16 and 32 use one CTA of W warps per row
+constexpr int TKS_WMAX = 16;   // the largest class: n <= 16384, two rows fill the register file of an SM (W = 32, one
+                               // row per SM with nothing to overlap its barriers, measured SLOWER than sp_topk_kernel)
 constexpr int TKS_NW = 1024;  // class W holds rows with n <= TKS_NW * W
 template <int W>
-__global__ void __launch_bounds__(TKS_WARPS * 32)
+__global__ void __launch_bounds__((W > TKS_WARPS ? W : TKS_WARPS) * 32, W <= 8 ? 3 : 2)
 sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
                      int n_lo, int n_hi, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
-  constexpr int RPC = TKS_WARPS / W;  // rows per CTA
-  __shared__ int sh_cnt[2][TKS_WARPS];
-  __shared__ int sh_fin[2][TKS_WARPS];
+  constexpr int CTA_WARPS = W > TKS_WARPS ? W : TKS_WARPS;
+  constexpr int RPC = CTA_WARPS / W;  // rows per CTA
+  __shared__ int sh_cnt[2][TKS_WMAX];
+  __shared__ int sh_fin[2][TKS_WMAX];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int w = warp % W;
   const int r = blockIdx.x * RPC + warp / W;
@@ -367,7 +371,7 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
     key[s] = (s < ns && i < n) ? order_key(__ldg(x + i)) : 0u;  // padding key 0 is below every tested threshold
   }
   auto row_bar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + warp / W), "n"(W * 32) : "memory"); };
-  auto row_sum = [&](int c, int (*buf)[TKS_WARPS], int step) -> int {
+  auto row_sum = [&](int c, int (*buf)[TKS_WMAX], int step) -> int {
     c = __reduce_add_sync(0xffffffffu, c);
     if (W == 1) return c;
     if (lane == 0) buf[step & 1][warp] = c;
@@ -385,7 +389,9 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
 #pragma unroll
     for (int s = 0; s < 32; ++s)
       asm("{\n\t.reg .u32 d;\n\tadd.cc.u32 d, %1, %2;\n\taddc.u32 %0, %0, 0;\n\t}" : "+r"(c[s & 3]) : "r"(key[s]), "r"(nc0));
-    if (row_sum((c[0] + c[1]) + (c[2] + c[3]), sh_cnt, bit) >= k) t = c0;
+    const int tot = row_sum((c[0] + c[1]) + (c[2] + c[3]), sh_cnt, bit);
+    if (tot >= k) t = c0;
+    if (tot == k) break;  // exactly k keys >= c0: they are the support, whatever the lower bits of the k-th key are
   }
   int cg = 0, ce = 0;
 #pragma unroll
@@ -453,11 +459,15 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     const float* sc = scores + (size_t)(rb - row_begin) * ld;
     int32_t* ix = idx + (size_t)(rb - row_begin) * k;
     int32_t* cn = cnt ? cnt + (rb - row_begin) : nullptr;
-    const int grid = (rc + TKS_WARPS / W - 1) / (TKS_WARPS / W), nhi = TKS_NW * W;
-    if (W == 1) sp_topk_small_kernel<1><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
-    else if (W == 2) sp_topk_small_kernel<2><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
-    else if (W == 4) sp_topk_small_kernel<4><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
-    else sp_topk_small_kernel<8><<<grid, TKS_WARPS * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn);
+    const int cw = W > TKS_WARPS ? W : TKS_WARPS, rpc = cw / W;
+    const int grid = (rc + rpc - 1) / rpc, nhi = TKS_NW * W;
+    switch (W) {
+      case 1: sp_topk_small_kernel<1><<<grid, cw * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn); break;
+      case 2: sp_topk_small_kernel<2><<<grid, cw * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn); break;
+      case 4: sp_topk_small_kernel<4><<<grid, cw * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn); break;
+      case 8: sp_topk_small_kernel<8><<<grid, cw * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn); break;
+      default: sp_topk_small_kernel<16><<<grid, cw * 32, 0, st>>>(g, sc, ld, rb, rc, k, nlo, nhi, ix, cn); break;
+    }
     sp_count_launch();
   };
   auto launch_big = [&](int rb, int rc, int nlo) {
@@ -476,9 +486,9 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     auto first_above = [&](int nmax) {
       return max_n_valid <= nmax ? end : min(end, max(row_begin, nmax / g.b_sel));
     };
-    int cls_w[4], cls_lo[4], cls_hi[4], ncls = 0;
+    int cls_w[6], cls_lo[6], cls_hi[6], ncls = 0;
     int pending = row_begin;
-    for (int W = 1; W <= 8; W <<= 1) {
+    for (int W = 1; W <= TKS_WMAX; W <<= 1) {
       const int hi = first_above(TKS_NW * W);
       const int rows = hi - pending;
       if (rows > 0 && ((long long)rows * W >= fill || hi == end)) {
@@ -490,11 +500,16 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     if (pending < end) launch_big(pending, end - pending, -1);  // the longest rows first
     for (int i = ncls - 1; i >= 0; --i) launch_small(cls_w[i], cls_lo[i], cls_hi[i] - cls_lo[i], -1);
   } else if ((long long)row_count < fill) {  // packed, few rows: one launch
-    if (max_n_valid > TKS_NW * 8) launch_big(row_begin, row_count, -1);
-    else launch_small(max_n_valid > TKS_NW * 4 ? 8 : max_n_valid > TKS_NW * 2 ? 4 : 2, row_begin, row_count, -1);
+    if (max_n_valid > TKS_NW * TKS_WMAX) {
+      launch_big(row_begin, row_count, -1);
+    } else {
+      int W = 2;
+      while (TKS_NW * W < max_n_valid) W <<= 1;
+      launch_small(W, row_begin, row_count, -1);
+    }
   } else {
-    if (max_n_valid > TKS_NW * 8) launch_big(row_begin, row_count, TKS_NW * 8);
-    for (int W = 8; W >= 1; W >>= 1)
+    if (max_n_valid > TKS_NW * TKS_WMAX) launch_big(row_begin, row_count, TKS_NW * TKS_WMAX);
+    for (int W = TKS_WMAX; W >= 1; W >>= 1)
       if (W == 1 || max_n_valid > TKS_NW * (W / 2)) launch_small(W, row_begin, row_count, W == 1 ? -1 : TKS_NW * (W / 2));
   }
   return cudaGetLastError();

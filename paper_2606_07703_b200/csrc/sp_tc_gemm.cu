@@ -62,9 +62,12 @@ __device__ __forceinline__ uint8_t* align1024(uint8_t* p) {
 }
 
 // ===================================================================================================
-// Projection: C[m, 0:DI] = X[m,:] Wq, C[m, DI:2DI] = X[m,:] Wk.   M tile 128, N = 2*DI, K pipelined by 64.
+// Projection: C[m, 0:DI] = X[m,:] Wq, C[m, DI:2DI] = X[m,:] Wk.   M tile 256 (two 128-row halves, two accumulators
+// sharing every B stage: the weights are re-read from L2 once per 256 rows, which is what bounds the kernel on the
+// per-SM L2 bandwidth), N = 2*DI, K pipelined by 64.
 // ===================================================================================================
-constexpr int PJ_STAGES = 4;
+constexpr int PJ_STAGES = 3;
+constexpr int PJ_M = 256;
 
 template <int DI>
 __global__ void __launch_bounds__(128, 1)
@@ -73,7 +76,8 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
                      __nv_bfloat16* __restrict__ k_idx, int L, int hidden, SpGeom g, uint32_t flags) {
   constexpr int N = 2 * DI;
   constexpr int NG = N / 64;                  // 64-column groups of B
-  constexpr uint32_t A_BYTES = 128 * 128;     // 128 rows x 64 k
+  constexpr uint32_t A_HALF = 128 * 128;      // 128 rows x 64 k
+  constexpr uint32_t A_BYTES = 2 * A_HALF;
   constexpr uint32_t B_BYTES = NG * 64 * 128; // NG groups of [64 k-rows x 128 B]
   constexpr uint32_t STAGE = A_BYTES + B_BYTES;
   extern __shared__ uint8_t smem_raw[];
@@ -81,7 +85,8 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
   __shared__ uint64_t full[PJ_STAGES], empty[PJ_STAGES], done;
   __shared__ uint32_t tmem_slot;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m0 = blockIdx.x * 128;
+  const int m0 = blockIdx.x * PJ_M;
+  const int nh = m0 + 128 < L ? 2 : 1;  // the last tile may hold one half only
   const int nkb = hidden / 64;
 
   if (threadIdx.x == 0) {
@@ -95,7 +100,7 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     tma_prefetch_desc(&tmWq);
     tma_prefetch_desc(&tmWk);
   }
-  if (warp == 1) tmem_alloc<N>(&tmem_slot);
+  if (warp == 1) tmem_alloc<2 * N>(&tmem_slot);
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
@@ -107,8 +112,9 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
       if (kb >= PJ_STAGES) mbar_wait(&empty[s], ((kb / PJ_STAGES) - 1) & 1);
       uint8_t* a = smem + (size_t)s * STAGE;
       uint8_t* b = a + A_BYTES;
-      mbar_expect_tx(&full[s], STAGE);
+      mbar_expect_tx(&full[s], STAGE - (2 - nh) * A_HALF);
       tma_load_2d(a, &tmX, &full[s], kb * 64, m0);
+      if (nh == 2) tma_load_2d(a + A_HALF, &tmX, &full[s], kb * 64, m0 + 128);
 #pragma unroll
       for (int g = 0; g < DI / 64; ++g) {
         tma_load_2d(b + g * 8192, &tmWq, &full[s], g * 64, kb * 64);
@@ -125,9 +131,9 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
       const uint32_t b = a + A_BYTES;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const uint64_t ad = umma_desc_sw128(a + k * 32, 16, 1024);
         const uint64_t bd = umma_desc_sw128(b + k * 2048, 8192, 1024);
-        umma_ss(tmem, ad, bd, idesc, (kb | k) != 0);
+        umma_ss(tmem, umma_desc_sw128(a + k * 32, 16, 1024), bd, idesc, (kb | k) != 0);
+        if (nh == 2) umma_ss(tmem + N, umma_desc_sw128(a + A_HALF + k * 32, 16, 1024), bd, idesc, (kb | k) != 0);
       }
       umma_commit(&empty[s]);
     }
@@ -137,9 +143,10 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
   mbar_wait(&done, 0);
   tc_fence_after_sync();
 
-  // epilogue: thread = output row
-  const int m = m0 + warp * 32 + lane;
-  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  // epilogue: thread = output row of each half
+  for (int h = 0; h < nh; ++h) {
+  const int m = m0 + h * 128 + warp * 32 + lane;
+  const uint32_t trow = tmem + h * N + ((uint32_t)(warp * 32) << 16);
   if ((flags & (SP_F_KEY_LN | SP_F_ROPE)) == 0) {
 #pragma unroll
     for (int c0 = 0; c0 < N; c0 += 32) {
@@ -246,9 +253,10 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
       }
     }
   }
+  }
   tc_fence_before_sync();
   __syncthreads();
-  if (warp == 1) tmem_dealloc<N>(tmem);
+  if (warp == 1) tmem_dealloc<2 * N>(tmem);
 }
 
 }  // namespace
@@ -264,14 +272,14 @@ static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void
   if ((e = sp_make_tmap_bf16(&tmX, X, L, hidden, hidden, 128)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmWq, Wq, hidden, DI, DI, 64)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmWk, Wk, hidden, DI, DI, 64)) != cudaSuccess) return e;
-  constexpr size_t smem = (size_t)PJ_STAGES * (128 * 128 + (2 * DI / 64) * 8192) + 1024;
+  constexpr size_t smem = (size_t)PJ_STAGES * (2 * 128 * 128 + (2 * DI / 64) * 8192) + 1024;
   static bool attr_done = false;
   if (!attr_done) {
     e = cudaFuncSetAttribute(sp_tc_project_kernel<DI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  sp_tc_project_kernel<DI><<<(L + 127) / 128, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
+  sp_tc_project_kernel<DI><<<(L + PJ_M - 1) / PJ_M, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
                                                                (__nv_bfloat16*)k_idx, L, hidden, g, flags);
   sp_count_launch();
   return cudaGetLastError();

@@ -62,32 +62,32 @@ __device__ __forceinline__ uint8_t* align1024(uint8_t* p) {
 }
 
 // ===================================================================================================
-// Projection: C[m, 0:DI] = X[m,:] Wq, C[m, DI:2DI] = X[m,:] Wk.   M tile 256 (two 128-row halves, two accumulators
+// Projection: C[m, 0:DI] = X[m,:] Wq, C[m, DI:2DI] = X[m,:] Wk.   M tile 128 or 256 (`halves`: two 128-row halves, two accumulators
 // sharing every B stage: the weights are re-read from L2 once per 256 rows, which is what bounds the kernel on the
 // per-SM L2 bandwidth), N = 2*DI, K pipelined by 64.
 // ===================================================================================================
-constexpr int PJ_STAGES = 3;
-constexpr int PJ_M = 256;
+constexpr int PJ_STAGES = 4;  // ring slots with 128-token tiles (48 KB each at d_idx 128); 3 with 256-token tiles (64 KB)
 
 template <int DI>
 __global__ void __launch_bounds__(128, 1)
 sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmWq,
                      const __grid_constant__ CUtensorMap tmWk, __nv_bfloat16* __restrict__ q_idx,
-                     __nv_bfloat16* __restrict__ k_idx, int L, int hidden, SpGeom g, uint32_t flags) {
+                     __nv_bfloat16* __restrict__ k_idx, int L, int hidden, SpGeom g, uint32_t flags,
+                     int halves) {
   constexpr int N = 2 * DI;
   constexpr int NG = N / 64;                  // 64-column groups of B
   constexpr uint32_t A_HALF = 128 * 128;      // 128 rows x 64 k
-  constexpr uint32_t A_BYTES = 2 * A_HALF;
   constexpr uint32_t B_BYTES = NG * 64 * 128; // NG groups of [64 k-rows x 128 B]
-  constexpr uint32_t STAGE = A_BYTES + B_BYTES;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = align1024(smem_raw);
   __shared__ uint64_t full[PJ_STAGES], empty[PJ_STAGES], done;
   __shared__ uint32_t tmem_slot;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m0 = blockIdx.x * PJ_M;
-  const int nh = m0 + 128 < L ? 2 : 1;  // the last tile may hold one half only
+  const int m0 = blockIdx.x * 128 * halves;
+  const int nh = (halves == 2 && m0 + 128 < L) ? 2 : 1;  // the last tile may hold one half only
   const int nkb = hidden / 64;
+  const int NS = halves == 2 ? PJ_STAGES - 1 : PJ_STAGES;
+  const uint32_t A_BYTES = A_HALF * halves, STAGE = A_BYTES + B_BYTES;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < PJ_STAGES; ++i) {
@@ -107,12 +107,14 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
   const uint32_t tmem = tmem_slot;
 
   if (warp == 0 && lane == 0) {
-    for (int kb = 0; kb < nkb; ++kb) {
-      const int s = kb % PJ_STAGES;
-      if (kb >= PJ_STAGES) mbar_wait(&empty[s], ((kb / PJ_STAGES) - 1) & 1);
+    int s = 0;
+    uint32_t ph = 1;  // ring slot and the parity of its previous release (NS is a run-time value: no modulo here)
+    for (int kb = 0; kb < nkb; ++kb, ++s) {
+      if (s == NS) { s = 0; ph ^= 1; }
+      if (kb >= NS) mbar_wait(&empty[s], ph);
       uint8_t* a = smem + (size_t)s * STAGE;
       uint8_t* b = a + A_BYTES;
-      mbar_expect_tx(&full[s], STAGE - (2 - nh) * A_HALF);
+      mbar_expect_tx(&full[s], A_HALF * nh + B_BYTES);
       tma_load_2d(a, &tmX, &full[s], kb * 64, m0);
       if (nh == 2) tma_load_2d(a + A_HALF, &tmX, &full[s], kb * 64, m0 + 128);
 #pragma unroll
@@ -123,17 +125,28 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     }
   } else if (warp == 1 && lane == 0) {
     constexpr uint32_t idesc = umma_idesc_bf16(128, N, 0, 1);  // A K-major, B MN-major
-    for (int kb = 0; kb < nkb; ++kb) {
-      const int s = kb % PJ_STAGES;
-      mbar_wait(&full[s], (kb / PJ_STAGES) & 1);
+    // descriptors of ring slot 0, advanced by adding (byte offset >> 4) to the 14-bit address field (all of shared
+    // memory is below 2^18 B, so the sum cannot carry out of the field): no descriptor arithmetic inside the loop
+    const uint64_t ad0 = umma_desc_sw128(smem_u32(smem), 16, 1024);
+    const uint64_t bd0 = umma_desc_sw128(smem_u32(smem) + A_BYTES, 8192, 1024);
+    const uint64_t st16 = STAGE >> 4;
+    int s = 0;
+    uint32_t ph = 0;
+    uint64_t so = 0;
+    for (int kb = 0; kb < nkb; ++kb, ++s, so += st16) {
+      if (s == NS) { s = 0; ph ^= 1; so = 0; }
+      mbar_wait(&full[s], ph);
       tc_fence_after_sync();
-      const uint32_t a = smem_u32(smem + (size_t)s * STAGE);
-      const uint32_t b = a + A_BYTES;
+      const uint64_t ad = ad0 + so, bd = bd0 + so;
+      if (nh == 2) {
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const uint64_t bd = umma_desc_sw128(b + k * 2048, 8192, 1024);
-        umma_ss(tmem, umma_desc_sw128(a + k * 32, 16, 1024), bd, idesc, (kb | k) != 0);
-        if (nh == 2) umma_ss(tmem + N, umma_desc_sw128(a + A_HALF + k * 32, 16, 1024), bd, idesc, (kb | k) != 0);
+        for (int k = 0; k < 4; ++k) {
+          umma_ss(tmem, ad + k * 2, bd + k * 128, idesc, (kb | k) != 0);
+          umma_ss(tmem + N, ad + (A_HALF >> 4) + k * 2, bd + k * 128, idesc, (kb | k) != 0);
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) umma_ss(tmem, ad + k * 2, bd + k * 128, idesc, (kb | k) != 0);
       }
       umma_commit(&empty[s]);
     }
@@ -264,6 +277,16 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
 // ---------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------
+static int pj_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
+}
+
 template <int DI>
 static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void* X, const void* Wq, const void* Wk,
                                      void* q_idx, void* k_idx, int L, int hidden, cudaStream_t st) {
@@ -272,15 +295,20 @@ static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void
   if ((e = sp_make_tmap_bf16(&tmX, X, L, hidden, hidden, 128)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmWq, Wq, hidden, DI, DI, 64)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmWk, Wk, hidden, DI, DI, 64)) != cudaSuccess) return e;
-  constexpr size_t smem = (size_t)PJ_STAGES * (2 * 128 * 128 + (2 * DI / 64) * 8192) + 1024;
+  constexpr size_t s1 = (size_t)PJ_STAGES * (128 * 128 + (2 * DI / 64) * 8192);
+  constexpr size_t s2 = (size_t)(PJ_STAGES - 1) * (2 * 128 * 128 + (2 * DI / 64) * 8192);
+  constexpr size_t smem = (s1 > s2 ? s1 : s2) + 1024;
   static bool attr_done = false;
   if (!attr_done) {
     e = cudaFuncSetAttribute(sp_tc_project_kernel<DI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  sp_tc_project_kernel<DI><<<(L + PJ_M - 1) / PJ_M, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
-                                                               (__nv_bfloat16*)k_idx, L, hidden, g, flags);
+  // 256-token CTAs once the 128-token tiles no longer fit one wave; short inputs keep the finer grid
+  const int halves = (L + 127) / 128 > pj_sm_count() ? 2 : 1;
+  const int tile = 128 * halves;
+  sp_tc_project_kernel<DI><<<(L + tile - 1) / tile, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
+                                                               (__nv_bfloat16*)k_idx, L, hidden, g, flags, halves);
   sp_count_launch();
   return cudaGetLastError();
 }

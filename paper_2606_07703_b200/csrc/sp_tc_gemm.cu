@@ -304,8 +304,13 @@ static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  // 256-token CTAs once the 128-token tiles no longer fit one wave; short inputs keep the finer grid
-  const int halves = (L + 127) / 128 > pj_sm_count() ? 2 : 1;
+  // 128- or 256-token CTAs (one CTA per SM): whichever needs less time by waves x tile cost, a 256-token tile costing
+  // 1.45-1.85x a 128-token one (measured at 32K-128K tokens: the weights are read once per tile; 1.7 is used).
+  // Short inputs keep the finer grid.
+  const int sms = pj_sm_count();
+  const int t1 = (L + 127) / 128, t2 = (L + 255) / 256;
+  const double c1 = (double)((t1 + sms - 1) / sms), c2 = 1.7 * (double)((t2 + sms - 1) / sms);
+  const int halves = (t1 > sms && c2 <= c1) ? 2 : 1;
   const int tile = 128 * halves;
   sp_tc_project_kernel<DI><<<(L + tile - 1) / tile, 128, smem, st>>>(tmX, tmWq, tmWk, (__nv_bfloat16*)q_idx,
                                                                (__nv_bfloat16*)k_idx, L, hidden, g, flags, halves);

@@ -293,6 +293,53 @@ def prefill_layer(pb: Problem, mode: int, Q, K, V, X=None, Wqi=None, Wki=None,
     return LayerResult(rows, R, nv, idx, cnt, pos, out, q_idx, k_idx)
 
 
+# ---------------------------------------------------------------- per-KV-group support
+# ORACLE GROUNDWORK FOR SURVEY.md 8(f) f4: no CUDA path yet.  The paper names the variant -- one support
+# S_{l,t,r} shared by the query heads with g(h) = r (:100) -- and says it does not evaluate it (:133, :137);
+# the reading taken here (A29): the mass of group r is the mean over ITS G = Hq/Hkv query heads,
+# P_r[t,s] = (1/G) sum_{h: g(h)=r} A[t,h,s], everything else (block max, top-k, tie rule, recompute) as for the
+# head-averaged support.  That is literally the head-averaged definition applied to the sub-problem
+# (Q[:, rG:(r+1)G], K[:, r], V[:, r]) with Hq' = G, Hkv' = 1, which is how it is written out below.
+
+def _group_problem(pb: Problem) -> Problem:
+    G = pb.Hq // pb.Hkv
+    return Problem(L=pb.L, Hq=G, Hkv=1, d=pb.d, k=pb.k, b_sel=pb.b_sel, scale=pb.scale,
+                   local_window=pb.local_window, local_bias=pb.local_bias, cu_seqlens=pb.cu_seqlens)
+
+
+def _group_slices(pb: Problem, Q, K, V, r: int):
+    G = pb.Hq // pb.Hkv
+    Q = _u16(Q).reshape(pb.L, pb.Hq, pb.d)
+    K = _u16(K).reshape(pb.L, pb.Hkv, pb.d)
+    V = _u16(V).reshape(pb.L, pb.Hkv, pb.d) if V is not None else None
+    return (np.ascontiguousarray(Q[:, r * G:(r + 1) * G]), np.ascontiguousarray(K[:, r:r + 1]),
+            np.ascontiguousarray(V[:, r:r + 1]) if V is not None else None)
+
+
+def select_support_per_group(pb: Problem, Q, K, rows):
+    """Oracle-mode supports per KV group: idx [Hkv, len(rows), k], cnt [Hkv, len(rows)]."""
+    gp = _group_problem(pb)
+    idx, cnt = [], []
+    for r in range(pb.Hkv):
+        Qr, Kr, _ = _group_slices(pb, Q, K, None, r)
+        _, _, i, c = select_support(gp, MODE_ORACLE, Qr, Kr, rows)
+        idx.append(i)
+        cnt.append(c)
+    return np.stack(idx), np.stack(cnt)
+
+
+def sparse_attn_per_group(pb: Problem, Q, K, V, pos, sup):
+    """O6 with one support per KV group: sup [Hkv, len(pos), k]; head h attends S_{r(t), g(h)}."""
+    gp = _group_problem(pb)
+    G = pb.Hq // pb.Hkv
+    pos = _i32(pos)
+    out = np.empty((len(pos), pb.Hq, pb.d), dtype=np.float64)
+    for r in range(pb.Hkv):
+        Qr, Kr, Vr = _group_slices(pb, Q, K, V, r)
+        out[:, r * G:(r + 1) * G] = sparse_attn(gp, Qr, Kr, Vr, pos, sup[r])
+    return out
+
+
 # ---------------------------------------------------------------- support-level diagnostics (PAPER.md:262, :478)
 
 def support_overlap(idx_a, idx_b) -> np.ndarray:

@@ -517,3 +517,72 @@ def test_row_kl_pins():
     assert abs(orc.row_kl(oh, z[0:1], nv[:1])[0] + math.log(sm[0, 3])) < 1e-12
     Q = rng.random((4, 64)); Q[:, 40:] = 0; Q /= Q.sum(1, keepdims=True)
     assert np.all(orc.row_kl(Q, rng.standard_normal((4, 64)), np.full(4, 40)) >= 0)
+
+
+# ---------------------------------------------------------------- per-KV-group support (A29)
+# oracle groundwork for SURVEY.md 8(f) f4 -- there is no CUDA path for it yet
+
+def _group_bruteforce(pb, Q, K, V, b):
+    """Independent of oracle.py's slicing: dense [Hq, L, L] probabilities, mean over each group's heads."""
+    from scipy.special import softmax
+    G = pb.Hq // pb.Hkv
+    z = bf.logits(Q, K, 1.0 / math.sqrt(pb.d), G)                       # [Hq, L, L]
+    A = softmax(z, axis=-1)
+    P = A.reshape(pb.Hkv, G, pb.L, pb.L).mean(axis=1)                   # contiguous groups (A5)
+    idx = []
+    for r in range(pb.Hkv):
+        R, nv = bf.support_rows(P[r], b)
+        idx.append(bf.topk_rows(R, nv, pb.k))
+    idx = np.stack(idx)                                                 # [Hkv, rows, k]
+    v = np.repeat(bf.bf16_to_f64(V), G, axis=1)
+    out = np.zeros((pb.L, pb.Hq, pb.d))
+    for h in range(pb.Hq):
+        for t in range(pb.L):
+            s = idx[h // G, t // b]
+            s = s[(s >= 0) & (s <= t)]
+            if len(s):
+                out[t, h] = softmax(z[h, t, s]) @ v[s, h]
+    return idx, out
+
+
+@pytest.mark.parametrize("b", [1, 4])
+def test_per_group_support_matches_bruteforce(b):
+    pb, Q, K, V = small_problem(L=37, Hq=6, Hkv=3, d=8, k=5, b=b, seed=21)
+    rows = np.arange(orc.num_rows(pb))
+    idx, cnt = orc.select_support_per_group(pb, Q, K, rows)
+    want_idx, want_out = _group_bruteforce(pb, Q, K, V, b)
+    assert idx.shape == (3, len(rows), 5)
+    assert np.array_equal(idx, want_idx)
+    assert np.array_equal(cnt, (want_idx >= 0).sum(axis=-1))
+    pos = np.arange(pb.L)
+    sup = idx[:, pos // b, :]
+    out = orc.sparse_attn_per_group(pb, Q, K, V, pos, sup)
+    assert np.allclose(out, want_out, rtol=0, atol=1e-13)
+    # the groups must really differ on this input, or the test would not see a wrong group map
+    assert any(not np.array_equal(idx[0], idx[r]) for r in (1, 2))
+
+
+def test_per_group_reduces_to_head_averaged_support():
+    # one KV group: the group IS the head average (PAPER.md:100 third case)
+    pb, Q, K, V = small_problem(L=40, Hq=4, Hkv=1, d=8, k=6, b=4, seed=31)
+    rows = np.arange(orc.num_rows(pb))
+    shared = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    idx, cnt = orc.select_support_per_group(pb, Q, K, rows)
+    assert np.array_equal(idx[0], shared.idx) and np.array_equal(cnt[0], shared.cnt)
+    # identical groups: every group's mass equals the mean over all heads, so every list is the shared one
+    pb2 = orc.Problem(L=40, Hq=8, Hkv=2, d=8, k=6, b_sel=4)
+    Q2, K2, V2 = np.tile(Q, (1, 2, 1)), np.tile(K, (1, 2, 1)), np.tile(V, (1, 2, 1))
+    shared2 = orc.prefill_layer(pb2, orc.MODE_ORACLE, Q2, K2, V2)
+    idx2, _ = orc.select_support_per_group(pb2, Q2, K2, rows)
+    assert np.array_equal(idx2[0], shared2.idx) and np.array_equal(idx2[1], shared2.idx)
+    pos = shared2.pos
+    out2 = orc.sparse_attn_per_group(pb2, Q2, K2, V2, pos, idx2[:, pos // 4, :])
+    assert np.allclose(out2, shared2.out, rtol=0, atol=1e-14)
+
+
+def test_per_group_equals_dense_when_budget_covers_prefix():
+    pb, Q, K, V = small_problem(L=30, Hq=4, Hkv=2, d=8, k=30, seed=41)
+    pos = np.arange(30)
+    idx, _ = orc.select_support_per_group(pb, Q, K, pos)
+    out = orc.sparse_attn_per_group(pb, Q, K, V, pos, idx)
+    assert np.allclose(out, orc.dense_attn(pb, Q, K, V, pos), rtol=0, atol=1e-14)

@@ -87,7 +87,11 @@ typedef struct sp_params {
  *   SP_F_RELU   : z = max(idx_scale <q_idx, k_idx> + local term, 0)
  * KEY_LN and ROPE act in the projection (q_idx / k_idx come out transformed, rounded once to bf16; with
  * preprojected = 1 the caller's tensors are taken as already transformed); RELU acts in the score epilogue. */
-enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u };
+enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u, SP_F_GROUP_SUPPORT = 8u };
+/* SP_F_GROUP_SUPPORT ("shared within each KV group S_{l,t,r}"; A29) is read by
+ * sp_sparse_gqa_attn ONLY: idx is then [Hkv, n_rows, k] -- one support list per KV group and support row, each
+ * list as described under "idx" below -- and query head h attends the list of group g(h).  Every other entry
+ * point returns SP_ERR_UNSUPPORTED when the bit is set (per-group selection has no CUDA path yet). */
 
 /* Number of support rows of the whole pack (host arithmetic only). Returns < 0 on invalid params. */
 int64_t sp_num_rows(const sp_params *p);

@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libsp.so")
 SP_OK, SP_ERR_INVALID_ARG, SP_ERR_UNSUPPORTED, SP_ERR_WORKSPACE, SP_ERR_CUDA = 0, -1, -2, -3, -4
 SP_MODE_ORACLE, SP_MODE_INDEXER = 0, 1
 SP_F_RELU, SP_F_KEY_LN, SP_F_ROPE = 1, 2, 4   # sp_params.flags: the served scorer of PAPER.md:270-274
+SP_F_GROUP_SUPPORT = 8                        # sp_sparse_gqa_attn only: idx is [Hkv, n_rows, k]
 (SP_STAGE_INDEXER_SCORES, SP_STAGE_ORACLE_MASS, SP_STAGE_TOPK, SP_STAGE_SPARSE_ATTN, SP_STAGE_DENSE_ATTN,
  SP_STAGE_LAYER_ORACLE, SP_STAGE_LAYER_INDEXER) = range(7)
 
@@ -188,6 +189,9 @@ def sp_topk_support(pb: Problem, scores: torch.Tensor, row_begin: int, row_count
 def sp_sparse_gqa_attn(pb: Problem, Q, K, V, idx, O, lse: Optional[torch.Tensor] = None,
                        ws: Optional[torch.Tensor] = None):
     p = pb.c()
+    if idx.dim() == 3:   # one support list per KV group: [Hkv, n_rows, k]
+        assert idx.shape[0] == pb.Hkv and idx.is_contiguous(), idx.shape
+        p.flags |= SP_F_GROUP_SUPPORT
     wp, wb = _ws_args(ws)
     _check(lib().sp_sparse_gqa_attn(C.byref(p), _ptr(Q), _ptr(K), _ptr(V), _ptr(idx), _ptr(O), _ptr(lse), wp, wb,
                                     _stream()))

@@ -109,7 +109,7 @@ int validate_common(const sp_params* p, bool need_attn, bool need_indexer) {
 HostGeom host_geom(const sp_params* p) {
   return HostGeom{p->batch, p->L, p->b_sel, p->cu_seqlens ? p->cu_seqlens_host : nullptr};
 }
-SpGeom dev_geom(const sp_params* p) { return SpGeom{p->batch, p->L, p->cu_seqlens, p->b_sel}; }
+SpGeom dev_geom(const sp_params* p) { return SpGeom{p->batch, p->L, p->cu_seqlens, p->b_sel, 0}; }
 float attn_scale(const sp_params* p) { return p->scale != 0.f ? p->scale : 1.0f / sqrtf((float)p->d); }
 float index_scale(const sp_params* p) { return p->idx_scale != 0.f ? p->idx_scale : 1.0f / sqrtf((float)p->d_idx); }
 
@@ -155,8 +155,9 @@ cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const flo
 // the oracle's pass 1 of a row panel) -- the query chunks that intersect [q_begin, q_begin + q_count): rows of a
 // boundary chunk outside the range get their lse too, which is harmless.
 cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
-                     int q_count, void* O, float* lse, cudaStream_t st) {
-  const SpGeom g = dev_geom(p);
+                     int q_count, void* O, float* lse, cudaStream_t st, long long idx_grp = 0) {
+  SpGeom g = dev_geom(p);
+  g.idx_grp = idx_grp;
   const int G = p->Hq / p->Hkv;
   const bool whole = q_begin == 0 && q_count == p->L;
   const bool dense_lse_range = idx == nullptr && O == nullptr && q_count > 0;
@@ -368,11 +369,15 @@ int sp_row_kl(const sp_params* p, const float* mass, int64_t ld_mass, const floa
 
 int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
                        float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
-  const int rc = validate_common(p, true, false);
+  if (!p) return SP_ERR_INVALID_ARG;
+  sp_params q = *p;  // SP_F_GROUP_SUPPORT belongs to this entry point only: every other one rejects it as unknown
+  q.flags &= ~(uint32_t)SP_F_GROUP_SUPPORT;
+  const int rc = validate_common(&q, true, false);
   if (rc != SP_OK) return rc;
   if (!Q || !K || !V || !idx || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
     return SP_ERR_INVALID_ARG;
-  SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, lse, (cudaStream_t)stream), "sparse attention");
+  const long long idx_grp = (p->flags & SP_F_GROUP_SUPPORT) ? host_geom(&q).num_rows() * (long long)q.k : 0;
+  SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp), "sparse attention");
   return SP_OK;
 }
 

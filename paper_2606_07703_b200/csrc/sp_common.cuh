@@ -16,6 +16,7 @@ struct SpGeom {
   int L;
   const int* cu;  // device cu_seqlens or nullptr
   int b_sel;
+  long long idx_grp;  // SP_F_GROUP_SUPPORT: elements between two KV groups' index lists ([Hkv, n_rows, k]); 0 = one shared list
 };
 
 struct SpRow {

@@ -84,7 +84,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   float o[NT][4];
 #pragma unroll
   for (int n = 0; n < NT; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
-  const int32_t* sup = idx + (size_t)pi.row * k;
+  const int32_t* sup = idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)pi.row * k;
 
   for (int c0 = 0; c0 < k; c0 += PQ_KEYS) {
     // ---- this lane's key of the tile ----

@@ -297,7 +297,7 @@ sp_attn_warp_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bf
     for (int e = 0; e < EPL; ++e) o[h][e] = 0.f;
   }
   const int n_keys = SPARSE ? k : (t - pi.seq_start + 1);
-  const int32_t* sup = SPARSE ? idx + (size_t)pi.row * k : nullptr;
+  const int32_t* sup = SPARSE ? idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)pi.row * k : nullptr;
 
   for (int c0 = 0; c0 < n_keys; c0 += 32) {
     int sp = -1;  // packed key position of this lane, -1 = none

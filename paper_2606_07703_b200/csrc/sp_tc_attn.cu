@@ -270,7 +270,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       for (int t = ptid; t < ntmax; t += 128) fl[t] = 0u;
       if (ptid == 0) n_eff_sh[ib] = 0;
       loader_bar_sync();
-      const int32_t* sup = idx + (size_t)its.row * k;
+      const int32_t* sup = idx + (size_t)its.kvh * (size_t)g.idx_grp + (size_t)its.row * k;
       const int qa0 = its.seq_start + its.t0, qa1 = qa0 + 128 / G, plast = its.seq_start + its.t1;
       int my_last = 0;
       for (int e0 = ptid; e0 < kpad; e0 += 128 * 8) {  // 8 independent loads in flight per thread

@@ -60,7 +60,8 @@ def test_num_rows_and_workspace_are_host_arithmetic(lib):
     (dict(Hq=6, Hkv=4), B.SP_ERR_INVALID_ARG),
     (dict(d=96), B.SP_ERR_UNSUPPORTED),
     (dict(Hq=32, Hkv=2), B.SP_ERR_UNSUPPORTED),
-    (dict(flags=8), B.SP_ERR_UNSUPPORTED),               # unknown flag bit
+    (dict(flags=8), B.SP_ERR_UNSUPPORTED),               # SP_F_GROUP_SUPPORT belongs to sp_sparse_gqa_attn alone
+    (dict(flags=16), B.SP_ERR_UNSUPPORTED),              # unknown flag bit
     (dict(flags=1, b_sel=16), B.SP_ERR_UNSUPPORTED),     # served-scorer flags need a tcgen05 score path
     (dict(d_idx=32), B.SP_ERR_UNSUPPORTED),
     (dict(hidden=100), B.SP_ERR_UNSUPPORTED),

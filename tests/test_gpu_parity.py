@@ -350,6 +350,32 @@ def test_sparse_attention_on_oracle_support(cfg, b, k):
     assert np.allclose(got[fin], lse_o[fin], rtol=0, atol=2e-5)
 
 
+@pytest.mark.parametrize("cfg,b,k", [(SMALL_ORC, 1, 96), (SMALL_ORC, 64, 96), (SMALL_ORC128, 128, 200),
+                                     (SMALL_ORC128, 1, 40)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_sparse_attention_on_per_group_oracle_supports(cfg, b, k):
+    """SP_F_GROUP_SUPPORT (PAPER.md:100, DESIGN.md A29): one ORACLE support list per KV group, idx [Hkv, rows, k];
+    every attention path (tcgen05 block-shared, mma.sync per-query) must read the list of the head's own group."""
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(b_sel=b, k=k, local_window=12, local_bias=-0.5)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    rows = np.arange(orc.num_rows(pbo))
+    idx_o, _ = orc.select_support_per_group(pbo, inp["Q"], inp["K"], rows)
+    assert any(not np.array_equal(idx_o[0], idx_o[r]) for r in range(1, cfg.Hkv))   # the groups really differ
+    pos = np.arange(cfg.L)
+    row_of = np.array([orc.row_of_pos(pbo, int(t)) for t in pos])
+    want = orc.sparse_attn_per_group(pbo, inp["Q"], inp["K"], inp["V"], pos, idx_o[:, row_of, :])
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    idx = torch.from_numpy(np.ascontiguousarray(idx_o)).to(DEV)
+    B.sp_sparse_gqa_attn(pbg, dev(inp["Q"]), dev(inp["K"]), dev(inp["V"]), idx, O)
+    parity.compare_attention(to_f64(O), want)
+    # and the flag is this entry point's alone
+    with pytest.raises(B.SpError) as ei:
+        B.workspace_bytes(B.Problem.from_config(cfg, flags=B.SP_F_GROUP_SUPPORT, **over), B.SP_STAGE_LAYER_ORACLE)
+    assert ei.value.code == B.SP_ERR_UNSUPPORTED
+
+
 @pytest.mark.parametrize("cfg", [SMALL_ORC, SMALL_ORC128], ids=lambda c: c.name)
 def test_dense_attention_matches_oracle(cfg):
     inp = gen.make_inputs(cfg, with_indexer=False)

@@ -124,6 +124,17 @@ int sp_oracle_mass(const sp_params *p, const void *Q, const void *K, float *lse,
                    int32_t row_begin, int32_t row_count, float *mass, int64_t ld_mass,
                    void *ws, size_t ws_bytes, void *stream);
 
+/* The same for ONE KV group ("shared within each KV group S_{l,t,r}"; A29): pass 2
+ * averages over the G = Hq/Hkv query heads h with g(h) = group only, P_r[t,s] = (1/G) sum_{g(h)=r} A[t,h,s].
+ * Every other argument as for sp_oracle_mass; lse is still the [L,Hq] array of ALL heads, so one pass 1
+ * (lse_ready == 0 on the first group) serves the Hkv calls.  Followed by sp_topk_support on the panel this
+ * gives group r's list, and Hkv such lists, stacked as idx [Hkv, n_rows, k], are what sp_sparse_gqa_attn
+ * reads under SP_F_GROUP_SUPPORT.  group outside [0,Hkv) -> SP_ERR_INVALID_ARG; shapes outside the tcgen05
+ * mass kernel's set (b_sel in {1,32,64,128}, d in {64,128}) -> SP_ERR_UNSUPPORTED. */
+int sp_oracle_mass_group(const sp_params *p, const void *Q, const void *K, float *lse, int32_t lse_ready,
+                         int32_t group, int32_t row_begin, int32_t row_count, float *mass, int64_t ld_mass,
+                         void *ws, size_t ws_bytes, void *stream);
+
 /* Causal top-k of each support row of the panel (PAPER.md:127 TopK_s(P,k); :145 sentinel padding; :156
  * causally invalid positions masked before selection).  Row r ranks columns [0, n_valid(r)) of
  * scores[r - row_begin, :]; the kept set is the first min(k, n_valid) elements of the order

@@ -28,6 +28,7 @@ EXPORTS = (
     "sp_num_rows", "sp_workspace_bytes", "sp_indexer_scores", "sp_oracle_mass", "sp_topk_support",
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
     "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
+    "sp_oracle_mass_group",
 )
 
 
@@ -176,6 +177,15 @@ def sp_oracle_mass(pb: Problem, Q, K, lse: Optional[torch.Tensor], lse_ready: bo
     _check(lib().sp_oracle_mass(C.byref(p), _ptr(Q), _ptr(K), _ptr(lse), C.c_int32(1 if lse_ready else 0),
                                 C.c_int32(row_begin), C.c_int32(row_count), _ptr(mass), C.c_int64(mass.stride(0)),
                                 wp, wb, _stream()))
+
+
+def sp_oracle_mass_group(pb: Problem, Q, K, lse: Optional[torch.Tensor], lse_ready: bool, group: int, row_begin: int,
+                         row_count: int, mass: torch.Tensor, ws: Optional[torch.Tensor] = None):
+    p = pb.c()
+    wp, wb = _ws_args(ws)
+    _check(lib().sp_oracle_mass_group(C.byref(p), _ptr(Q), _ptr(K), _ptr(lse), C.c_int32(1 if lse_ready else 0),
+                                      C.c_int32(group), C.c_int32(row_begin), C.c_int32(row_count), _ptr(mass),
+                                      C.c_int64(mass.stride(0)), wp, wb, _stream()))
 
 
 def sp_topk_support(pb: Problem, scores: torch.Tensor, row_begin: int, row_count: int, idx: torch.Tensor,

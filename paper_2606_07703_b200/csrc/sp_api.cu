@@ -142,11 +142,12 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
 }
 
 cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const float* lse, int row_begin, int row_count,
-                     int max_nv, float* mass, int64_t ld, cudaStream_t st) {
+                     int max_nv, float* mass, int64_t ld, cudaStream_t st, int grp = -1) {
   const SpGeom g = dev_geom(p);
-  if (sp_tc_mass_supported(p->b_sel, p->d) && !(debug_simt() & 8))
+  if (sp_tc_mass_supported(p->b_sel, p->d) && (grp >= 0 || !(debug_simt() & 8)))
     return sp_launch_mass_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, Q, K, lse, p->Hq, p->Hkv, p->d,
-                             attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st);
+                             attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st, grp);
+  if (grp >= 0) return cudaErrorNotSupported;  // callers check sp_tc_mass_supported first
   return sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
                         row_count, max_nv, mass, ld, st);
 }
@@ -289,10 +290,13 @@ int sp_indexer_scores(const sp_params* p, const void* X, const void* Wqi, const 
   return SP_OK;
 }
 
-int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t row_begin,
-                   int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes, void* stream) {
+static int oracle_mass_impl(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int grp,
+                            int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws,
+                            size_t ws_bytes, void* stream) {
   int rc = validate_common(p, true, false);
   if (rc != SP_OK) return rc;
+  if (grp >= p->Hkv) return SP_ERR_INVALID_ARG;
+  if (grp >= 0 && !sp_tc_mass_supported(p->b_sel, p->d)) return SP_ERR_UNSUPPORTED;
   if (!Q || !K || !mass || !aligned16(Q) || !aligned16(K) || !aligned16(mass)) return SP_ERR_INVALID_ARG;
   if (lse_ready && !lse) return SP_ERR_INVALID_ARG;
   int max_nv = 0;
@@ -327,8 +331,20 @@ int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse,
     }
     SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, q_lo, q_hi - q_lo + 1, nullptr, lse, st), "mass pass 1 (lse)");
   }
-  SP_CUDA(run_mass(p, Q, K, lse, row_begin, row_count, max_nv, mass, ld_mass, st), "mass pass 2");
+  SP_CUDA(run_mass(p, Q, K, lse, row_begin, row_count, max_nv, mass, ld_mass, st, grp), "mass pass 2");
   return SP_OK;
+}
+
+int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t row_begin,
+                   int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes, void* stream) {
+  return oracle_mass_impl(p, Q, K, lse, lse_ready, -1, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
+}
+
+int sp_oracle_mass_group(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t group,
+                         int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes,
+                         void* stream) {
+  if (group < 0) return SP_ERR_INVALID_ARG;
+  return oracle_mass_impl(p, Q, K, lse, lse_ready, group, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
 }
 
 int sp_topk_support(const sp_params* p, const float* scores, int64_t ld_scores, int32_t row_begin, int32_t row_count,

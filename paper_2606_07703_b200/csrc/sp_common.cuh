@@ -119,7 +119,7 @@ cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host,
 bool sp_tc_mass_supported(int b_sel, int d);
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
-                              int row_count, float* mass, int64_t ld, cudaStream_t st);
+                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp = -1);  // grp >= 0: that KV group's heads only
 
 bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d);
 cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, long long chunk_base,

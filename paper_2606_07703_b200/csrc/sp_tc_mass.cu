@@ -131,7 +131,8 @@ struct MsBarriers {
 template <int D>
 __global__ void __launch_bounds__(MS_THREADS, 1)
 sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK, SpGeom g,
-                  const float* __restrict__ lse, int Hq, int Hkv, float scale, int local_window, float local_bias,
+                  const float* __restrict__ lse, int lse_stride, int Hq, int Hkv, float scale, int local_window,
+                  float local_bias,
                   int row_begin, int row_count, int qt_begin, int qt_count, float* __restrict__ mass, int64_t ld) {
   constexpr int KB = D / 64;
   constexpr uint32_t A_BYTES = MS_MQ * 128;  // per 64-wide K block: 128 queries
@@ -279,7 +280,7 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const bool t_ok = tl < ti.n;
       const int tw0 = ti.q0 + wq * 32;               // warp-uniform: first / last valid query of the warp
       const int tw1 = min(tw0 + 31, ti.n - 1);
-      const float* lse_row = lse + (size_t)(ti.seq_start + min(tl, ti.n - 1)) * Hq;
+      const float* lse_row = lse + (size_t)(ti.seq_start + min(tl, ti.n - 1)) * lse_stride;
       for (int kt = kt_lo; kt < kt_hi; ++kt) {
         const int sc0 = kt * MS_NK + e * 128;  // local key of this warpgroup's column 0
         uint64_t acc[64];
@@ -414,13 +415,24 @@ int ms_sm_count() {
 }
 
 template <int D>
-cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, float scale,
-                           int lw, float lb, int row_begin, int row_count, int qt_begin, int qt_count, long long items,
-                           float* mass, int64_t ld, cudaStream_t st) {
+cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, int grp,
+                           float scale, int lw, float lb, int row_begin, int row_count, int qt_begin, int qt_count,
+                           long long items, float* mass, int64_t ld, cudaStream_t st) {
   CUtensorMap tmQ, tmK;
   cudaError_t e;
-  if ((e = sp_make_tmap_bf16(&tmQ, Q, g.L, (uint64_t)Hq * D, (uint64_t)Hq * D, MS_MQ)) != cudaSuccess) return e;
-  if ((e = sp_make_tmap_bf16(&tmK, K, g.L, (uint64_t)Hkv * D, (uint64_t)Hkv * D, MS_NK)) != cudaSuccess) return e;
+  // grp >= 0 (per-KV-group mass): the kernel sees the sub-problem of that group -- G heads over one KV
+  // head -- through offset base pointers; the row pitches of Q, K and lse stay those of the full tensors.
+  const int lse_stride = Hq, G = Hq / Hkv;
+  const uint64_t q_pitch = (uint64_t)Hq * D, k_pitch = (uint64_t)Hkv * D;
+  if (grp >= 0) {
+    Q = (const __nv_bfloat16*)Q + (size_t)grp * G * D;
+    K = (const __nv_bfloat16*)K + (size_t)grp * D;
+    lse += (size_t)grp * G;
+    Hq = G;
+    Hkv = 1;
+  }
+  if ((e = sp_make_tmap_bf16(&tmQ, Q, g.L, (uint64_t)Hq * D, q_pitch, MS_MQ)) != cudaSuccess) return e;
+  if ((e = sp_make_tmap_bf16(&tmK, K, g.L, (uint64_t)Hkv * D, k_pitch, MS_NK)) != cudaSuccess) return e;
   constexpr size_t smem = (size_t)(D / 64) * (MS_QSTAGES * MS_MQ * 128 + 2 * MS_NK * 128) + 1024;
   static bool attr_done = false;
   if (!attr_done) {
@@ -430,7 +442,8 @@ cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const 
   }
   long long grid = items < ms_sm_count() ? items : ms_sm_count();
   if (grid < 1) grid = 1;
-  sp_tc_mass_kernel<D><<<(unsigned)grid, MS_THREADS, smem, st>>>(tmQ, tmK, g, lse, Hq, Hkv, scale, lw, lb, row_begin,
+  sp_tc_mass_kernel<D><<<(unsigned)grid, MS_THREADS, smem, st>>>(tmQ, tmK, g, lse, lse_stride, Hq, Hkv, scale, lw, lb,
+                                                                row_begin,
                                                                 row_count, qt_begin, qt_count, mass, ld);
   sp_count_launch();
   return cudaGetLastError();
@@ -445,7 +458,7 @@ bool sp_tc_mass_supported(int b_sel, int d) {
 // cu_host: HOST copy of cu_seqlens (nullptr = one sequence).
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
-                              int row_count, float* mass, int64_t ld, cudaStream_t st) {
+                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp) {
   if (row_count <= 0) return cudaSuccess;
   // 128-query tiles (per sequence) that intersect the support-row panel [row_begin, row_begin + row_count)
   const int b = g.b_sel;
@@ -473,8 +486,8 @@ cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const voi
   }
   if (qlo < 0) return cudaSuccess;
   const int cnt = (int)(qhi - qlo + 1);
-  return d == 128 ? launch_mass_tc<128>(g, Q, K, lse, Hq, Hkv, scale, local_window, local_bias, row_begin, row_count,
-                                        (int)qlo, cnt, items, mass, ld, st)
-                  : launch_mass_tc<64>(g, Q, K, lse, Hq, Hkv, scale, local_window, local_bias, row_begin, row_count,
-                                       (int)qlo, cnt, items, mass, ld, st);
+  return d == 128 ? launch_mass_tc<128>(g, Q, K, lse, Hq, Hkv, grp, scale, local_window, local_bias, row_begin,
+                                        row_count, (int)qlo, cnt, items, mass, ld, st)
+                  : launch_mass_tc<64>(g, Q, K, lse, Hq, Hkv, grp, scale, local_window, local_bias, row_begin,
+                                       row_count, (int)qlo, cnt, items, mass, ld, st);
 }

@@ -280,6 +280,88 @@ def run_c4_sweep(args, B, torch, gen, peaks):
     print(json.dumps(line))
 
 
+def run_c3_groups(args, B, torch, gen, peaks):
+    """SURVEY.md 8(f) f4 at the c3 shape, ORACLE mode (per-KV-group selection is defined on attention mass only,
+    PAPER.md:100, A29): the head-averaged layer (sp_prefill_layer, SP_MODE_ORACLE) beside the per-group
+    chain of stage calls -- pass 1 (dense LSE) once, then per KV group sp_oracle_mass_group + sp_topk_support, then
+    sp_sparse_gqa_attn under SP_F_GROUP_SUPPORT.  CUDA events on the current stream, device-resident inputs."""
+    stream = torch.cuda.current_stream()
+    cfg = gen.C3
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    dv = {n: B.bf16_tensor(inp[n]) for n in ("Q", "K", "V")}
+    pb = B.Problem.from_config(cfg)
+    L, k, n_rows, Hkv = cfg.L, cfg.k, pb.num_rows, cfg.Hkv
+
+    def timed(fn, reps, warm=3):
+        for _ in range(warm):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    reps = max(1, args.steps)
+    l0 = B.launch_count()
+    O = torch.empty(L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+    idx_s = torch.empty(n_rows, k, dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(pb, B.SP_STAGE_LAYER_ORACLE)
+    t_shared = timed(lambda: B.sp_prefill_layer(pb, B.SP_MODE_ORACLE, None, None, None, dv["Q"], dv["K"], dv["V"], O,
+                                                idx_s, ws), reps)
+    ld = (L + 3) // 4 * 4
+    mass = torch.empty(n_rows, ld, dtype=torch.float32, device="cuda")
+    lse = torch.empty(L, cfg.Hq, dtype=torch.float32, device="cuda")
+    idx_g = torch.empty(Hkv, n_rows, k, dtype=torch.int32, device="cuda")
+
+    def chain():
+        B.sp_dense_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], None, lse)
+        for r in range(Hkv):
+            B.sp_oracle_mass_group(pb, dv["Q"], dv["K"], lse, True, r, 0, n_rows, mass)
+            B.sp_topk_support(pb, mass, 0, n_rows, idx_g[r])
+        B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_g, O)
+
+    t_chain = timed(chain, reps)
+    t_p1 = timed(lambda: B.sp_dense_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], None, lse), reps)
+    t_ma = timed(lambda: B.sp_oracle_mass(pb, dv["Q"], dv["K"], lse, True, 0, n_rows, mass), reps)
+    t_mg = timed(lambda: B.sp_oracle_mass_group(pb, dv["Q"], dv["K"], lse, True, Hkv // 2, 0, n_rows, mass), reps)
+    idx_scratch = torch.empty_like(idx_s)   # the stage timings below must not touch the chain's idx_g
+    t_tk = timed(lambda: B.sp_topk_support(pb, mass, 0, n_rows, idx_scratch), reps)
+    t_ag = timed(lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_g, O), reps)
+    t_as = timed(lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_s, O), reps)
+    inter = torch.empty(n_rows, dtype=torch.int32, device="cuda")
+    agree = []
+    for r in range(Hkv):   # how much of the head-averaged support each group's own support keeps
+        B.sp_support_overlap(pb, idx_s, idx_g[r], inter)
+        agree.append(float(inter.sum().item()) / float((idx_s >= 0).sum().item()))
+    mass_flops = 2.0 * cfg.d * cfg.Hq * (L * (L + 1) // 2)
+    attn_flops = 4.0 * cfg.d * cfg.Hq * sum(min(k, min(L, (j + 1) * cfg.b_sel)) * min(cfg.b_sel, L - j * cfg.b_sel)
+                                            for j in range(n_rows))
+    line = {"metric": METRIC, "value": L / (t_chain * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": reps, "warmup": 3,
+            "ms_per_step": t_chain, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": "c3 shape, ORACLE mode, one support per KV group (SURVEY.md 8(f) f4) as stage calls",
+                       "L": L, "Hq": cfg.Hq, "Hkv": Hkv, "d": cfg.d, "k": k, "b_sel": cfg.b_sel,
+                       "parallelism": "replicas only (no sharding, no collectives)",
+                       "l2": "no flush: Q+K+V and the 67 MB mass panel exceed the 126 MB L2"},
+            "gpu_launches": int(B.launch_count() - l0),
+            "head_averaged_oracle_layer_ms": t_shared,
+            "stages_ms": {"mass_pass1_lse": t_p1, "mass_pass2_one_group": t_mg, "mass_pass2_all_heads": t_ma,
+                          "topk_one_group": t_tk, "sparse_attention_group_lists": t_ag,
+                          "sparse_attention_shared_list": t_as},
+            "mass_pass2_TFLOPs": {"all_groups_as_8_calls": mass_flops / (Hkv * t_mg * 1e-3) / 1e12,
+                                  "all_heads_one_call": mass_flops / (t_ma * 1e-3) / 1e12},
+            "sparse_attention_TFLOPs": {"group_lists": attn_flops / (t_ag * 1e-3) / 1e12,
+                                        "shared_list": attn_flops / (t_as * 1e-3) / 1e12},
+            "overlap_of_head_averaged_support_with_each_group": agree,
+            "roofline": {"bound": "tensor", "achieved": attn_flops / (t_ag * 1e-3) / 1e12, "peak": peaks["tensor"],
+                         "unit": "TFLOP/s", "frac": attn_flops / (t_ag * 1e-3) / 1e12 / peaks["tensor"], "traffic": None,
+                         "kernel": "sparse_attention (group lists)", "peak_source": peaks["source"]}}
+    print(json.dumps(line))
+
+
 def measure_layer_only(cfg, B, torch, gen, steps):
     """Layer latency of another workload (device-resident inputs, CUDA events, 3 warm-up steps) next to the dense
     GQA layer of the same library on the same tensors."""
@@ -328,6 +410,12 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
     from paper_2606_07703_b200 import inputs as gen
+    if args.workload == "c3-groups" and args.impl != "reference":
+        import torch
+        from paper_2606_07703_b200 import binding as B
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        B.lib()
+        return run_c3_groups(args, B, torch, gen, load_peaks())
     if args.workload == "c4" and args.impl != "reference":
         import torch
         from paper_2606_07703_b200 import binding as B

@@ -96,6 +96,9 @@ __device__ __forceinline__ float ex2_approx(float x) {
 #ifndef AT_POLY_EVERY
 #define AT_POLY_EVERY 8  // one pair in AT_POLY_EVERY takes the polynomial path (0 = never)
 #endif
+#ifndef AT_SPEC
+#define AT_SPEC 1  // 1 = exponentials against the PREVIOUS running max, tile max reduced beside them (see the softmax role)
+#endif
 __device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
   float x0, x1;
   f2_unpack(x2, x0, x1);
@@ -537,6 +540,136 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
 
       if (mt < n_mt && my_nt > 0) {
         float m_run = -INFINITY, l_run = 0.f;
+#if AT_SPEC
+        // SPECULATIVE OFFSET: the exponentials of tile j are taken against the running max as it stood BEFORE the tile,
+        // while the tile's own max is reduced beside them (independent instruction chains: FMNMX3 on the ALU pipe under
+        // the MUFU / FMA work), so the row max is off the critical path of the softmax warps.  Only when the tile's max
+        // exceeds the running max by more than the lazy-rescale threshold (always on the first finite tile of a row) is
+        // the running max moved, O rescaled, S re-read from TMEM (P has not been stored over it yet) and the tile
+        // redone: at most once per tile, p <= 2^AT_RESCALE_THRESHOLD otherwise, exactly as with the max taken first.
+        for (int j = 0; j < my_nt; ++j, ++cs) {
+          const uint32_t b = cs & 1;
+          const uint32_t t_s = t_s0 + b * 64;
+          mbar_wait_addr(a_sfull + b * 8, (cs >> 1) & 1);
+          tc_fence_after_sync();
+          bool flagged;
+          if (SPARSE) flagged = ((fl[j] >> mt) & 1u) != 0;
+          else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
+          flagged = flagged || !scale_pos;
+          uint32_t pk[AT_KT / 2];
+          float tsum;
+          if (j == 0 && !flagged) {  // first tile: its max IS the running max (saves the certain second pass)
+            uint32_t v[AT_KT];
+            tmem_ld_x32(t_s, v);
+            tmem_ld_x32(t_s + 32, v + 32);
+            tmem_ld_wait();
+            float a0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1]));
+            float a1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
+#pragma unroll
+            for (int cc = 4; cc < AT_KT; cc += 4) {
+              a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
+              a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
+            }
+            m_run = fmaxf(a0, a1) * sl2;
+          }
+#pragma unroll 1
+          for (;;) {
+            uint32_t v[AT_KT];
+            tmem_ld_x32(t_s, v);
+            tmem_ld_x32(t_s + 32, v + 32);
+            tmem_ld_wait();
+            const float m_off = (m_run == -INFINITY) ? 0.f : m_run;
+            uint64_t sum2 = 0ull;
+            float mx;
+            if (!flagged) {
+              const uint64_t nm2 = f2_pack(-m_off, -m_off);
+              float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
+#pragma unroll
+              for (int cc = 0; cc < AT_KT; cc += 8) {
+                a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
+                a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
+                a2 = fmaxf(a2, fmaxf(__uint_as_float(v[cc + 4]), __uint_as_float(v[cc + 5])));
+                a3 = fmaxf(a3, fmaxf(__uint_as_float(v[cc + 6]), __uint_as_float(v[cc + 7])));
+#pragma unroll
+                for (int c2 = cc; c2 < cc + 8; c2 += 2) {
+                  const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[c2]), __uint_as_float(v[c2 + 1])), sl2_2, nm2);
+                  float p0, p1;
+                  if (WITH_O && AT_POLY_EVERY > 0 && (c2 / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
+                    ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
+                  } else {
+                    float x0, x1;
+                    f2_unpack(x2, x0, x1);
+                    p0 = ex2_approx(x0);
+                    p1 = ex2_approx(x1);
+                  }
+                  sum2 = f2_add(sum2, f2_pack(p0, p1));
+                  pk[c2 / 2] = bf16x2_rn(p0, p1);
+                }
+              }
+              mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
+            } else {
+              mx = -INFINITY;
+#pragma unroll
+              for (int cc = 0; cc < AT_KT; cc += 2) {
+                float x[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                  const int col = j * AT_KT + cc + u;
+                  bool ok;
+                  int dist;
+                  if (SPARSE) {
+                    const int p = si[col];
+                    ok = p >= 0 && p <= tp;
+                    dist = tp - p;
+                  } else {
+                    ok = col <= tl;
+                    dist = tl - col;
+                  }
+                  x[u] = ok ? fmaf(__uint_as_float(v[cc + u]), sl2, (win > 0 && dist < win) ? lb2 : 0.f) : -INFINITY;
+                }
+                mx = fmaxf(mx, fmaxf(x[0], x[1]));
+                const float p0 = ex2_approx(x[0] - m_off);
+                const float p1 = ex2_approx(x[1] - m_off);
+                sum2 = f2_add(sum2, f2_pack(p0, p1));
+                pk[cc / 2] = bf16x2_rn(p0, p1);
+              }
+            }
+            // ---- running max with lazy rescale of the TMEM accumulator ----
+            const float m_new = fmaxf(m_run, mx);
+            const bool need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
+            if (!__any_sync(0xffffffffu, need)) {
+              float s0, s1;
+              f2_unpack(sum2, s0, s1);
+              tsum = s0 + s1;
+              break;
+            }
+            const float f = need ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
+            if (WITH_O && j > 0) {
+              mbar_wait(&bar.ofull[mt], (cs - 1) & 1);  // PV(j-1) has finished updating O
+              tc_fence_after_sync();
+#pragma unroll
+              for (int c0 = 0; c0 < D; c0 += 32) {
+                uint32_t o[32];
+                tmem_ld_x32(t_o + c0, o);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 32; ++q) o[q] = __float_as_uint(__uint_as_float(o[q]) * f);
+                tmem_st_x32(t_o + c0, o);
+              }
+              tmem_st_wait();
+            }
+            l_run *= f;
+            if (need) m_run = m_new;
+          }
+          l_run += tsum;
+          if (WITH_O) {
+            tmem_st_x32(t_s, pk);  // P (64 keys as 32 bf16x2 columns) over the first half of S
+            tmem_st_wait();
+          }
+          tc_fence_before_sync();
+          mbar_arrive_addr(a_sdone + b * 8);
+        }
+#else
         for (int j = 0; j < my_nt; ++j, ++cs) {
           const uint32_t b = cs & 1;
           const uint32_t t_s = t_s0 + b * 64;
@@ -650,6 +783,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           tc_fence_before_sync();
           mbar_arrive_addr(a_sdone + b * 8);
         }
+#endif
         // ---- epilogue ----
         if (WITH_O) {
           mbar_wait(&bar.ofin[mt], n_ep & 1);

@@ -1,7 +1,9 @@
 """GPU parity tests proper: the CUDA path (through the C ABI, via the thin binding) against the fp64
 CPU oracle on the same seeded inputs.  Stage-isolated tests feed ORACLE-produced inputs to one GPU
 stage; chained tests run sp_prefill_layer end to end.  Rules and tolerances: tests/parity.py."""
+import json
 import math
+import os
 
 import numpy as np
 import pytest
@@ -14,6 +16,34 @@ from paper_2606_07703_b200 import inputs as gen
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
+
+# chained parity: at least this fraction of the sampled support rows BEYOND the budget must carry the oracle's exact
+# index list (rows with near-tied k-th scores may swap keys within the overlap rule; measured fractions are recorded
+# by record_stats and kept under profiles/)
+CHAINED_IDENTICAL_FLOOR = 0.5
+# fraction of projected bf16 elements allowed to differ (by one ulp) from the oracle's fp64-sum rounding; set from the
+# measured rates
+PROJ_MISMATCH_RATE = 5e-3
+PROJ_SERVED_MISMATCH_RATE = 1e-2
+STATS_PATH = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out", "parity_stats.json")
+_STATS = {}
+
+
+def record_stats(name, stats):
+    """What each chained / projection test actually compared, dumped for profiles/ (one JSON object per test)."""
+    def plain(v):
+        if isinstance(v, dict):
+            return {k: plain(x) for k, x in v.items()}
+        if isinstance(v, (np.floating, np.integer)):
+            return v.item()
+        return v
+    _STATS[name] = plain(stats)
+    try:
+        os.makedirs(os.path.dirname(STATS_PATH), exist_ok=True)
+        with open(STATS_PATH, "w") as f:
+            json.dump(_STATS, f, indent=1, sort_keys=True)
+    except OSError:
+        pass
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -168,15 +198,19 @@ def test_projection_matches_oracle(cfg):
     ws = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
     B.sp_indexer_scores(pbg, dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"]), q, k, False, 0, rows, sc, ws)
     torch.cuda.synchronize()
-    for got, want in ((bf16_bits(q), want_q), (bf16_bits(k), want_k)):
+    rates = {}
+    for name, got, want in (("q_idx", bf16_bits(q), want_q), ("k_idx", bf16_bits(k), want_k)):
         diff = got != want
+        rates[name] = float(diff.mean())
         # fp32 vs fp64 accumulation may flip a rounding tie: rare, and never by more than one bf16 ulp --
         # plus the absolute error of an fp32 sum of `hidden` unit-scale products (~ sqrt(hidden) * 2^-24 * |terms|,
-        # bounded here by 1e-5), which dominates for projected values that cancel to ~0.
-        assert diff.mean() < 5e-3, diff.mean()
+        # bounded here by 1e-5), which dominates for projected values that cancel to ~0.  Rate bound: DESIGN.md
+        # "Arithmetic and tolerances" (3x the measured rate kept in profiles/r2_parity.json).
+        assert diff.mean() < PROJ_MISMATCH_RATE, diff.mean()
         a = orc.bf16_to_f64(got[diff])
         b = orc.bf16_to_f64(want[diff])
         assert np.all(np.abs(a - b) <= np.abs(b) * 2.0 ** -7 + 1e-5)
+    record_stats(f"projection_mismatch_rate:{cfg.name}:L{cfg.L}:hidden{cfg.hidden}:d_idx{cfg.d_idx}", rates)
 
 
 @pytest.mark.parametrize("cfg,b", [(SMALL_IDX, 64), (SMALL_IDX, 1), (SMALL_IDX128, 64), (SMALL_IDX128, 128),
@@ -229,14 +263,17 @@ def test_served_projection_matches_oracle(cfg):
     ws = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
     B.sp_indexer_scores(pbg, dev(inp["X"]), dev(inp["Wqi"]), dev(inp["Wki"]), q, k, False, 0, rows, sc, ws)
     torch.cuda.synchronize()
-    for got, want in ((bf16_bits(q), want_q), (bf16_bits(k), want_k)):
+    rates = {}
+    for name, got, want in (("q_idx", bf16_bits(q), want_q), ("k_idx", bf16_bits(k), want_k)):
         diff = got != want
+        rates[name] = float(diff.mean())
         # fp32 (tensor-core sum, LayerNorm, sin/cos.approx after a double-precision range reduction) vs fp64: a value
         # close to a bf16 rounding boundary may land on the other side -- rare, and never by more than one ulp
-        assert diff.mean() < 1e-2, diff.mean()
+        assert diff.mean() < PROJ_SERVED_MISMATCH_RATE, diff.mean()
         a = orc.bf16_to_f64(got[diff])
         b = orc.bf16_to_f64(want[diff])
         assert np.all(np.abs(a - b) <= np.abs(b) * 2.0 ** -7 + 2e-5)
+    record_stats(f"served_projection_mismatch_rate:{cfg.name}:L{cfg.L}:hidden{cfg.hidden}:d_idx{cfg.d_idx}", rates)
     # the key rows are normalised: zero mean, unit variance over d_idx (up to bf16 rounding), rotation keeps that norm
     kf = to_f64(k)
     assert np.allclose((kf ** 2).sum(1), cfg.d_idx, rtol=2e-2)
@@ -543,17 +580,34 @@ def run_layer_and_compare(cfg, rows, n_queries, mode=None, seed=0, inputs=None):
 
     idx_gpu = idx.cpu().numpy()
     stats = parity.compare_supports(idx_gpu[rows], res.idx, res.scores, res.n_valid, cfg.k)
-    # chained: GPU end-to-end vs oracle end-to-end.  On a fuzzy row the two supports may legitimately differ
-    # (overlap rule above), and then so do the two outputs -- by the attention weight of the swapped keys, which
-    # no tolerance bounds.  Those queries are covered by the stage-isolated check below (GPU attention on the
-    # ORACLE's support); the chained tolerance applies to every query whose support row matched exactly.
+    # chained: GPU end-to-end vs oracle end-to-end, on EVERY sampled query.
+    #  * queries whose support row is identical on both sides: GPU output vs the oracle's end-to-end output;
+    #  * queries on a row where the two (rule-valid, see compare_supports) supports differ in near-tied keys: the
+    #    outputs then differ by the attention weight of the swapped keys, which no tolerance bounds (A18),
+    #    so the GPU's end-to-end output is compared with the ORACLE's attention (O6) recomputed on the GPU's own
+    #    support row -- selection is covered by the overlap rule, the recompute by this check.
+    # A floor on the identical fraction among rows BEYOND the budget (rows with n_valid <= k match trivially) keeps
+    # the first kind from becoming vacuous.
     same_row = {int(r): bool(np.array_equal(idx_gpu[r], res.idx[i])) for i, r in enumerate(rows)}
     keep = np.array([same_row[orc.row_of_pos(pbo, int(t))] for t in pos], dtype=bool)
+    beyond = [int(r) for i, r in enumerate(rows) if int(res.n_valid[i]) > cfg.k]
+    n_same_beyond = sum(same_row[r] for r in beyond)
+    stats["rows_sampled"] = int(len(rows))
+    stats["rows_beyond_budget"] = len(beyond)
+    stats["rows_beyond_budget_identical"] = int(n_same_beyond)
     stats["chained_queries"] = int(keep.sum())
-    stats["chained_skipped_fuzzy"] = int((~keep).sum())
-    assert keep.any() or len(pos) == 0, "no row with identical supports: nothing to compare end to end"
+    stats["chained_on_gpu_support"] = int((~keep).sum())
+    if beyond:
+        frac = n_same_beyond / len(beyond)
+        floor = 1.0 if stats["overlap"] == 1.0 else CHAINED_IDENTICAL_FLOOR
+        assert frac >= floor, f"only {n_same_beyond} of {len(beyond)} beyond-budget rows have identical supports"
     o_gpu = to_f64(O[torch.from_numpy(pos).to(DEV)])
-    stats["chained"] = parity.compare_attention(o_gpu[keep], res.out[keep])
+    if keep.any():
+        stats["chained"] = parity.compare_attention(o_gpu[keep], res.out[keep])
+    if (~keep).any():
+        sup_gpu = np.stack([idx_gpu[orc.row_of_pos(pbo, int(t))] for t in pos[~keep]])
+        want = orc.sparse_attn(pbo, inp["Q"], inp["K"], inp["V"], pos[~keep], sup_gpu)
+        stats["chained_gpu_support"] = parity.compare_attention(o_gpu[~keep], want)
     # stage-isolated: GPU attention on the ORACLE's supports for the sampled rows
     idx_mix = idx.clone()
     idx_mix[torch.from_numpy(rows).to(DEV)] = torch.from_numpy(res.idx).to(DEV)
@@ -565,6 +619,7 @@ def run_layer_and_compare(cfg, rows, n_queries, mode=None, seed=0, inputs=None):
     cnt = (idx_gpu >= 0).sum(axis=1)
     nv_all = np.array([orc.row_info(pbo, r)[2] + 1 for r in range(0, n_rows, max(1, n_rows // 997))])
     assert np.array_equal(cnt[::max(1, n_rows // 997)], np.minimum(cfg.k, nv_all))
+    record_stats(f"{cfg.name}:{mode or cfg.mode}:L{cfg.L}:k{cfg.k}:b{cfg.b_sel}", stats)
     return stats
 
 
@@ -579,8 +634,10 @@ def test_config2_indexer_block_shared_full_supports():
 
 
 def test_config3_9b_layer_sampled():
-    rows = [0, 1, 31, 32, 33, 200, 389, 511]
-    run_layer_and_compare(gen.C3, rows=rows, n_queries=256)
+    rng = np.random.Generator(np.random.Philox(3303))
+    rows = [0, 1, 31, 32, 33, 200, 389, 511] + list(rng.choice(np.arange(34, 511), size=28, replace=False))
+    st = run_layer_and_compare(gen.C3, rows=rows, n_queries=768)      # 36 rows, 32 of them beyond the budget
+    assert st["rows_sampled"] >= 32 and st["rows_beyond_budget"] >= 24
 
 
 @pytest.mark.parametrize("cfg", gen.C4_SWEEP, ids=lambda c: c.name)
@@ -593,8 +650,10 @@ def test_config4_sweep_sampled(cfg, mode):
 
 
 def test_config5_long_context_sampled():
-    rows = [0, 15, 16, 17, 500, 1023]
-    run_layer_and_compare(gen.C5, rows=rows, n_queries=192)
+    rng = np.random.Generator(np.random.Philox(5505))
+    rows = [0, 15, 16, 17, 500, 1023] + list(rng.choice(np.arange(18, 1023), size=18, replace=False))
+    st = run_layer_and_compare(gen.C5, rows=rows, n_queries=384)      # 24 rows, 21 beyond the budget
+    assert st["rows_sampled"] >= 24 and st["rows_beyond_budget"] >= 18
 
 
 def test_config5_varlen_pack_sampled():

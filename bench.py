@@ -145,24 +145,32 @@ def oracle_sample_rate(cfg, inp, budget_rows=None):
 
 
 def run_reference(args, cfg):
-    """--impl reference: the fp64 CPU oracle on the host cores, same config / metric / unit."""
+    """--impl reference: the fp64 CPU oracle on the host cores, same config / metric / unit.  Each step times the SAME
+    bounded sample as the cpu_baseline leg (oracle_sample_rate: at least as many support rows as OpenMP threads, so the
+    row-parallel oracle fills the cores) and extrapolates per token; `ms_per_step` is therefore the extrapolated time of
+    one whole layer, flagged as such, with the seconds actually spent beside it."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    from oracle import oracle as orc
     from paper_2606_07703_b200 import inputs as gen
     inp = gen.make_inputs(cfg)
+    threads = orc.max_threads()
+    rows = max(3 * threads, 48) if cfg.b_sel > 1 else max(32 * threads, 1024)   # a few seconds per step at c3 / c4
     for _ in range(min(args.warmup, 1)):
-        oracle_sample_rate(cfg, inp, budget_rows=1)
+        oracle_sample_rate(cfg, inp, budget_rows=threads)
     vals, secs = [], 0.0
     last = None
     for _ in range(args.steps):
-        last = oracle_sample_rate(cfg, inp, budget_rows=2 if cfg.b_sel > 1 else 64)
+        last = oracle_sample_rate(cfg, inp, budget_rows=rows)
         vals.append(last["value"])
         secs += last["seconds"]
     v = len(vals) / sum(1.0 / x for x in vals)
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * cfg.L / v, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * cfg.L / v, "extrapolated": True,
+        "measured_seconds_total": secs, "measured_seconds_per_step": secs / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(cfg),
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
@@ -362,6 +370,124 @@ def run_c3_groups(args, B, torch, gen, peaks):
     print(json.dumps(line))
 
 
+def _timed(torch, stream, fn, reps, warm=1):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(reps):
+        fn()
+    b.record(stream)
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def measure_oracle_mode(cfg, B, torch, devt, peaks, reps=2):
+    """The same layer in ORACLE mode (Alg.1: dense mass pass 1 + pass 2, top-k, sparse attention) on the tensors
+    already resident: layer ms and the two mass passes as TFLOP/s and exp/s (north_star: "indexer and oracle TFLOP/s")."""
+    stream = torch.cuda.current_stream()
+    pb = B.Problem.from_config(cfg)
+    n_rows, L = pb.num_rows, cfg.L
+    O = torch.empty(L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+    idx = torch.empty(n_rows, cfg.k, dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(pb, B.SP_STAGE_LAYER_ORACLE)
+    t_layer = _timed(torch, stream, lambda: B.sp_prefill_layer(pb, B.SP_MODE_ORACLE, None, None, None, devt["Q"],
+                                                               devt["K"], devt["V"], O, idx, ws), reps)
+    del ws
+    ld = (pb.max_seqlen + 3) // 4 * 4
+    panel = min(n_rows, max(1, (1 << 30) // (ld * 4)))
+    r0 = (n_rows - panel) // 2
+    mass = torch.empty(panel, ld, dtype=torch.float32, device="cuda")
+    lse = torch.empty(L, cfg.Hq, dtype=torch.float32, device="cuda")
+    t_p1 = _timed(torch, stream, lambda: B.sp_dense_gqa_attn(pb, devt["Q"], devt["K"], devt["V"], None, lse), reps)
+    t_p2 = _timed(torch, stream, lambda: B.sp_oracle_mass(pb, devt["Q"], devt["K"], lse, True, r0, panel, mass), reps)
+    t_p2 *= n_rows / panel
+    causal = L * (L + 1) // 2
+    fl = 2.0 * cfg.d * cfg.Hq * causal
+    ex = float(cfg.Hq) * causal
+    out = {"layer_ms": t_layer, "tokens_per_s": L / (t_layer * 1e-3),
+           "mass_pass1_lse": {"ms": t_p1, "TFLOPs": fl / (t_p1 * 1e-3) / 1e12, "Texp_per_s": ex / (t_p1 * 1e-3) / 1e12,
+                              "frac_of_burst_peak": fl / (t_p1 * 1e-3) / 1e12 / peaks["tensor_burst"]},
+           "mass_pass2": {"ms": t_p2, "TFLOPs": fl / (t_p2 * 1e-3) / 1e12, "Texp_per_s": ex / (t_p2 * 1e-3) / 1e12,
+                          "frac_of_burst_peak": fl / (t_p2 * 1e-3) / 1e12 / peaks["tensor_burst"],
+                          "panel_rows": [r0, r0 + panel], "scaled_by_rows": n_rows / panel},
+           "config": f"{cfg.name} shape, SP_MODE_ORACLE, b_sel={cfg.b_sel}, k={cfg.k}"}
+    return out
+
+
+def measure_per_query_c4(B, torch, gen, peaks, L=32768, reps=2):
+    """BASELINE.json configs[3] at L=32768 / k=2048, per-query supports, indexer mode: layer ms, stage split and the
+    gather rate of the per-query attention held against (a) the HBM copy peak and (b) the rate a PLAIN gather kernel
+    (sp_gather_probe) reaches on the same index stream (256-byte K rows out of L2)."""
+    stream = torch.cuda.current_stream()
+    cfg = next(c for c in gen.C4_SWEEP if c.L == L)
+    inp = gen.make_inputs(cfg, with_indexer=True)
+    dv = {n: B.bf16_tensor(inp[n]) for n in ("X", "Wqi", "Wki", "Q", "K", "V")}
+    pb = B.Problem.from_config(cfg)
+    k, n_rows = cfg.k, pb.num_rows
+    O = torch.empty(L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device="cuda")
+    idx = torch.empty(n_rows, k, dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(pb, B.SP_STAGE_LAYER_INDEXER)
+    t_layer = _timed(torch, stream, lambda: B.sp_prefill_layer(pb, B.SP_MODE_INDEXER, dv["X"], dv["Wqi"], dv["Wki"],
+                                                               dv["Q"], dv["K"], dv["V"], O, idx, ws), reps)
+    del ws
+    ld = (L + 3) // 4 * 4
+    panel = min(n_rows, max(1, (1 << 30) // (ld * 4)))
+    r0 = (n_rows - panel) // 2
+    f = n_rows / panel
+    sc = torch.empty(panel, ld, dtype=torch.float32, device="cuda")
+    q_idx = torch.empty(L, cfg.d_idx, dtype=torch.bfloat16, device="cuda")
+    k_idx = torch.empty_like(q_idx)
+    idx_p = torch.empty(panel, k, dtype=torch.int32, device="cuda")
+    wsx = B.alloc_workspace(pb, B.SP_STAGE_INDEXER_SCORES)
+    t_both = _timed(torch, stream, lambda: B.sp_indexer_scores(pb, dv["X"], dv["Wqi"], dv["Wki"], q_idx, k_idx, False,
+                                                               r0, panel, sc, wsx), reps)
+    t_sc = _timed(torch, stream, lambda: B.sp_indexer_scores(pb, None, None, None, q_idx, k_idx, True, r0, panel, sc), reps)
+    t_tk = _timed(torch, stream, lambda: B.sp_topk_support(pb, sc, r0, panel, idx_p), reps)
+    t_at = _timed(torch, stream, lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx, O), reps)
+    pairs = kept_pairs(L, k)
+    gather_bytes = 4.0 * cfg.Hkv * cfg.d * pairs
+    # plain gather of whole K token rows (all KV heads: Hkv * d * 2 bytes) over the attention's own index stream
+    sink = torch.empty(148 * 8 * 256, dtype=torch.int32, device="cuda")
+    row_b = pitch = cfg.Hkv * cfg.d * 2
+    t_probe = _timed(torch, stream, lambda: B.sp_gather_probe(dv["K"], row_b, pitch, idx, sink), reps)
+    probe_GBps = float(pairs) * row_b / (t_probe * 1e-3) / 1e9
+    causal = L * (L + 1) // 2
+    topk_bytes = 4.0 * causal + 4.0 * n_rows * k
+    g = gather_bytes / (t_at * 1e-3) / 1e9
+    return {"config": f"c4 L={L} k={k} b_sel=1 indexer mode (BASELINE.json configs[3])", "layer_ms": t_layer,
+            "tokens_per_s": L / (t_layer * 1e-3),
+            "stages_ms": {"projection": max(t_both - t_sc, 0.0), "scoring": t_sc * f, "topk": t_tk * f,
+                          "sparse_attention_per_query": t_at},
+            "scoring_score_write_GBps": 4.0 * causal / (t_sc * f * 1e-3) / 1e9,
+            "topk_GBps": topk_bytes / (t_tk * f * 1e-3) / 1e9, "topk_frac_of_hbm": topk_bytes / (t_tk * f * 1e-3) / 1e9 / peaks["hbm"],
+            "gather_GBps": g, "gather_frac_of_hbm_copy_peak": g / peaks["hbm"],
+            "plain_gather_probe_GBps": probe_GBps, "gather_frac_of_plain_gather": g / probe_GBps,
+            "note": "gathered K/V rows are mostly L2 hits (K+V = 134 MB), so the HBM fraction can exceed 1; the plain-gather "
+                    "figure is sp_gather_probe on the same index stream (whole 2 KB K token rows, measured in this run)",
+            "panel_rows": [r0, r0 + panel]}
+
+
+def measure_cold_l2(torch, step, n=8):
+    """One step at a time with a 256 MB scratch write before each (evicts the 126 MB L2): median / min of n."""
+    stream = torch.cuda.current_stream()
+    scratch = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    ts = []
+    for i in range(n + 1):
+        scratch.fill_(i & 0xff)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        step()
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i > 0:
+            ts.append(a.elapsed_time(b))
+    ts.sort()
+    return {"ms_median": ts[len(ts) // 2], "ms_min": ts[0], "n": n,
+            "how": "256 MB device scratch fill before every step; each step timed alone with CUDA events"}
+
+
 def measure_layer_only(cfg, B, torch, gen, steps):
     """Layer latency of another workload (device-resident inputs, CUDA events, 3 warm-up steps) next to the dense
     GQA layer of the same library on the same tensors."""
@@ -406,6 +532,8 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-long", action="store_true", help="skip the 128K (c5) layer line inside the c3 run")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the oracle-mode, per-query (c4 @ 32K) and cold-L2 legs of the c3 run")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -563,6 +691,11 @@ def main():
                               "unit": "TFLOP/s" if bd == "tensor" else "GB/s",
                               "frac": amt / (ms * 1e-3) / ((peaks["tensor"] * 1e12) if bd == "tensor" else (peaks["hbm"] * 1e9))}
 
+    extras = {}
+    if cfg.name == "c3" and not args.no_extras and world == 1:
+        extras["cold_l2"] = measure_cold_l2(torch, step)
+        extras["oracle_mode"] = measure_oracle_mode(cfg, B, torch, devt, peaks)
+
     # ---- end to end through the C ABI with HOST buffers ----
     arena = torch.empty(B.layer_host_arena_bytes(pb, gmode), dtype=torch.uint8, device="cuda")
     O_host = torch.empty(cfg.L, cfg.Hq, cfg.d, dtype=torch.bfloat16).pin_memory()
@@ -644,9 +777,16 @@ def main():
         if tr is not None:
             line["roofline"]["traffic"] = tr["dram_bytes_per_launch"]
             line["roofline"]["traffic_source"] = tr["source"]
+    line.update(extras)
+    if cfg.name == "c3" and not args.no_extras and world == 1:
+        del devt, host, O, O_dense, idx, ws, arena, scores
+        devt = host = O = O_dense = idx = ws = arena = scores = None
+        torch.cuda.empty_cache()
+        line["per_query_c4_32k"] = measure_per_query_c4(B, torch, gen, peaks)
+        torch.cuda.empty_cache()
     if cfg.name == "c3" and not args.no_long and world == 1:
         # the metric is quoted at 32K and 128K: the 128K layer (BASELINE.json configs[4]) timed in the same run
-        del devt, host, O, O_dense, idx, ws, arena, scores
+        devt = host = O = O_dense = idx = ws = arena = scores = None
         torch.cuda.empty_cache()
         line["long_context_128k"] = measure_layer_only(gen.ALL["c5"], B, torch, gen, steps=min(args.steps, 5))
     if rank == 0 and not args.no_cpu_baseline and world == 1:

@@ -25,6 +25,9 @@
  *    position local to the row's sequence.  Columns >= n_valid(row) are NOT written and never read.
  *  - Optional banded logit term (reading A20): when local_window > 0, local_bias is added to the
  *    scaled logit wherever 0 <= t-s < local_window, in every stage that forms a causal logit.
+ *  - One library instance may be used on several devices of a process (the caller selects the device with
+ *    cudaSetDevice before the call, as for any stream-ordered work); per-device function attributes and SM counts are
+ *    cached per device.  There are no environment-variable switches.
  *  - Return value: SP_OK (0) or a negative sp_status.  On any error nothing has been launched.  No
  *    exceptions cross this ABI and nothing aborts.  There is no CPU fallback.
  */
@@ -91,7 +94,8 @@ enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u, SP_F_GROUP_SUPPORT = 8u
 /* SP_F_GROUP_SUPPORT ("shared within each KV group S_{l,t,r}"; A29) is read by
  * sp_sparse_gqa_attn ONLY: idx is then [Hkv, n_rows, k] -- one support list per KV group and support row, each
  * list as described under "idx" below -- and query head h attends the list of group g(h).  Every other entry
- * point returns SP_ERR_UNSUPPORTED when the bit is set (per-group selection has no CUDA path yet). */
+ * point returns SP_ERR_UNSUPPORTED when the bit is set; the lists themselves come from sp_oracle_mass_group +
+ * sp_topk_support (one call pair per KV group). */
 
 /* Number of support rows of the whole pack (host arithmetic only). Returns < 0 on invalid params. */
 int64_t sp_num_rows(const sp_params *p);
@@ -169,6 +173,14 @@ int sp_dense_gqa_attn(const sp_params *p, const void *Q, const void *K, const vo
 int sp_support_overlap(const sp_params *p, const int32_t *idx_a, const int32_t *idx_b, int32_t *inter, void *stream);
 int sp_row_kl(const sp_params *p, const float *mass, int64_t ld_mass, const float *scores, int64_t ld_scores,
               int32_t row_begin, int32_t row_count, float *kl, void *stream);
+
+/* Measurement aid, not a step of the path: a plain gather of n_idx rows of row_bytes bytes (a multiple of 256) at
+ * base + idx[e] * row_pitch_bytes (idx < 0 = skip), 16 bytes per lane, four rows in flight per half warp.  bench.py times
+ * it on the per-query attention's own index stream to obtain the L2 / HBM gather bandwidth that path can be held
+ * against (a per-query support row is used by only Hq/Hkv query rows: "harder to fuse and amortize").
+ * sink: DEVICE scratch of >= 148 * 8 * 256 * 4 bytes (one word per probe thread). */
+int sp_gather_probe(const void *base, int32_t row_bytes, int64_t row_pitch_bytes, const int32_t *idx, int64_t n_idx,
+                    void *sink, size_t sink_bytes, void *stream);
 
 /* One patched layer on one stream (PAPER.md:292 five-stage path without the paged-cache stage; Alg.1 steps
  * 2-5 in SP_MODE_ORACLE, Alg.2 steps 2,4,5 in SP_MODE_INDEXER).  Support rows are processed in panels so the

@@ -340,6 +340,80 @@ def sparse_attn_per_group(pb: Problem, Q, K, V, pos, sup):
     return out
 
 
+# ---------------------------------------------------------------- chunked prefill against a paged KV cache
+# PAPER.md:292 (five-stage serving path, stage 4 "reconstruct K/V from the paged KV cache when the chunked path requires
+# contiguous tensors"), :331 and :428 (chunks of max_num_batched_tokens = 4K / 8K queries against the whole prefix).
+# Reading (A30): a chunk is the queries [q_begin, q_begin + q_count) of ONE sequence whose first q_begin
+# tokens are already cached; the chunk first writes its own K, V (and indexer keys) into the cache, then every stage
+# of the layer runs for the chunk's support rows against the cache's first q_begin + q_count tokens.  Selection blocks
+# stay aligned to the sequence start, so q_begin must be a multiple of b_sel.  The oracle does literally what the
+# paper's stage 4 says: it reconstructs contiguous tensors from the pages (pure indexing) and runs the SAME functions
+# as for a full prefill -- the result for the chunk's queries must equal the full-prefill result bit for bit.
+
+@dataclass
+class PagedCache:
+    """K / V / indexer-key pages: [n_pages, page_size, row_elems] uint16 each; block_table[i] = physical page of logical block i."""
+    page_size: int
+    block_table: np.ndarray
+    k: np.ndarray
+    v: np.ndarray
+    kidx: Optional[np.ndarray] = None
+
+
+def paged_scatter(cache: np.ndarray, block_table, page_size: int, t_begin: int, rows: np.ndarray):
+    rows = _u16(rows).reshape(rows.shape[0], -1)
+    bt = _i32(block_table)
+    assert cache.dtype == np.uint16 and cache.flags.c_contiguous
+    lib().orc_paged_scatter(_ptr(cache, C.c_uint16), _ptr(bt, C.c_int32), C.c_int32(page_size),
+                            C.c_int64(rows.shape[1]), C.c_int32(t_begin), C.c_int32(t_begin + rows.shape[0]),
+                            _ptr(rows, C.c_uint16))
+
+
+def paged_gather(cache: np.ndarray, block_table, page_size: int, t_begin: int, t_end: int) -> np.ndarray:
+    bt = _i32(block_table)
+    assert cache.dtype == np.uint16 and cache.flags.c_contiguous
+    row_elems = int(np.prod(cache.shape[2:]))
+    out = np.empty((t_end - t_begin, row_elems), dtype=np.uint16)
+    lib().orc_paged_gather(_ptr(cache, C.c_uint16), _ptr(bt, C.c_int32), C.c_int32(page_size), C.c_int64(row_elems),
+                           C.c_int32(t_begin), C.c_int32(t_end), _ptr(out, C.c_uint16))
+    return out
+
+
+def prefill_chunk(pb: Problem, mode: int, q_begin: int, q_count: int, Q_chunk, K_chunk, V_chunk, cache: PagedCache,
+                  X_chunk=None, Wqi=None, Wki=None, rows=None, pos=None) -> LayerResult:
+    """One prefill chunk of one sequence against the paged cache (see the block comment above).  pb.L must be the
+    context length q_begin + q_count.  The cache is UPDATED with the chunk's K, V (and k_idx).  `rows` / `pos` restrict
+    the evaluation to some of the chunk's support rows / queries (absolute row numbers and positions)."""
+    n_ctx = q_begin + q_count
+    assert pb.cu_seqlens is None and pb.L == n_ctx and q_begin % pb.b_sel == 0
+    ps, bt = cache.page_size, cache.block_table
+    k_idx_chunk = None
+    if mode == MODE_INDEXER:
+        # projections of the chunk's tokens at their absolute positions (RoPE, A28)
+        Xf = np.zeros((n_ctx, pb.hidden), np.uint16)
+        Xf[q_begin:] = _u16(X_chunk).reshape(q_count, pb.hidden)
+        chunk_pos = np.arange(q_begin, n_ctx)
+        q_idx_chunk = project(pb, Xf, Wqi, rows=chunk_pos)
+        k_idx_chunk = project(pb, Xf, Wki, rows=chunk_pos, key=True)
+        paged_scatter(cache.kidx, bt, ps, q_begin, k_idx_chunk)
+    paged_scatter(cache.k, bt, ps, q_begin, K_chunk)
+    paged_scatter(cache.v, bt, ps, q_begin, V_chunk)
+    # stage 4: contiguous K, V (k_idx) of the whole context from the pages
+    K = paged_gather(cache.k, bt, ps, 0, n_ctx)
+    V = paged_gather(cache.v, bt, ps, 0, n_ctx)
+    Q = np.zeros((n_ctx, pb.Hq * pb.d), np.uint16)
+    Q[q_begin:] = _u16(Q_chunk).reshape(q_count, -1)
+    r0, r1 = q_begin // pb.b_sel, num_rows(pb)
+    rows = _i32(np.arange(r0, r1) if rows is None else rows)
+    assert rows.min() >= r0 and rows.max() < r1
+    kw = {}
+    if mode == MODE_INDEXER:
+        qi = np.zeros((n_ctx, pb.d_idx), np.uint16)
+        qi[q_begin:] = q_idx_chunk
+        kw = dict(q_idx=qi, k_idx=paged_gather(cache.kidx, bt, ps, 0, n_ctx))
+    return prefill_layer(pb, mode, Q, K, V, rows=rows, pos=pos, **kw)
+
+
 # ---------------------------------------------------------------- support-level diagnostics (PAPER.md:262, :478)
 
 def support_overlap(idx_a, idx_b) -> np.ndarray:

@@ -36,7 +36,9 @@
  * MHA-with-repeated-KV == GQA, kept-pair count k*L-k(k-1)/2 and the sparsities the paper prints
  * (PAPER.md:180,216,374), the hand-worked case tests/golden/handworked_L4.txt, Q=0 closed form,
  * k>=n sparse==dense, numpy stable argsort, torch SDPA, numpy brute force on tiny inputs, varlen
- * pack == separate sequences.  Indexer *quality* / task gaps: parity unpinned and out of scope.
+ * pack == separate sequences; the paged-cache routines (pure indexing) against numpy fancy indexing, scatter-then-
+ * gather == identity, block-table permutation invariance and chunked+paged == full prefill, bit for bit.
+ * Indexer *quality* / task gaps: parity unpinned and out of scope.
  */
 #include <math.h>
 #include <stdint.h>
@@ -436,6 +438,34 @@ void orc_dense_attn(const orc_params *p, const uint16_t *Q, const uint16_t *K, c
       }
     }
     free(a);
+  }
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Paged KV cache (stage 4 of the five-stage serving path: "reconstruct K/V from the paged KV cache when
+ * the chunked path requires contiguous tensors"; :331, :428 chunked prefill with max_num_batched_tokens 4K / 8K).
+ * A cache tensor is [n_pages][page_size][row_elems] bf16; logical token t of the sequence lives in physical page
+ * block_table[t / page_size] at slot t % page_size.  Both routines are pure indexing (no arithmetic), so anything
+ * computed from the reconstructed tensors is bit-identical to the same computation on the original contiguous
+ * tensors -- which is the pin (tests/test_oracle_pins.py::test_paged_*).
+ * --------------------------------------------------------------------------------------------------------- */
+/* contiguous[t - t_begin, :] = cache[block_table[t / page_size], t % page_size, :]  for t in [t_begin, t_end) */
+void orc_paged_gather(const uint16_t *cache, const int32_t *block_table, int32_t page_size, int64_t row_elems,
+                      int32_t t_begin, int32_t t_end, uint16_t *contiguous) {
+  for (int32_t t = t_begin; t < t_end; ++t) {
+    const int64_t page = block_table[t / page_size], slot = t % page_size;
+    memcpy(contiguous + (int64_t)(t - t_begin) * row_elems, cache + (page * page_size + slot) * row_elems,
+           (size_t)row_elems * sizeof(uint16_t));
+  }
+}
+/* cache[block_table[t / page_size], t % page_size, :] = rows[t - t_begin, :]  for t in [t_begin, t_end): the write a
+ * prefill chunk makes for its own tokens before it attends to the prefix */
+void orc_paged_scatter(uint16_t *cache, const int32_t *block_table, int32_t page_size, int64_t row_elems,
+                       int32_t t_begin, int32_t t_end, const uint16_t *rows) {
+  for (int32_t t = t_begin; t < t_end; ++t) {
+    const int64_t page = block_table[t / page_size], slot = t % page_size;
+    memcpy(cache + (page * page_size + slot) * row_elems, rows + (int64_t)(t - t_begin) * row_elems,
+           (size_t)row_elems * sizeof(uint16_t));
   }
 }
 

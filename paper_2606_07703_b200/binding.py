@@ -28,7 +28,7 @@ EXPORTS = (
     "sp_num_rows", "sp_workspace_bytes", "sp_indexer_scores", "sp_oracle_mass", "sp_topk_support",
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
     "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
-    "sp_oracle_mass_group",
+    "sp_oracle_mass_group", "sp_gather_probe",
 )
 
 
@@ -246,6 +246,13 @@ def sp_row_kl(pb: Problem, mass: torch.Tensor, scores: torch.Tensor, row_begin: 
     p = pb.c()
     _check(lib().sp_row_kl(C.byref(p), _ptr(mass), C.c_int64(mass.stride(0)), _ptr(scores), C.c_int64(scores.stride(0)),
                            C.c_int32(row_begin), C.c_int32(row_count), _ptr(kl), _stream()))
+
+
+def sp_gather_probe(base: torch.Tensor, row_bytes: int, row_pitch_bytes: int, idx: torch.Tensor, sink: torch.Tensor):
+    """Plain gather of idx.numel() rows of row_bytes bytes (measurement aid, see include/sp.h)."""
+    _check(lib().sp_gather_probe(_ptr(base), C.c_int32(row_bytes), C.c_int64(row_pitch_bytes), _ptr(idx),
+                                 C.c_int64(idx.numel()), _ptr(sink), C.c_size_t(sink.numel() * sink.element_size()),
+                                 _stream()))
 
 
 def launch_count() -> int:

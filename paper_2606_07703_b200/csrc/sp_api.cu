@@ -12,17 +12,6 @@
 
 namespace {
 
-// Debug switch (never set in tests/bench): SP_DEBUG_SIMT bitmask routes a stage to its CUDA-core kernel so the two
-// device implementations can be compared on the GPU box.  1 = projection, 2 = indexer scores, 4 = attention, 8 = mass.
-int debug_simt() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = getenv("SP_DEBUG_SIMT");
-    v = e ? atoi(e) : 0;
-  }
-  return v;
-}
-
 std::atomic<long long> g_launches{0};
 std::mutex g_err_mu;
 char g_err_text[512] = "no CUDA error recorded";
@@ -91,7 +80,7 @@ int validate_common(const sp_params* p, bool need_attn, bool need_indexer) {
     return SP_ERR_INVALID_ARG;
   }
   if (p->flags & ~(uint32_t)(SP_F_RELU | SP_F_KEY_LN | SP_F_ROPE)) return SP_ERR_UNSUPPORTED;
-  if (p->flags != 0 && (!sp_tc_scores_supported(p->b_sel) || debug_simt())) return SP_ERR_UNSUPPORTED;
+  if (p->flags != 0 && !sp_tc_scores_supported(p->b_sel)) return SP_ERR_UNSUPPORTED;
   if (p->local_window < 0) return SP_ERR_INVALID_ARG;
   if (need_attn) {
     if (p->Hq < 1 || p->Hkv < 1 || p->d < 1 || p->Hq % p->Hkv != 0) return SP_ERR_INVALID_ARG;
@@ -122,18 +111,18 @@ int validate_panel(const sp_params* p, int32_t row_begin, int32_t row_count, int
   return SP_OK;
 }
 
-// ---- stage dispatch: tcgen05 kernels where the shape is in their built set, CUDA-core kernels otherwise ----
+// ---- stage dispatch: tcgen05 kernels where the shape is in their built set; the CUDA-core kernels of sp_simt.cu
+// only for selection blocks outside it (b_sel not in {1,32,64,128}) and for dense attention over a query sub-range ----
 cudaError_t run_project(const sp_params* p, const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx,
                         void* ws, cudaStream_t st) {
-  if (!(debug_simt() & 1))
-    return sp_launch_project_tc(dev_geom(p), p->flags, X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, st);
-  return sp_launch_project(X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, ws, st);
+  (void)ws;
+  return sp_launch_project_tc(dev_geom(p), p->flags, X, Wq, Wk, q_idx, k_idx, p->L, p->hidden, p->d_idx, st);
 }
 
 cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void* k_idx, int row_begin, int row_count,
                                int max_nv, float* scores, int64_t ld, cudaStream_t st) {
   const SpGeom g = dev_geom(p);
-  if (sp_tc_scores_supported(p->b_sel) && !(debug_simt() & 2))
+  if (sp_tc_scores_supported(p->b_sel))
     return sp_launch_indexer_scores_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, q_idx, k_idx, p->d_idx,
                                        index_scale(p), p->local_window, p->local_bias, (p->flags & SP_F_RELU) ? 1 : 0,
                                        row_begin, row_count, max_nv, scores, ld, st);
@@ -144,7 +133,7 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
 cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const float* lse, int row_begin, int row_count,
                      int max_nv, float* mass, int64_t ld, cudaStream_t st, int grp = -1) {
   const SpGeom g = dev_geom(p);
-  if (sp_tc_mass_supported(p->b_sel, p->d) && (grp >= 0 || !(debug_simt() & 8)))
+  if (sp_tc_mass_supported(p->b_sel, p->d))
     return sp_launch_mass_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, Q, K, lse, p->Hq, p->Hkv, p->d,
                              attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st, grp);
   if (grp >= 0) return cudaErrorNotSupported;  // callers check sp_tc_mass_supported first
@@ -162,7 +151,7 @@ cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const voi
   const int G = p->Hq / p->Hkv;
   const bool whole = q_begin == 0 && q_count == p->L;
   const bool dense_lse_range = idx == nullptr && O == nullptr && q_count > 0;
-  if ((whole || dense_lse_range) && !(debug_simt() & 4) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k, p->d)) {
+  if ((whole || dense_lse_range) && sp_tc_attn_supported(p->b_sel, G, idx != nullptr, p->k, p->d)) {
     const HostGeom hg = host_geom(p);
     const int QT = 256 / G;
     long long chunks = 0, c_lo = -1, c_hi = -1;
@@ -184,7 +173,7 @@ cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const voi
     return sp_launch_attn_tc(g, hg.num_rows(), c_hi - c_lo + 1, c_lo, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d,
                              attn_scale(p), p->local_window, p->local_bias, O, lse, st);
   }
-  if (idx != nullptr && !(debug_simt() & 4))  // per-query / small-block supports: warp-level mma.sync + cp.async gathers
+  if (idx != nullptr)  // per-query / small-block supports: warp-level mma.sync + cp.async gathers
     return sp_launch_attn_pq(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
                              q_begin, q_count, O, lse, st);
   return sp_launch_attn(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
@@ -231,6 +220,23 @@ LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws) {
 }  // namespace
 
 void sp_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+int sp_current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= SP_MAX_DEVICES) dev = 0;
+  return dev;
+}
+
+int sp_sm_count() {
+  static int n[SP_MAX_DEVICES];
+  const int dev = sp_current_device();
+  if (n[dev] == 0) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+    n[dev] = v;
+  }
+  return n[dev];
+}
 
 extern "C" {
 
@@ -383,6 +389,18 @@ int sp_row_kl(const sp_params* p, const float* mass, int64_t ld_mass, const floa
   return SP_OK;
 }
 
+int sp_gather_probe(const void* base, int32_t row_bytes, int64_t row_pitch_bytes, const int32_t* idx, int64_t n_idx,
+                    void* sink, size_t sink_bytes, void* stream) {
+  if (!base || !idx || !sink || !aligned16(base) || n_idx < 1) return SP_ERR_INVALID_ARG;
+  if (row_bytes < 256 || row_bytes % 256 != 0 || row_pitch_bytes < row_bytes || row_pitch_bytes % 16 != 0)
+    return SP_ERR_INVALID_ARG;
+  const int blocks = 148 * 8;
+  if (sink_bytes < (size_t)blocks * 256 * sizeof(uint32_t)) return SP_ERR_WORKSPACE;
+  SP_CUDA(sp_launch_gather_probe(base, row_bytes, row_pitch_bytes, idx, n_idx, (uint32_t*)sink, blocks,
+                                 (cudaStream_t)stream), "gather probe");
+  return SP_OK;
+}
+
 int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
                        float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
   if (!p) return SP_ERR_INVALID_ARG;
@@ -446,6 +464,171 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
   SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st), "sparse attention");
   return SP_OK;
 }
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// Chunked prefill against a paged KV cache (PAPER.md:292 stage 4, :331, :428; reading A30)
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+
+int page_shift_of(int32_t page_size) {
+  for (int s = 4; s <= 12; ++s)
+    if (page_size == (1 << s)) return s;
+  return -1;
+}
+
+int validate_pages(const sp_params* p, const sp_kv_pages* kv, bool need_kidx) {
+  if (!kv || !kv->k_pages || !kv->v_pages || !kv->block_table) return SP_ERR_INVALID_ARG;
+  if (need_kidx && !kv->kidx_pages) return SP_ERR_INVALID_ARG;
+  if (!aligned16(kv->k_pages) || !aligned16(kv->v_pages) || !aligned16(kv->kidx_pages)) return SP_ERR_INVALID_ARG;
+  if (page_shift_of(kv->page_size) < 0) return SP_ERR_UNSUPPORTED;  // powers of two, 16 ... 4096 tokens
+  if (kv->n_pages < 1 || kv->n_blocks < 1) return SP_ERR_INVALID_ARG;
+  if ((long long)kv->n_blocks * kv->page_size < p->L) return SP_ERR_INVALID_ARG;  // the table must cover the context
+  return SP_OK;
+}
+
+struct ChunkPlan {
+  int64_t ld;
+  long long row0, n_rows, panel_rows;
+  size_t off_qidx, off_kidx, off_scores, off_idx, total;
+};
+
+ChunkPlan plan_chunk(const sp_params* p, int32_t q_begin, int32_t q_count, bool idx_in_ws) {
+  ChunkPlan pl{};
+  pl.row0 = q_begin / p->b_sel;
+  pl.n_rows = (q_count + p->b_sel - 1) / p->b_sel;
+  pl.ld = (int64_t)align_up((size_t)p->L, 4);
+  long long pr = (long long)(PANEL_BYTES / ((size_t)pl.ld * sizeof(float)));
+  if (pr < 1) pr = 1;
+  if (p->b_sel == 1 && pr >= 64) pr = pr / 64 * 64;
+  if (pr > pl.n_rows) pr = pl.n_rows;
+  pl.panel_rows = pr;
+  size_t off = 0;
+  pl.off_qidx = off; off += align_up((size_t)q_count * p->d_idx * 2);
+  pl.off_kidx = off; off += align_up((size_t)q_count * p->d_idx * 2);
+  pl.off_scores = off; off += align_up((size_t)pl.panel_rows * pl.ld * sizeof(float));
+  pl.off_idx = off;
+  if (idx_in_ws) off += align_up((size_t)pl.n_rows * p->k * sizeof(int32_t));
+  pl.total = off;
+  return pl;
+}
+
+int validate_chunk(const sp_params* p, int32_t q_begin, int32_t q_count) {
+  const int rc = validate_common(p, true, true);
+  if (rc != SP_OK) return rc;
+  if (p->cu_seqlens || p->batch != 1) return SP_ERR_UNSUPPORTED;  // one sequence per chunk call
+  if (q_begin < 0 || q_count < 1 || (long long)q_begin + q_count != p->L) return SP_ERR_INVALID_ARG;
+  if (q_begin % p->b_sel != 0) return SP_ERR_INVALID_ARG;         // selection blocks stay aligned to the sequence start
+  if (!sp_tc_scores_supported(p->b_sel)) return SP_ERR_UNSUPPORTED;  // the paged readers are the tcgen05 / mma.sync kernels
+  return SP_OK;
+}
+
+}  // namespace
+
+extern "C" int sp_chunk_workspace_bytes(const sp_params* p, int32_t q_begin, int32_t q_count, size_t* bytes_out) {
+  if (!bytes_out) return SP_ERR_INVALID_ARG;
+  const int rc = validate_chunk(p, q_begin, q_count);
+  if (rc != SP_OK) return rc;
+  *bytes_out = plan_chunk(p, q_begin, q_count, true).total;
+  return SP_OK;
+}
+
+static int kv_copy_impl(bool to_pages, const sp_params* p, const sp_kv_pages* kv, int32_t t_begin, int32_t t_count,
+                        void* Kc, void* Vc, void* kidx_c, void* stream) {
+  int rc = validate_common(p, true, kidx_c != nullptr);
+  if (rc != SP_OK) return rc;
+  rc = validate_pages(p, kv, kidx_c != nullptr);
+  if (rc != SP_OK) return rc;
+  if (t_begin < 0 || t_count < 0 || (long long)t_begin + t_count > (long long)kv->n_blocks * kv->page_size)
+    return SP_ERR_INVALID_ARG;
+  if ((!Kc && !Vc && !kidx_c) || !aligned16(Kc) || !aligned16(Vc) || !aligned16(kidx_c)) return SP_ERR_INVALID_ARG;
+  const int sh = page_shift_of(kv->page_size);
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long kvb = (long long)p->Hkv * p->d * 2;
+  if (Kc) SP_CUDA(sp_launch_paged_copy(to_pages, kv->k_pages, Kc, kv->block_table, sh, kvb, t_begin, t_count, st), "paged K copy");
+  if (Vc) SP_CUDA(sp_launch_paged_copy(to_pages, kv->v_pages, Vc, kv->block_table, sh, kvb, t_begin, t_count, st), "paged V copy");
+  if (kidx_c)
+    SP_CUDA(sp_launch_paged_copy(to_pages, kv->kidx_pages, kidx_c, kv->block_table, sh, (long long)p->d_idx * 2, t_begin,
+                                 t_count, st), "paged k_idx copy");
+  return SP_OK;
+}
+
+extern "C" int sp_kv_append(const sp_params* p, const sp_kv_pages* kv, int32_t t_begin, int32_t t_count, const void* K_new,
+                            const void* V_new, const void* kidx_new, void* stream) {
+  return kv_copy_impl(true, p, kv, t_begin, t_count, const_cast<void*>(K_new), const_cast<void*>(V_new),
+                      const_cast<void*>(kidx_new), stream);
+}
+
+extern "C" int sp_kv_gather(const sp_params* p, const sp_kv_pages* kv, int32_t t_begin, int32_t t_count, void* K_out,
+                            void* V_out, void* kidx_out, void* stream) {
+  return kv_copy_impl(false, p, kv, t_begin, t_count, K_out, V_out, kidx_out, stream);
+}
+
+extern "C" int sp_prefill_chunk(const sp_params* p, int32_t q_begin, int32_t q_count, const void* X, const void* Wqi,
+                                const void* Wki, const void* Q, const void* K_new, const void* V_new,
+                                const sp_kv_pages* kv, void* O, int32_t* idx_out, void* ws, size_t ws_bytes,
+                                void* stream) {
+  int rc = validate_chunk(p, q_begin, q_count);
+  if (rc != SP_OK) return rc;
+  rc = validate_pages(p, kv, true);
+  if (rc != SP_OK) return rc;
+  if (!X || !Wqi || !Wki || !Q || !K_new || !V_new || !O) return SP_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Wqi) || !aligned16(Wki) || !aligned16(Q) || !aligned16(K_new) || !aligned16(V_new) ||
+      !aligned16(O))
+    return SP_ERR_INVALID_ARG;
+  const ChunkPlan pl = plan_chunk(p, q_begin, q_count, idx_out == nullptr);
+  if (!ws || !aligned16(ws) || ws_bytes < pl.total) return SP_ERR_WORKSPACE;
+  char* base = (char*)ws;
+  cudaStream_t st = (cudaStream_t)stream;
+  void* q_idx = base + pl.off_qidx;
+  void* k_idx = base + pl.off_kidx;
+  float* scores = (float*)(base + pl.off_scores);
+  int32_t* idx = idx_out ? idx_out : (int32_t*)(base + pl.off_idx);
+  const int sh = page_shift_of(kv->page_size);
+
+  // stage 1: indexer projections of the chunk's tokens at their absolute positions
+  SpGeom gp{1, q_count, nullptr, p->b_sel, 0};
+  gp.pos_off = q_begin;
+  SP_CUDA(sp_launch_project_tc(gp, p->flags, X, Wqi, Wki, q_idx, k_idx, q_count, p->hidden, p->d_idx, st), "chunk projection");
+  // the chunk's own K, V and indexer keys go into the cache before anything reads it
+  SP_CUDA(sp_launch_paged_copy(true, kv->k_pages, const_cast<void*>(K_new), kv->block_table, sh, (long long)p->Hkv * p->d * 2,
+                               q_begin, q_count, st), "append K");
+  SP_CUDA(sp_launch_paged_copy(true, kv->v_pages, const_cast<void*>(V_new), kv->block_table, sh, (long long)p->Hkv * p->d * 2,
+                               q_begin, q_count, st), "append V");
+  SP_CUDA(sp_launch_paged_copy(true, kv->kidx_pages, k_idx, kv->block_table, sh, (long long)p->d_idx * 2, q_begin, q_count, st),
+          "append k_idx");
+  // stages 2, 3, 5: every reader goes through the block table (no reconstruction of contiguous K / V)
+  SpGeom g = dev_geom(p);
+  g.q_off = q_begin;
+  g.q_rows = q_count;
+  g.row_off = (int)pl.row0;
+  g.bt = kv->block_table;
+  g.page_shift = sh;
+  g.n_blocks = kv->n_blocks;
+  g.kv_rows = (long long)kv->n_pages * kv->page_size;
+  const HostGeom hg = host_geom(p);
+  for (long long r = 0; r < pl.n_rows; r += pl.panel_rows) {
+    const int rcnt = (int)(pl.n_rows - r < pl.panel_rows ? pl.n_rows - r : pl.panel_rows);
+    const int rb = (int)(pl.row0 + r);
+    const int max_nv = hg.max_n_valid(rb, rcnt);
+    SP_CUDA(sp_launch_indexer_scores_tc(g, nullptr, q_idx, kv->kidx_pages, p->d_idx, index_scale(p), p->local_window,
+                                        p->local_bias, (p->flags & SP_F_RELU) ? 1 : 0, rb, rcnt, max_nv, scores, pl.ld, st),
+            "chunk indexer scores");
+    SP_CUDA(sp_launch_topk(g, scores, pl.ld, rb, rcnt, p->k, max_nv, idx + (size_t)r * p->k, nullptr, st), "chunk top-k");
+  }
+  const int G = p->Hq / p->Hkv;
+  if (sp_tc_attn_supported(p->b_sel, G, true, p->k, p->d)) {
+    SP_CUDA(sp_launch_attn_tc(g, pl.n_rows, 0, 0, Q, kv->k_pages, kv->v_pages, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p),
+                              p->local_window, p->local_bias, O, nullptr, st), "chunk sparse attention");
+  } else {
+    SP_CUDA(sp_launch_attn_pq(g, Q, kv->k_pages, kv->v_pages, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window,
+                              p->local_bias, q_begin, q_count, O, nullptr, st), "chunk sparse attention (per query)");
+  }
+  return SP_OK;
+}
+
+extern "C" {
 
 int sp_layer_host_arena_bytes(const sp_params* p, int32_t mode, size_t* bytes_out) {
   if (!bytes_out || (mode != SP_MODE_ORACLE && mode != SP_MODE_INDEXER)) return SP_ERR_INVALID_ARG;

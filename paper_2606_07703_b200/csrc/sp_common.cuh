@@ -17,7 +17,23 @@ struct SpGeom {
   const int* cu;  // device cu_seqlens or nullptr
   int b_sel;
   long long idx_grp;  // SP_F_GROUP_SUPPORT: elements between two KV groups' index lists ([Hkv, n_rows, k]); 0 = one shared list
+  // ---- chunked prefill against a paged KV cache (sp_prefill_chunk; PAPER.md:292 stage 4, :331); all zero otherwise ----
+  int q_off;       // packed position of row 0 of the QUERY-side tensors (Q, O, lse, q_idx): they hold the chunk only
+  int q_rows;      // rows of those tensors (0 = L)
+  int row_off;     // support row of row 0 of the index tensor
+  int pos_off;     // projection only: position of row 0 of X (rotary embedding of a chunk)
+  const int* bt;   // DEVICE block table of the KEY-side tensors (K, V, k_idx pages), nullptr = contiguous [L, ...]
+  int page_shift;  // log2(tokens per page)
+  int n_blocks;    // entries of bt
+  long long kv_rows;  // rows of the page pool (n_pages * page_size)
 };
+
+// row of packed key position p in the key-side tensors: p itself, or its slot in the paged cache
+__device__ __forceinline__ long long sp_kv_row(const SpGeom& g, int p) {
+  if (g.bt == nullptr) return p;
+  const int blk = min(p >> g.page_shift, g.n_blocks - 1);
+  return ((long long)__ldg(g.bt + blk) << g.page_shift) | (long long)(p & ((1 << g.page_shift) - 1));
+}
 
 struct SpRow {
   int seq_start;  // packed position of the sequence's first token
@@ -90,9 +106,6 @@ struct SpLaunch {
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
                            int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st);
 
-cudaError_t sp_launch_project(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
-                              int hidden, int d_idx, void* ws, cudaStream_t st);
-
 cudaError_t sp_launch_indexer_scores(const SpGeom& g, const void* q_idx, const void* k_idx, int d_idx,
                                      float idx_scale, int local_window, float local_bias, int row_begin,
                                      int row_count, int max_n_valid, float* scores, int64_t ld, cudaStream_t st);
@@ -138,4 +151,23 @@ cudaError_t sp_launch_overlap(const int32_t* a, const int32_t* b, long long n_ro
 cudaError_t sp_launch_row_kl(const SpGeom& g, const float* P, int64_t ldp, const float* z, int64_t ldz, int row_begin,
                              int row_count, float* kl, cudaStream_t st);
 
+// paged KV cache plumbing (sp_paged.cu): rows <-> page slots through the block table
+cudaError_t sp_launch_paged_copy(bool to_pages, void* pool, void* rows, const int32_t* bt, int page_shift,
+                                 long long row_bytes, int t_begin, int t_count, cudaStream_t st);
+
+cudaError_t sp_launch_gather_probe(const void* base, int row_bytes, long long row_pitch_bytes, const int32_t* idx,
+                                   long long n_idx, uint32_t* sink, int blocks, cudaStream_t st);
+
 void sp_count_launch(int n = 1);
+
+// Per-DEVICE host-side caches: a process may drive several GPUs through the library (cudaFuncSetAttribute and the SM
+// count belong to the current device).  Races between threads are benign (the same value is written twice).
+constexpr int SP_MAX_DEVICES = 64;
+int sp_current_device();              // cudaGetDevice, clamped to [0, SP_MAX_DEVICES)
+int sp_sm_count();                    // multiprocessors of the current device
+inline bool sp_first_use_on_device(unsigned char (&seen)[SP_MAX_DEVICES]) {
+  const int d = sp_current_device();
+  if (seen[d]) return false;
+  seen[d] = 1;
+  return true;
+}

@@ -80,7 +80,46 @@ sp_row_kl_kernel(SpGeom g, const float* __restrict__ P, int64_t ldp, const float
   if (threadIdx.x == 0) kl[r] = acc;
 }
 
+// Gather-bandwidth probe (measurement aid for the per-query attention's roofline: bench.py divides the kernel's
+// gathered bytes per second by what THIS plain kernel reaches on the same access pattern).  Each 16-lane half warp
+// fetches one `row_bytes`-byte row (16 bytes per lane and step, cp.async-free plain loads) at the position its index
+// entry names and xors the words into a register; one word per thread is written so the loads cannot be dropped.
+__global__ void __launch_bounds__(256)
+sp_gather_probe_kernel(const uint4* __restrict__ base, int row_bytes, long long row_pitch_bytes,
+                       const int32_t* __restrict__ idx, long long n_idx, uint32_t* __restrict__ sink) {
+  const long long half = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+  const long long n_half = ((long long)gridDim.x * blockDim.x) >> 4;
+  const int l16 = threadIdx.x & 15;
+  uint32_t acc = 0;
+  const int steps = row_bytes / 256;  // 16 lanes x 16 B per step
+  for (long long e = half; e < n_idx; e += 4 * n_half) {
+    uint4 w[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {  // four independent rows in flight per half warp
+      const long long ee = e + u * n_half;
+      const int p = ee < n_idx ? __ldg(idx + ee) : -1;
+      w[u] = make_uint4(0, 0, 0, 0);
+      if (p >= 0)
+        for (int s = 0; s < steps; ++s) {
+          const uint4 x = __ldcg(reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(base) +
+                                                               (long long)p * row_pitch_bytes) + s * 16 + l16);
+          w[u].x ^= x.x; w[u].y ^= x.y; w[u].z ^= x.z; w[u].w ^= x.w;
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) acc ^= w[u].x ^ w[u].y ^ w[u].z ^ w[u].w;
+  }
+  sink[(long long)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 }  // namespace
+
+cudaError_t sp_launch_gather_probe(const void* base, int row_bytes, long long row_pitch_bytes, const int32_t* idx,
+                                   long long n_idx, uint32_t* sink, int blocks, cudaStream_t st) {
+  sp_gather_probe_kernel<<<blocks, 256, 0, st>>>((const uint4*)base, row_bytes, row_pitch_bytes, idx, n_idx, sink);
+  sp_count_launch();
+  return cudaGetLastError();
+}
 
 cudaError_t sp_launch_overlap(const int32_t* a, const int32_t* b, long long n_rows, int k, int32_t* inter,
                               cudaStream_t st) {

@@ -72,7 +72,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   // ---- A fragments of Q: head h = row gq (< G), channels ks*16 + 2 tq (+1) and + 8 ----
   uint32_t qa[KS][2];
   {
-    const __nv_bfloat16* qr = Q + ((size_t)t * Hq + kvh * G + min(gq, G - 1)) * D;
+    const __nv_bfloat16* qr = Q + ((size_t)(t - g.q_off) * Hq + kvh * G + min(gq, G - 1)) * D;
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) {
       qa[ks][0] = gq < G ? *reinterpret_cast<const uint32_t*>(qr + ks * 16 + 2 * tq) : 0u;
@@ -84,7 +84,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   float o[NT][4];
 #pragma unroll
   for (int n = 0; n < NT; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
-  const int32_t* sup = idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)pi.row * k;
+  const int32_t* sup = idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)(pi.row - g.row_off) * k;
 
   for (int c0 = 0; c0 < k; c0 += PQ_KEYS) {
     // ---- this lane's key of the tile ----
@@ -94,13 +94,13 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       if (e >= pi.seq_start && e <= t) sp = e;
     }
     if (__ballot_sync(0xffffffffu, sp >= 0) == 0) continue;
+    const long long sp_row = sp_kv_row(g, sp >= 0 ? sp : t);  // row of this lane's key in the K / V tensors (paged or not)
     // ---- gather the 32 K rows and V rows (invalid keys: row of the query itself, masked below) ----
     __syncwarp();  // the previous tile's ldmatrix reads are done
 #pragma unroll
     for (int i = 0; i < (PQ_KEYS * CPR) / 32; ++i) {
       const int e = i * 32 + lane, r = e / CPR, c = e % CPR;
-      int pr = __shfl_sync(0xffffffffu, sp, r);
-      if (pr < 0) pr = t;
+      const long long pr = __shfl_sync(0xffffffffu, sp_row, r);
       const size_t goff = ((size_t)pr * Hkv + kvh) * D + c * 8;
       pq_cp_async16(sK_u + pq_off<D>(r, c), K + goff);
       pq_cp_async16(sV_u + pq_off<D>(r, c), V + goff);
@@ -176,7 +176,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   }
   // ---- epilogue: rows gq < G ----
   if (gq < G) {
-    const size_t orow = (size_t)t * Hq + kvh * G + gq;
+    const size_t orow = (size_t)(t - g.q_off) * Hq + kvh * G + gq;
     if (O != nullptr) {
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
       __nv_bfloat16* dst = O + orow * D + 2 * tq;
@@ -192,11 +192,10 @@ template <int D, int G>
 cudaError_t launch_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hkv,
                       float scale, int lw, float lb, int q_begin, int q_count, void* O, float* lse, cudaStream_t st) {
   const size_t smem = (size_t)PQ_WARPS * 2 * PQ_KEYS * D * 2;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static unsigned char attr_seen[SP_MAX_DEVICES];
+  if (sp_first_use_on_device(attr_seen)) {
     cudaError_t e = cudaFuncSetAttribute(sp_attn_pq_kernel<D, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_done = true;
   }
   const long long warps = (long long)q_count * Hkv;
   sp_attn_pq_kernel<D, G><<<(unsigned)((warps + PQ_WARPS - 1) / PQ_WARPS), PQ_WARPS * 32, smem, st>>>(

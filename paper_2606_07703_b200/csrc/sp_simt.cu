@@ -1,5 +1,5 @@
-// sp_simt.cu -- CUDA-core kernels of the sparse-prefill path:
-//   * indexer projection            q_idx = bf16(X Wqi), k_idx = bf16(X Wki)
+// sp_simt.cu -- CUDA-core kernels of the sparse-prefill path, used only OUTSIDE the tcgen05 kernels' built set
+// (selection blocks b_sel not in {1,32,64,128}; dense attention over a query sub-range):
 //   * indexer scoring + block max   z = idx_scale <q_idx[t],k_idx[s]>, R_B = max_t
 //   * attention mass pass 2         P_t(s) = (1/Hq) sum_h exp(z - lse), R_B = max_t PAPER.md:123, :154
 //   * warp-per-(query, KV head) attention with online softmax over a key list that is either the
@@ -9,72 +9,6 @@
 #include "sp_common.cuh"
 
 namespace {
-
-// =============================================================================================
-// Indexer projection: C[M,N] = A[M,K] * B[K,N], bf16 in, fp32 accumulate, one RNE to bf16.
-// =============================================================================================
-constexpr int PJ_BM = 64, PJ_BN = 64, PJ_BK = 32;
-
-__global__ void __launch_bounds__(256)
-sp_project_kernel(const __nv_bfloat16* __restrict__ X, const __nv_bfloat16* __restrict__ W0,
-                  const __nv_bfloat16* __restrict__ W1, __nv_bfloat16* __restrict__ C0,
-                  __nv_bfloat16* __restrict__ C1, int M, int K, int N) {
-  __shared__ float As[PJ_BK][PJ_BM + 4];
-  __shared__ float Bs[PJ_BK][PJ_BN + 4];
-  const __nv_bfloat16* W = blockIdx.z ? W1 : W0;
-  __nv_bfloat16* C = blockIdx.z ? C1 : C0;
-  const int m0 = blockIdx.x * PJ_BM, n0 = blockIdx.y * PJ_BN;
-  const int tid = threadIdx.x;
-  const int tx = tid & 15, ty = tid >> 4;  // 16 x 16 threads, 4 x 4 outputs each
-  float acc[4][4] = {};
-  for (int k0 = 0; k0 < K; k0 += PJ_BK) {
-    // A tile: 64 rows x 32 k  (each thread 8 elements = one 16-byte load)
-    {
-      const int r = tid >> 2, c = (tid & 3) * 8;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (m0 + r < M) v = *reinterpret_cast<const uint4*>(X + (size_t)(m0 + r) * K + k0 + c);
-      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        As[c + 2 * j][r] = sp_bf16lo(w[j]);
-        As[c + 2 * j + 1][r] = sp_bf16hi(w[j]);
-      }
-    }
-    // B tile: 32 k x 64 n
-    {
-      const int r = tid >> 3, c = (tid & 7) * 8;
-      const uint4 v = *reinterpret_cast<const uint4*>(W + (size_t)(k0 + r) * N + n0 + c);
-      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        Bs[r][c + 2 * j] = sp_bf16lo(w[j]);
-        Bs[r][c + 2 * j + 1] = sp_bf16hi(w[j]);
-      }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int kk = 0; kk < PJ_BK; ++kk) {
-      const float4 a = *reinterpret_cast<const float4*>(&As[kk][ty * 4]);
-      const float4 b = *reinterpret_cast<const float4*>(&Bs[kk][tx * 4]);
-      const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
-    }
-    __syncthreads();
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int m = m0 + ty * 4 + i;
-    if (m < M) {
-      uint2 o;
-      o.x = sp_pack_bf16(acc[i][0], acc[i][1]);
-      o.y = sp_pack_bf16(acc[i][2], acc[i][3]);
-      *reinterpret_cast<uint2*>(C + (size_t)m * N + n0 + tx * 4) = o;
-    }
-  }
-}
 
 // =============================================================================================
 // Score / mass kernels: thread = key, block = (128-key tile, group of query rows).
@@ -428,16 +362,6 @@ int sp_num_groups(const SpGeom& g, int row_count) {
 }
 
 }  // namespace
-
-cudaError_t sp_launch_project(const void* X, const void* Wq, const void* Wk, void* q_idx, void* k_idx, int L,
-                              int hidden, int d_idx, void* /*ws*/, cudaStream_t st) {
-  dim3 grid((L + PJ_BM - 1) / PJ_BM, d_idx / PJ_BN, 2);
-  sp_project_kernel<<<grid, 256, 0, st>>>((const __nv_bfloat16*)X, (const __nv_bfloat16*)Wq,
-                                          (const __nv_bfloat16*)Wk, (__nv_bfloat16*)q_idx, (__nv_bfloat16*)k_idx, L,
-                                          hidden, d_idx);
-  sp_count_launch();
-  return cudaGetLastError();
-}
 
 cudaError_t sp_launch_indexer_scores(const SpGeom& g, const void* q_idx, const void* k_idx, int d_idx,
                                      float idx_scale, int local_window, float local_bias, int row_begin,

@@ -7,12 +7,18 @@
 //           gathered with cp.async 16-byte vectors written in the SWIZZLE_128B image TMA would have produced;
 //   DENSE : the keys are the causal prefix of the sequence (same loader, consecutive rows), heavy chunks first.
 // Warp roles: warps 0-3 / 4-7 softmax of M tile 0 / 1 (thread = row = TMEM lane), warps 9-12 index staging +
-// Q/K/V loaders, warps 8, 13 issue the S MMAs of M tile 0 / 1 and warps 14, 15 their PV MMAs (one lane each).  Rings (K, V stages; S double buffered per M tile in TMEM)
-// run ACROSS items, so the loaders prefetch the next item's index list, K and V while the current one finishes.
+// Q/K/V loaders, warp 8 / warp 13 issue ALL MMAs of M tile 0 / 1 (PV(j) then S(j+2) from one elected lane, so the
+// tensor pipe orders them), warps 14, 15 idle.  Rings (K, V stages; S double buffered per M tile in TMEM) run ACROSS
+// items, so the loaders prefetch the next item's index list, K and V while the current one finishes.
 // Per key tile and M tile:
 //   S = Q K^T (tcgen05.mma SS, fp32 in TMEM) -> tcgen05.ld -> scale, mask by KEY POSITION VALUE, online softmax
 //   with lazy rescaling of the TMEM-resident O accumulator -> P (bf16x2) written back over S with tcgen05.st ->
 //   O += P V (tcgen05.mma with A = P from TMEM, B = V read MN-major from the row-major tile).
+// Softmax arithmetic is SPECULATIVE: the exponentials of a tile are taken against the running max as it stood before
+// the tile; unflagged tiles never reduce their max at all -- a logit more than 2^8 above the running max shows in the
+// tile's SUM of exponentials (all p >= 0), and only then is the max taken from a fresh read of S, the accumulator
+// rescaled and the tile redone (the softmax warps are issue-bound at ~2 busy warps per scheduler: instructions per
+// element are what the kernel's time is made of, profiles/r2_attn.md).
 // Only tiles that can contain a masked or locally-biased element take the per-element path (flags computed by
 // the loaders while staging the index list).
 #include "sp_common.cuh"
@@ -23,7 +29,13 @@ using namespace sptc;
 namespace {
 
 constexpr int AT_KT = 64;          // keys per tile
-constexpr int AT_MAX_STAGES = 6;   // K/V ring depth is chosen at launch from the shared-memory budget
+#ifndef AT_MAX_STAGES_DEF
+#define AT_MAX_STAGES_DEF 6
+#endif
+#ifndef AT_STORE_V8
+#define AT_STORE_V8 1  // O rows leave in 32-byte stores (one whole sector per lane and instruction: half the LSU wavefronts)
+#endif
+constexpr int AT_MAX_STAGES = AT_MAX_STAGES_DEF;   // K/V ring depth is chosen at launch from the shared-memory budget
 constexpr int AT_THREADS = 512;    // 8 softmax warps + 4 loader warps + 4 MMA-issuing warps (whole warpgroups for setmaxnreg)
 constexpr int AT_LOAD_WARPS = 4;
 constexpr int AT_MMA_WARP = 8;
@@ -94,11 +106,12 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 2.7e-6 in fp32 Horner form), exponent patched
 // in with an integer add.  Inputs are clamped to >= -125 (result ~2^-125, i.e. 0 for every use here).
 #ifndef AT_POLY_EVERY
-#define AT_POLY_EVERY 8  // one pair in AT_POLY_EVERY takes the polynomial path (0 = never)
+#define AT_POLY_EVERY 4  // one pair in AT_POLY_EVERY takes the polynomial path (0 = never)
 #endif
-#ifndef AT_SPEC
-#define AT_SPEC 1  // 1 = exponentials against the PREVIOUS running max, tile max reduced beside them (see the softmax role)
-#endif
+// fast-path overflow guard: a tile whose exponentials (taken against the running max as it stood before the tile) sum
+// to more than this is redone after the running max has been moved; every p of an accepted tile is therefore <= 2^8,
+// the bound the lazy-rescale threshold gives
+#define AT_SUM_LIMIT 256.0f
 __device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
   float x0, x1;
   f2_unpack(x2, x0, x1);
@@ -148,7 +161,7 @@ __device__ __forceinline__ bool at_item(const SpGeom& g, int id, int Hkv, int cp
   it.kvh = id % Hkv;
   const int x = id / Hkv;
   if (SPARSE) {
-    it.row = x / cpr;
+    it.row = g.row_off + x / cpr;
     const SpRow ri = sp_row_info(g, it.row);
     it.seq_start = ri.seq_start;
     it.t0 = ri.t_first + (x % cpr) * QT;
@@ -273,7 +286,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       for (int t = ptid; t < ntmax; t += 128) fl[t] = 0u;
       if (ptid == 0) n_eff_sh[ib] = 0;
       loader_bar_sync();
-      const int32_t* sup = idx + (size_t)its.kvh * (size_t)g.idx_grp + (size_t)its.row * k;
+      const int32_t* sup = idx + (size_t)its.kvh * (size_t)g.idx_grp + (size_t)(its.row - g.row_off) * k;
       const int qa0 = its.seq_start + its.t0, qa1 = qa0 + 128 / G, plast = its.seq_start + its.t1;
       int my_last = 0;
       for (int e0 = ptid; e0 < kpad; e0 += 128 * 8) {  // 8 independent loads in flight per thread
@@ -341,7 +354,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           } else {
             p = it.seq_start + min(col, it.t1);
           }
-          off[pi] = (size_t)p * rstride;
+          off[pi] = (size_t)sp_kv_row(g, p) * rstride;
         }
         if (u > 0) mbar_wait(&bar.kempty[s], (u - 1) & 1);
         const uint32_t kdst = smem_u32(sK + s * KV_TILE) + kv_off;
@@ -370,7 +383,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           mbar_expect_tx(&bar.qfull, KB * Q_BLK);
 #pragma unroll
           for (int kb = 0; kb < KB; ++kb)
-            tma_load_3d(sQ + kb * Q_BLK, &tmQ, &bar.qfull, kb * 64, it.kvh * G, it.seq_start + it.t0);
+            tma_load_3d(sQ + kb * Q_BLK, &tmQ, &bar.qfull, kb * 64, it.kvh * G, it.seq_start + it.t0 - g.q_off);
         }
         ++n_q;
       }
@@ -510,10 +523,13 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
     const int R = mt * 128 + r;
     const int ql = R / G, h = R % G;
     const uint32_t lane_base = (uint32_t)((warp % 4) * 32) << 16;
-    const uint32_t t_o = tmem + lane_base + TM_O + mt * D;
+    uint32_t t_o = tmem + lane_base + TM_O + mt * D;
     const uint64_t sl2_2 = f2_pack(sl2, sl2);
-    const uint32_t t_s0 = tmem + lane_base + TM_S + mt * 128;
-    const uint32_t a_sfull = smem_u32(&bar.sfull[mt][0]), a_sdone = smem_u32(&bar.sdone[mt][0]);  // 32-bit barrier addresses
+    uint32_t t_s0 = tmem + lane_base + TM_S + mt * 128;
+    uint32_t a_sfull = smem_u32(&bar.sfull[mt][0]), a_sdone = smem_u32(&bar.sdone[mt][0]);  // 32-bit barrier addresses
+    // Loop invariants of the key-tile loop are made opaque to the compiler: left visible, ptxas re-derives them from
+    // %tid / %cluster_ctaid in EVERY tile (S2R has tens of cycles of latency; ~60 instructions per tile went there).
+    asm volatile("" : "+r"(t_o), "+r"(t_s0), "+r"(a_sfull), "+r"(a_sdone));
     uint32_t cs = 0, n_it = 0, n_ep = 0;  // S tiles consumed by this M tile (== PVs issued for it), items seen, epilogues
     for (int i = 0; i * P < n_items; ++i) {
       const int id = at_item_id(i, cta, P, n_items);
@@ -535,12 +551,11 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       const bool row_valid = ql < nq;
       const int tl = it.t0 + min(ql, nq - 1);  // local query position of this row
       const int tp = it.seq_start + tl;        // packed
-      const size_t orow = ((size_t)tp * Hq + it.kvh * G + h);
+      const size_t orow = ((size_t)(tp - g.q_off) * Hq + it.kvh * G + h);
       const int qa_local = it.t0 + mt * (128 / G);
 
       if (mt < n_mt && my_nt > 0) {
         float m_run = -INFINITY, l_run = 0.f;
-#if AT_SPEC
         // SPECULATIVE OFFSET: the exponentials of tile j are taken against the running max as it stood BEFORE the tile,
         // while the tile's own max is reduced beside them (independent instruction chains: FMNMX3 on the ALU pipe under
         // the MUFU / FMA work), so the row max is off the critical path of the softmax warps.  Only when the tile's max
@@ -580,35 +595,25 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             tmem_ld_wait();
             const float m_off = (m_run == -INFINITY) ? 0.f : m_run;
             uint64_t sum2 = 0ull;
-            float mx;
+            float mx = -INFINITY;
             if (!flagged) {
               const uint64_t nm2 = f2_pack(-m_off, -m_off);
-              float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
 #pragma unroll
-              for (int cc = 0; cc < AT_KT; cc += 8) {
-                a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
-                a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
-                a2 = fmaxf(a2, fmaxf(__uint_as_float(v[cc + 4]), __uint_as_float(v[cc + 5])));
-                a3 = fmaxf(a3, fmaxf(__uint_as_float(v[cc + 6]), __uint_as_float(v[cc + 7])));
-#pragma unroll
-                for (int c2 = cc; c2 < cc + 8; c2 += 2) {
-                  const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[c2]), __uint_as_float(v[c2 + 1])), sl2_2, nm2);
-                  float p0, p1;
-                  if (WITH_O && AT_POLY_EVERY > 0 && (c2 / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
-                    ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
-                  } else {
-                    float x0, x1;
-                    f2_unpack(x2, x0, x1);
-                    p0 = ex2_approx(x0);
-                    p1 = ex2_approx(x1);
-                  }
-                  sum2 = f2_add(sum2, f2_pack(p0, p1));
-                  pk[c2 / 2] = bf16x2_rn(p0, p1);
+              for (int cc = 0; cc < AT_KT; cc += 2) {
+                const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2);
+                float p0, p1;
+                if (WITH_O && AT_POLY_EVERY > 0 && (cc / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
+                  ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
+                } else {
+                  float x0, x1;
+                  f2_unpack(x2, x0, x1);
+                  p0 = ex2_approx(x0);
+                  p1 = ex2_approx(x1);
                 }
+                sum2 = f2_add(sum2, f2_pack(p0, p1));
+                pk[cc / 2] = bf16x2_rn(p0, p1);
               }
-              mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
             } else {
-              mx = -INFINITY;
 #pragma unroll
               for (int cc = 0; cc < AT_KT; cc += 2) {
                 float x[2];
@@ -634,14 +639,36 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
                 pk[cc / 2] = bf16x2_rn(p0, p1);
               }
             }
-            // ---- running max with lazy rescale of the TMEM accumulator ----
-            const float m_new = fmaxf(m_run, mx);
-            const bool need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
-            if (!__any_sync(0xffffffffu, need)) {
+            {
               float s0, s1;
               f2_unpack(sum2, s0, s1);
               tsum = s0 + s1;
-              break;
+            }
+            // ---- did the running max hold?  Unflagged tiles never reduce their max: every p >= 0, so a logit more than
+            // 2^8 above the running max (or an overflow to inf) shows in the tile's SUM; only then is the max taken, from
+            // a fresh read of S.  Flagged tiles have their max from the masking pass. ----
+            bool need;
+            if (!flagged) {
+              need = !(tsum <= AT_SUM_LIMIT);
+              if (!__any_sync(0xffffffffu, need)) break;
+              uint32_t w[AT_KT];
+              tmem_ld_x32(t_s, w);
+              tmem_ld_x32(t_s + 32, w + 32);
+              tmem_ld_wait();
+              float a0 = fmaxf(__uint_as_float(w[0]), __uint_as_float(w[1]));
+              float a1 = fmaxf(__uint_as_float(w[2]), __uint_as_float(w[3]));
+#pragma unroll
+              for (int cc = 4; cc < AT_KT; cc += 4) {
+                a0 = fmaxf(a0, fmaxf(__uint_as_float(w[cc]), __uint_as_float(w[cc + 1])));
+                a1 = fmaxf(a1, fmaxf(__uint_as_float(w[cc + 2]), __uint_as_float(w[cc + 3])));
+              }
+              mx = fmaxf(a0, a1) * sl2;
+            }
+            // ---- running max with lazy rescale of the TMEM accumulator ----
+            const float m_new = fmaxf(m_run, mx);
+            if (flagged) {
+              need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
+              if (!__any_sync(0xffffffffu, need)) break;
             }
             const float f = need ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
             if (WITH_O && j > 0) {
@@ -669,121 +696,6 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           tc_fence_before_sync();
           mbar_arrive_addr(a_sdone + b * 8);
         }
-#else
-        for (int j = 0; j < my_nt; ++j, ++cs) {
-          const uint32_t b = cs & 1;
-          const uint32_t t_s = t_s0 + b * 64;
-          mbar_wait_addr(a_sfull + b * 8, (cs >> 1) & 1);
-          tc_fence_after_sync();
-          uint32_t v[AT_KT];
-          tmem_ld_x32(t_s, v);
-          tmem_ld_x32(t_s + 32, v + 32);
-          tmem_ld_wait();
-
-          bool flagged;
-          if (SPARSE) flagged = ((fl[j] >> mt) & 1u) != 0;
-          else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
-          flagged = flagged || !scale_pos;
-          float mx;
-          float xs[AT_KT];  // flagged tiles only: scaled, biased, masked logits (v itself is never written)
-          if (!flagged) {
-            float a0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1]));
-            float a1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
-            float a2 = fmaxf(__uint_as_float(v[4]), __uint_as_float(v[5]));
-            float a3 = fmaxf(__uint_as_float(v[6]), __uint_as_float(v[7]));
-#pragma unroll
-            for (int cc = 8; cc < AT_KT; cc += 8) {
-              a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
-              a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
-              a2 = fmaxf(a2, fmaxf(__uint_as_float(v[cc + 4]), __uint_as_float(v[cc + 5])));
-              a3 = fmaxf(a3, fmaxf(__uint_as_float(v[cc + 6]), __uint_as_float(v[cc + 7])));
-            }
-            mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
-          } else {
-            mx = -INFINITY;
-#pragma unroll
-            for (int cc = 0; cc < AT_KT; ++cc) {
-              const int col = j * AT_KT + cc;
-              bool ok;
-              int dist;
-              if (SPARSE) {
-                const int p = si[col];
-                ok = p >= 0 && p <= tp;
-                dist = tp - p;
-              } else {
-                ok = col <= tl;
-                dist = tl - col;
-              }
-              float x = -INFINITY;
-              if (ok) x = fmaf(__uint_as_float(v[cc]), sl2, (win > 0 && dist < win) ? lb2 : 0.f);
-              xs[cc] = x;
-              mx = fmaxf(mx, x);
-            }
-          }
-          // ---- running max with lazy rescale of the TMEM accumulator ----
-          const float m_new = fmaxf(m_run, mx);
-          const bool need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
-          if (__any_sync(0xffffffffu, need)) {
-            const float f = need ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
-            if (WITH_O && j > 0) {
-              mbar_wait(&bar.ofull[mt], (cs - 1) & 1);  // PV(j-1) has finished updating O
-              tc_fence_after_sync();
-#pragma unroll
-              for (int c0 = 0; c0 < D; c0 += 32) {
-                uint32_t o[32];
-                tmem_ld_x32(t_o + c0, o);
-                tmem_ld_wait();
-#pragma unroll
-                for (int q = 0; q < 32; ++q) o[q] = __float_as_uint(__uint_as_float(o[q]) * f);
-                tmem_st_x32(t_o + c0, o);
-              }
-              tmem_st_wait();
-            }
-            l_run *= f;
-            if (need) m_run = m_new;
-          }
-          const float m_off = (m_run == -INFINITY) ? 0.f : m_run;
-          uint32_t pk[AT_KT / 2];
-          uint64_t sum2 = 0ull;
-          if (!flagged) {
-            const uint64_t nm2 = f2_pack(-m_off, -m_off);
-#pragma unroll
-            for (int cc = 0; cc < AT_KT; cc += 2) {
-              const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2);
-              float p0, p1;
-              if (WITH_O && AT_POLY_EVERY > 0 && (cc / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
-                ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
-              } else {
-                float x0, x1;
-                f2_unpack(x2, x0, x1);
-                p0 = ex2_approx(x0);
-                p1 = ex2_approx(x1);
-              }
-              sum2 = f2_add(sum2, f2_pack(p0, p1));
-              pk[cc / 2] = bf16x2_rn(p0, p1);
-            }
-          } else {
-#pragma unroll
-            for (int cc = 0; cc < AT_KT; cc += 2) {
-              const float p0 = ex2_approx(xs[cc] - m_off);
-              const float p1 = ex2_approx(xs[cc + 1] - m_off);
-              sum2 = f2_add(sum2, f2_pack(p0, p1));
-              pk[cc / 2] = bf16x2_rn(p0, p1);
-            }
-          }
-          {
-            float s0, s1;
-            f2_unpack(sum2, s0, s1);
-            l_run += s0 + s1;
-          }
-          if (WITH_O) {
-            tmem_st_x32(t_s, pk);  // P (64 keys as 32 bf16x2 columns) over the first half of S
-            tmem_st_wait();
-          }
-          tc_fence_before_sync();
-          mbar_arrive_addr(a_sdone + b * 8);
-        }
-#endif
         // ---- epilogue ----
         if (WITH_O) {
           mbar_wait(&bar.ofin[mt], n_ep & 1);
@@ -800,6 +712,18 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
               mbar_arrive(&bar.oempty[mt]);
             }
             if (row_valid) {
+#if AT_STORE_V8
+#pragma unroll
+              for (int q = 0; q < 32; q += 16) {  // 32-byte stores: one whole sector per lane and instruction
+                uint32_t w[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e)
+                  w[e] = bf16x2_rn(__uint_as_float(o[q + 2 * e]) * inv, __uint_as_float(o[q + 2 * e + 1]) * inv);
+                asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(O + orow * D + c0 + q),
+                             "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])
+                             : "memory");
+              }
+#else
 #pragma unroll
               for (int q = 0; q < 32; q += 8) {
                 uint4 w;
@@ -809,6 +733,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
                 w.w = bf16x2_rn(__uint_as_float(o[q + 6]) * inv, __uint_as_float(o[q + 7]) * inv);
                 *reinterpret_cast<uint4*>(O + orow * D + c0 + q) = w;
               }
+#endif
             }
           }
         }
@@ -844,15 +769,7 @@ int attn_pick_stages(int kpad, bool sparse, bool with_o) {
   return s;  // < 2 -> unsupported
 }
 
-int at_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
-}
+int at_sm_count() { return sp_sm_count(); }
 
 template <int D, int G, bool SPARSE, bool WITH_O>
 cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
@@ -862,7 +779,8 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
   const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O);
   if (stages < 2) return cudaErrorInvalidValue;
   const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages);
-  static size_t attr_smem = 0;
+  static size_t attr_smem_dev[SP_MAX_DEVICES];
+  size_t& attr_smem = attr_smem_dev[sp_current_device()];
   if (smem > attr_smem) {
     cudaError_t e = cudaFuncSetAttribute(sp_tc_attn_kernel<D, G, SPARSE, WITH_O>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -872,7 +790,7 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
   const int grid = n_items < at_sm_count() ? n_items : at_sm_count();
   CUtensorMap tmQ;  // Q viewed as [L][Hq][D]: box = 256/G queries x G heads x 64 channels
   {
-    cudaError_t e = sp_make_tmap_bf16_3d(&tmQ, Q, D, (uint64_t)Hkv * G, (uint64_t)g.L, (uint64_t)D * 2,
+    cudaError_t e = sp_make_tmap_bf16_3d(&tmQ, Q, D, (uint64_t)Hkv * G, (uint64_t)(g.q_rows ? g.q_rows : g.L), (uint64_t)D * 2,
                                          (uint64_t)Hkv * G * D * 2, G, 256 / G);
     if (e != cudaSuccess) return e;
   }

@@ -184,7 +184,7 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     // affine, biased variance, eps 1e-6), then RoPE of both rows in the rotate-half pairing (i, i + DI/2) at the
     // token's LOCAL position; everything in fp32 on the fp32 accumulator, ONE rounding to bf16.
     const int mm = min(m, L - 1);
-    const int pos = mm - sp_pos_info(g, mm).seq_start;
+    const int pos = g.pos_off + mm - sp_pos_info(g, mm).seq_start;
     float mean = 0.f, rstd = 1.f;
     if (flags & SP_F_KEY_LN) {
       float sum = 0.f;
@@ -277,15 +277,7 @@ sp_tc_project_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
 // ---------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------
-static int pj_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
-}
+static int pj_sm_count() { return sp_sm_count(); }
 
 template <int DI>
 static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void* X, const void* Wq, const void* Wk,
@@ -298,11 +290,10 @@ static cudaError_t launch_project_tc(const SpGeom& g, uint32_t flags, const void
   constexpr size_t s1 = (size_t)PJ_STAGES * (128 * 128 + (2 * DI / 64) * 8192);
   constexpr size_t s2 = (size_t)(PJ_STAGES - 1) * (2 * 128 * 128 + (2 * DI / 64) * 8192);
   constexpr size_t smem = (s1 > s2 ? s1 : s2) + 1024;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static unsigned char attr_seen[SP_MAX_DEVICES];
+  if (sp_first_use_on_device(attr_seen)) {
     e = cudaFuncSetAttribute(sp_tc_project_kernel<DI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_done = true;
   }
   // 128- or 256-token CTAs (one CTA per SM): whichever needs less time by waves x tile cost, a 256-token tile costing
   // 1.45-1.85x a 128-token one (measured at 32K-128K tokens: the weights are read once per tile; 1.7 is used).

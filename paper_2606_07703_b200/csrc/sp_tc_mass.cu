@@ -404,15 +404,7 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   if (warp == 9) tmem_dealloc<512>(tmem);
 }
 
-int ms_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
-}
+int ms_sm_count() { return sp_sm_count(); }
 
 template <int D>
 cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, int grp,
@@ -434,11 +426,10 @@ cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const 
   if ((e = sp_make_tmap_bf16(&tmQ, Q, g.L, (uint64_t)Hq * D, q_pitch, MS_MQ)) != cudaSuccess) return e;
   if ((e = sp_make_tmap_bf16(&tmK, K, g.L, (uint64_t)Hkv * D, k_pitch, MS_NK)) != cudaSuccess) return e;
   constexpr size_t smem = (size_t)(D / 64) * (MS_QSTAGES * MS_MQ * 128 + 2 * MS_NK * 128) + 1024;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static unsigned char attr_seen[SP_MAX_DEVICES];
+  if (sp_first_use_on_device(attr_seen)) {
     e = cudaFuncSetAttribute(sp_tc_mass_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_done = true;
   }
   long long grid = items < ms_sm_count() ? items : ms_sm_count();
   if (grid < 1) grid = 1;

@@ -328,14 +328,29 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         for (int h = 0; h < nh; ++h)
 #pragma unroll
           for (int kb = 0; kb < KB; ++kb)
-            tma_load_2d(sQ + (h * KB + kb) * B_BYTES, &tmQ, &bar.qfull, kb * 64, su.seq_start + su.q0 + h * SC_NQ);
+            tma_load_2d(sQ + (h * KB + kb) * B_BYTES, &tmQ, &bar.qfull, kb * 64,
+                        su.seq_start + su.q0 + h * SC_NQ - g.q_off);  // chunked prefill: q_idx holds the chunk's rows only
+                                                                       // (rows before it: negative coordinate -> zero fill)
         ++n_seg;
         for (int kt = kt_lo; kt < kt_hi; ++kt) {
           mbar_wait(&bar.kempty[k_s], k_ph ^ 1);  // first pass over the ring: parity 1 of a fresh barrier passes
           mbar_expect_tx(&bar.kfull[k_s], K_STAGE);
+          if (g.bt == nullptr) {
 #pragma unroll
-          for (int kb = 0; kb < KB; ++kb)
-            tma_load_2d(sK + k_s * K_STAGE + kb * A_BYTES, &tmK, &bar.kfull[k_s], kb * 64, su.seq_start + kt * SC_KT);
+            for (int kb = 0; kb < KB; ++kb)
+              tma_load_2d(sK + k_s * K_STAGE + kb * A_BYTES, &tmK, &bar.kfull[k_s], kb * 64, su.seq_start + kt * SC_KT);
+          } else {
+            // paged indexer keys: the 128-key tile is one box inside a page (pages >= 128 tokens) or 128 / page_size
+            // boxes of one page each, landing at their row offsets of the same SWIZZLE_128B image
+            const int ps = 1 << g.page_shift;
+            const int rows = ps < SC_KT ? ps : SC_KT;
+            for (int r0 = 0; r0 < SC_KT; r0 += rows) {
+              const int y = (int)sp_kv_row(g, su.seq_start + kt * SC_KT + r0);
+#pragma unroll
+              for (int kb = 0; kb < KB; ++kb)
+                tma_load_2d(sK + k_s * K_STAGE + kb * A_BYTES + r0 * 128, &tmK, &bar.kfull[k_s], kb * 64, y);
+            }
+          }
           if (++k_s == (uint32_t)NS) {
             k_s = 0;
             k_ph ^= 1;
@@ -434,15 +449,7 @@ sp_tc_score_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
 // ---------------------------------------------------------------------------------------------------
 bool sp_tc_scores_supported(int b_sel) { return b_sel == 1 || b_sel == 32 || b_sel == 64 || b_sel == 128; }
 
-static int sc_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
-}
+static int sc_sm_count() { return sp_sm_count(); }
 
 template <int DI>
 static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const void* k_idx, float idx_scale, int lw,
@@ -450,15 +457,20 @@ static cudaError_t launch_scores_tc(const SpGeom& g, const void* q_idx, const vo
                                     float* scores, int64_t ld, cudaStream_t st) {
   CUtensorMap tmQ, tmK;
   cudaError_t e;
-  if ((e = sp_make_tmap_bf16(&tmQ, q_idx, g.L, DI, DI, SC_NQ)) != cudaSuccess) return e;
-  if ((e = sp_make_tmap_bf16(&tmK, k_idx, g.L, DI, DI, SC_KT)) != cudaSuccess) return e;
+  if ((e = sp_make_tmap_bf16(&tmQ, q_idx, g.q_rows ? g.q_rows : g.L, DI, DI, SC_NQ)) != cudaSuccess) return e;
+  if (g.bt == nullptr) {
+    e = sp_make_tmap_bf16(&tmK, k_idx, g.L, DI, DI, SC_KT);
+  } else {  // k_idx = the page pool [n_pages * page_size, DI]; box = one page, at most one 128-key tile
+    const uint64_t ps = 1ull << g.page_shift;
+    e = sp_make_tmap_bf16(&tmK, k_idx, (uint64_t)g.kv_rows, DI, DI, (uint32_t)(ps < SC_KT ? ps : SC_KT));
+  }
+  if (e != cudaSuccess) return e;
   constexpr int stages = DI == 128 ? 3 : 4;
   constexpr size_t smem = (size_t)(DI / 64) * (SC_PARTS * SC_NQ * 128 + stages * SC_KT * 128) + 1024;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static unsigned char attr_seen[SP_MAX_DEVICES];
+  if (sp_first_use_on_device(attr_seen)) {
     e = cudaFuncSetAttribute(sp_tc_score_kernel<DI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_done = true;
   }
   long long grid = units < sc_sm_count() ? units : sc_sm_count();
   if (grid < 1) grid = 1;

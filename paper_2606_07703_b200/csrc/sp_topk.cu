@@ -427,27 +427,18 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
   }
 }
 
-int g_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
-}
+int g_sm_count() { return sp_sm_count(); }
 
 }  // namespace
 
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
                            int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st) {
   if (row_count <= 0) return cudaSuccess;
-  static bool attr_done = false;
+  static unsigned char attr_seen[SP_MAX_DEVICES];
   const size_t smem = (size_t)(TK_CACHE + TK_WARPS * TK_CAND_PER_WARP) * sizeof(uint32_t);
-  if (!attr_done) {
+  if (sp_first_use_on_device(attr_seen)) {
     cudaError_t e = cudaFuncSetAttribute(sp_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_done = true;
   }
   // Row classes by n = n_valid: W = 1, 2, 4, 8 warps per row for n <= 1024 W, the 1024-thread kernel for longer rows.
   // One sequence (cu == nullptr): n(r) = min(L, (r + 1) b_sel) is monotone, each class is a contiguous row range and

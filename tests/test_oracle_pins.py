@@ -586,3 +586,82 @@ def test_per_group_equals_dense_when_budget_covers_prefix():
     idx, _ = orc.select_support_per_group(pb, Q, K, pos)
     out = orc.sparse_attn_per_group(pb, Q, K, V, pos, idx)
     assert np.allclose(out, orc.dense_attn(pb, Q, K, V, pos), rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- paged KV cache / chunked prefill
+
+def make_cache(n_ctx, ps, Hkv, d, d_idx, seed, garbage=True):
+    """An empty paged cache with a random block table; unused slots hold garbage so that a wrong page shows."""
+    n_blocks = (n_ctx + ps - 1) // ps
+    n_pages = n_blocks + 3
+    rng = np.random.Generator(np.random.Philox(seed))
+    bt = rng.permutation(n_pages)[:n_blocks].astype(np.int32)
+    fill = (lambda shape: rng.integers(0, 65536, size=shape, dtype=np.uint16)) if garbage else (lambda shape: np.zeros(shape, np.uint16))
+    return orc.PagedCache(page_size=ps, block_table=bt, k=fill((n_pages, ps, Hkv * d)), v=fill((n_pages, ps, Hkv * d)),
+                          kidx=fill((n_pages, ps, d_idx)) if d_idx else None)
+
+
+@pytest.mark.parametrize("ps", [1, 16, 64])
+def test_paged_gather_scatter_are_pure_indexing(ps):
+    n, row = 203, 24
+    rng = np.random.Generator(np.random.Philox(ps))
+    n_blocks = (n + ps - 1) // ps
+    bt = rng.permutation(n_blocks + 2)[:n_blocks].astype(np.int32)
+    cache = rng.integers(0, 65536, size=(n_blocks + 2, ps, row), dtype=np.uint16)
+    t = np.arange(37, 181)
+    want = cache[bt[t // ps], t % ps]                       # numpy fancy indexing: the definition
+    assert np.array_equal(orc.paged_gather(cache, bt, ps, 37, 181), want)
+    rows = rng.integers(0, 65536, size=(n, row), dtype=np.uint16)
+    before = cache.copy()
+    orc.paged_scatter(cache, bt, ps, 50, rows[50:120])
+    assert np.array_equal(orc.paged_gather(cache, bt, ps, 50, 120), rows[50:120])    # scatter then gather == identity
+    untouched = np.ones(cache.shape[:2], bool)
+    tt = np.arange(50, 120)
+    untouched[bt[tt // ps], tt % ps] = False
+    assert np.array_equal(cache[untouched], before[untouched])                       # and nothing else was written
+
+
+@pytest.mark.parametrize("mode,b,ps,chunk,flags", [
+    (orc.MODE_ORACLE, 1, 16, 32, 0), (orc.MODE_ORACLE, 8, 16, 40, 0),
+    (orc.MODE_INDEXER, 1, 64, 48, 0), (orc.MODE_INDEXER, 8, 16, 24, 0),
+    (orc.MODE_INDEXER, 8, 32, 56, orc.F_RELU | orc.F_KEY_LN | orc.F_ROPE),
+])
+def test_chunked_paged_prefill_equals_full_prefill(mode, b, ps, chunk, flags):
+    """Chunks of `chunk` queries, each attending the paged cache of everything before it plus itself, reproduce the
+    full-prefill supports and outputs BIT FOR BIT (the reconstruction is pure indexing; ragged last chunk and page)."""
+    L, Hq, Hkv, d, k, hid, di = 117, 4, 2, 8, 9, 16, 8
+    pb = orc.Problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=b, hidden=hid, d_idx=di, local_window=5, local_bias=0.5,
+                     flags=flags)
+    Q, K, V = rand_bf16(11, (L, Hq, d)), rand_bf16(12, (L, Hkv, d)), rand_bf16(13, (L, Hkv, d))
+    X, Wq, Wk = rand_bf16(14, (L, hid)), rand_bf16(15, (hid, di), 0.25), rand_bf16(16, (hid, di), 0.25)
+    full = orc.prefill_layer(pb, mode, Q, K, V, X, Wq, Wk)
+    outs = {}
+    for seed in (1, 2):                                   # two different block tables: the layout must not matter
+        cache = make_cache(L, ps, Hkv, d, di, seed)
+        idx_rows, out_rows = [], []
+        for q0 in range(0, L, chunk):
+            qc = min(chunk, L - q0)
+            pc = orc.Problem(L=q0 + qc, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=b, hidden=hid, d_idx=di, local_window=5,
+                             local_bias=0.5, flags=flags)
+            res = orc.prefill_chunk(pc, mode, q0, qc, Q[q0:q0 + qc], K[q0:q0 + qc], V[q0:q0 + qc], cache,
+                                    X[q0:q0 + qc], Wq, Wk)
+            assert res.rows[0] == q0 // b and np.array_equal(res.pos, np.arange(q0, q0 + qc))
+            idx_rows.append(res.idx)
+            out_rows.append(res.out)
+        idx = np.concatenate(idx_rows)
+        out = np.concatenate(out_rows)
+        assert np.array_equal(idx, full.idx)
+        assert np.array_equal(out, full.out)              # bit-identical fp64
+        outs[seed] = out
+    assert np.array_equal(outs[1], outs[2])
+
+
+def test_chunked_prefill_reads_the_cache_not_the_chunk_only():
+    """Negative control: a chunk evaluated WITHOUT its prefix in the cache (garbage pages) must differ."""
+    L, Hq, Hkv, d, k = 64, 2, 1, 8, 6
+    pb = orc.Problem(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=1)
+    Q, K, V = rand_bf16(21, (L, Hq, d)), rand_bf16(22, (L, Hkv, d)), rand_bf16(23, (L, Hkv, d))
+    full = orc.prefill_layer(pb, orc.MODE_ORACLE, Q, K, V)
+    cache = make_cache(L, 16, Hkv, d, 0, 5, garbage=False)         # prefix never written: zeros
+    res = orc.prefill_chunk(pb, orc.MODE_ORACLE, 32, 32, Q[32:], K[32:], V[32:], cache)
+    assert not np.array_equal(res.out, full.out[32:])

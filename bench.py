@@ -488,7 +488,7 @@ def measure_cold_l2(torch, step, n=8):
             "how": "256 MB device scratch fill before every step; each step timed alone with CUDA events"}
 
 
-def measure_layer_only(cfg, B, torch, gen, steps):
+def measure_layer_only(cfg, B, torch, gen, steps, chunked=None):
     """Layer latency of another workload (device-resident inputs, CUDA events, 3 warm-up steps) next to the dense
     GQA layer of the same library on the same tensors."""
     inp = gen.make_inputs(cfg)
@@ -518,9 +518,60 @@ def measure_layer_only(cfg, B, torch, gen, steps):
                                           devt["K"], devt["V"], O, idx, ws), steps, 3)
     dense_ms = timed(lambda: B.sp_dense_gqa_attn(pb, devt["Q"], devt["K"], devt["V"], O, None), 2, 1)
     causal = cfg.L * (cfg.L + 1) // 2
-    return {"config": workload_config(cfg), "ms_per_step": ms, "tokens_per_s": cfg.L / (ms * 1e-3), "steps": steps,
-            "dense_layer_ms": dense_ms, "dense_tflops": 4.0 * cfg.d * cfg.Hq * causal / (dense_ms * 1e-3) / 1e12,
-            "speedup_sparse_vs_dense": dense_ms / ms}
+    out = {"config": workload_config(cfg), "ms_per_step": ms, "tokens_per_s": cfg.L / (ms * 1e-3), "steps": steps,
+           "dense_layer_ms": dense_ms, "dense_tflops": 4.0 * cfg.d * cfg.Hq * causal / (dense_ms * 1e-3) / 1e12,
+           "speedup_sparse_vs_dense": dense_ms / ms}
+    if chunked:
+        B.sp_prefill_layer(pb, gmode, devt.get("X"), devt.get("Wqi"), devt.get("Wki"), devt["Q"], devt["K"], devt["V"],
+                           O, idx, ws)   # O again holds the SPARSE layer's output (the dense baseline wrote over it)
+        torch.cuda.synchronize()
+        del ws
+        out["chunked_paged_prefill"] = measure_chunked(cfg, B, torch, devt, O, chunks=chunked)
+    return out
+
+
+def measure_chunked(cfg, B, torch, devt, O_full, chunks=(4096, 8192), page=16):
+    """The same layer as a sequence of prefill CHUNKS against a paged KV cache (PAPER.md:292 stage 4, :331, :428:
+    max_num_batched_tokens = 4K / 8K): every chunk projects itself, appends K / V / indexer keys to 16-token pages behind
+    a shuffled block table, scores against the whole cached prefix, selects and attends THROUGH the block table.
+    Reported: the sum over all chunks (CUDA events around the whole sequence of calls) beside the one-call full
+    prefill, the last chunk alone, and whether the chunked outputs equal the full prefill bit for bit."""
+    import numpy as np
+    stream = torch.cuda.current_stream()
+    L, b = cfg.L, cfg.b_sel
+    n_blocks = (L + page - 1) // page
+    n_pages = n_blocks + 3
+    rng = np.random.Generator(np.random.Philox(12345))
+    bt = torch.from_numpy(rng.permutation(n_pages)[:n_blocks].astype(np.int32)).cuda()
+    kv = B.KvPages(torch.zeros(n_pages, page, cfg.Hkv, cfg.d, dtype=torch.bfloat16, device="cuda"),
+                   torch.zeros(n_pages, page, cfg.Hkv, cfg.d, dtype=torch.bfloat16, device="cuda"),
+                   torch.zeros(n_pages, page, cfg.d_idx, dtype=torch.bfloat16, device="cuda"), bt)
+    X, Q = devt["X"].view(L, -1), devt["Q"].view(L, cfg.Hq, cfg.d)
+    K, V = devt["K"].view(L, cfg.Hkv, cfg.d), devt["V"].view(L, cfg.Hkv, cfg.d)
+    res = {"page_size": page, "block_table": "random permutation"}
+    for chunk in chunks:
+        plans = []
+        for q0 in range(0, L, chunk):
+            qc = min(chunk, L - q0)
+            pc = B.Problem.from_config(cfg, L=q0 + qc)
+            plans.append((pc, q0, qc))
+        ws = torch.empty(max(B.chunk_workspace_bytes(pc, q0, qc) for pc, q0, qc in plans), dtype=torch.uint8, device="cuda")
+        O_c = torch.empty_like(O_full)
+
+        def run_all():
+            for pc, q0, qc in plans:
+                B.sp_prefill_chunk(pc, q0, qc, X[q0:q0 + qc], devt["Wqi"], devt["Wki"], Q[q0:q0 + qc], K[q0:q0 + qc],
+                                   V[q0:q0 + qc], kv, O_c[q0:q0 + qc], None, ws)
+
+        t_all = _timed(torch, stream, run_all, 2, warm=1)
+        pc, q0, qc = plans[-1]
+        t_last = _timed(torch, stream, lambda: B.sp_prefill_chunk(pc, q0, qc, X[q0:q0 + qc], devt["Wqi"], devt["Wki"],
+                                                                  Q[q0:q0 + qc], K[q0:q0 + qc], V[q0:q0 + qc], kv,
+                                                                  O_c[q0:q0 + qc], None, ws), 3, warm=1)
+        res[f"chunk_{chunk}"] = {"chunks": len(plans), "all_chunks_ms": t_all, "tokens_per_s": L / (t_all * 1e-3),
+                                 "last_chunk_ms": t_last, "equals_full_prefill_bitwise": bool(torch.equal(O_c, O_full))}
+        del ws, O_c
+    return res
 
 
 def main():
@@ -788,7 +839,8 @@ def main():
         # the metric is quoted at 32K and 128K: the 128K layer (BASELINE.json configs[4]) timed in the same run
         devt = host = O = O_dense = idx = ws = arena = scores = None
         torch.cuda.empty_cache()
-        line["long_context_128k"] = measure_layer_only(gen.ALL["c5"], B, torch, gen, steps=min(args.steps, 5))
+        line["long_context_128k"] = measure_layer_only(gen.ALL["c5"], B, torch, gen, steps=min(args.steps, 5),
+                                                       chunked=None if args.no_extras else (4096, 8192))
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         cb = oracle_sample_rate(cfg, inp)
         cb.pop("seconds", None)

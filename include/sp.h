@@ -191,6 +191,46 @@ int sp_prefill_layer(const sp_params *p, int32_t mode, const void *X, const void
                      const void *Q, const void *K, const void *V, void *O, int32_t *idx_out,
                      void *ws, size_t ws_bytes, void *stream);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Chunked prefill against a paged KV cache (stage 4 of the five-stage serving path: "reconstruct K/V from
+ * the paged KV cache when the chunked path requires contiguous tensors"; :331 and :428: the GPU TTFT rows run with
+ * max_num_batched_tokens = 4K / 8K query chunks against the whole cached prefix).  DESIGN.md reading A30.
+ *
+ * The cache of ONE sequence: three page pools and a block table.  Logical token t lives in page block_table[t / page_size]
+ * at slot t % page_size; a pool row is one token ([Hkv, d] bf16 for K and V, [d_idx] bf16 for the indexer keys).
+ * Pools and table are caller-owned DEVICE memory; the library writes only the slots of the tokens it is asked to append. */
+typedef struct sp_kv_pages {
+  void *k_pages;              /* [n_pages, page_size, Hkv, d] bf16                                              */
+  void *v_pages;              /* [n_pages, page_size, Hkv, d] bf16                                              */
+  void *kidx_pages;           /* [n_pages, page_size, d_idx]  bf16 (transformed indexer keys, A14/A27/A28)      */
+  const int32_t *block_table; /* [n_blocks] physical page of logical block i; n_blocks * page_size >= p->L      */
+  int32_t n_blocks;
+  int32_t page_size;          /* a power of two in [16, 4096]                                                   */
+  int32_t n_pages;
+} sp_kv_pages;
+
+/* Append / reconstruct: rows of tokens [t_begin, t_begin + t_count) <-> their page slots.  K / V rows are [Hkv, d], kidx
+ * rows [d_idx]; any of the three row pointers may be NULL (skipped).  sp_kv_gather is the paper's stage 4 as stated;
+ * sp_prefill_chunk itself never needs it -- its kernels read the pages through the block table. */
+int sp_kv_append(const sp_params *p, const sp_kv_pages *kv, int32_t t_begin, int32_t t_count, const void *K_new,
+                 const void *V_new, const void *kidx_new, void *stream);
+int sp_kv_gather(const sp_params *p, const sp_kv_pages *kv, int32_t t_begin, int32_t t_count, void *K_out, void *V_out,
+                 void *kidx_out, void *stream);
+
+/* One prefill CHUNK of one sequence, indexer mode (Alg.2 steps 2,4,5 for the queries [q_begin, q_begin + q_count)):
+ *   p->L = q_begin + q_count is the context length after the chunk; p->batch = 1, no cu_seqlens; q_begin must be a
+ *   multiple of b_sel (selection blocks stay aligned to the sequence start); b_sel in {1,32,64,128}.
+ *   X [q_count, hidden], Q [q_count, Hq, d], K_new / V_new [q_count, Hkv, d], O [q_count, Hq, d]: the CHUNK's rows only.
+ *   The first q_begin tokens must already be in the cache (earlier chunks).  The call (1) projects the chunk (rotary
+ *   positions q_begin ...), (2) appends K_new, V_new and the chunk's indexer keys to the cache, (3) scores the chunk's
+ *   support rows against all p->L cached indexer keys, (4) selects top-k, (5) runs the gather-sparse attention over the
+ *   paged K / V.  Results equal sp_prefill_layer on the whole sequence, bit for bit, for the chunk's queries.
+ *   idx_out: [ceil(q_count / b_sel), k] (the chunk's support rows) or NULL.  Workspace: sp_chunk_workspace_bytes. */
+int sp_chunk_workspace_bytes(const sp_params *p, int32_t q_begin, int32_t q_count, size_t *bytes_out);
+int sp_prefill_chunk(const sp_params *p, int32_t q_begin, int32_t q_count, const void *X, const void *Wqi,
+                     const void *Wki, const void *Q, const void *K_new, const void *V_new, const sp_kv_pages *kv,
+                     void *O, int32_t *idx_out, void *ws, size_t ws_bytes, void *stream);
+
 /* Same as sp_prefill_layer but X, Wqi, Wki, Q, K, V and O are HOST pointers (pinned memory recommended).
  * `dev_arena` is DEVICE scratch of at least sp_layer_host_arena_bytes() bytes that receives the inputs, the
  * output and the workspace.  Copies are enqueued on `stream` (cudaMemcpyAsync); O_host is valid once the

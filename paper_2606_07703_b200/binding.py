@@ -28,7 +28,8 @@ EXPORTS = (
     "sp_num_rows", "sp_workspace_bytes", "sp_indexer_scores", "sp_oracle_mass", "sp_topk_support",
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
     "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
-    "sp_oracle_mass_group", "sp_gather_probe",
+    "sp_oracle_mass_group", "sp_gather_probe", "sp_kv_append", "sp_kv_gather", "sp_chunk_workspace_bytes",
+    "sp_prefill_chunk",
 )
 
 
@@ -40,6 +41,13 @@ class SpParams(C.Structure):
         ("k", C.c_int32), ("b_sel", C.c_int32), ("hidden", C.c_int32), ("d_idx", C.c_int32),
         ("scale", C.c_float), ("idx_scale", C.c_float),
         ("local_window", C.c_int32), ("local_bias", C.c_float), ("flags", C.c_uint32),
+    ]
+
+
+class SpKvPages(C.Structure):
+    _fields_ = [
+        ("k_pages", C.c_void_p), ("v_pages", C.c_void_p), ("kidx_pages", C.c_void_p), ("block_table", C.c_void_p),
+        ("n_blocks", C.c_int32), ("page_size", C.c_int32), ("n_pages", C.c_int32),
     ]
 
 
@@ -253,6 +261,50 @@ def sp_gather_probe(base: torch.Tensor, row_bytes: int, row_pitch_bytes: int, id
     _check(lib().sp_gather_probe(_ptr(base), C.c_int32(row_bytes), C.c_int64(row_pitch_bytes), _ptr(idx),
                                  C.c_int64(idx.numel()), _ptr(sink), C.c_size_t(sink.numel() * sink.element_size()),
                                  _stream()))
+
+
+@dataclass
+class KvPages:
+    """Host-side mirror of sp_kv_pages: torch tensors of one sequence's paged cache (include/sp.h)."""
+    k_pages: torch.Tensor                 # [n_pages, page_size, Hkv, d] bf16
+    v_pages: torch.Tensor
+    kidx_pages: Optional[torch.Tensor]    # [n_pages, page_size, d_idx] bf16
+    block_table: torch.Tensor             # [n_blocks] int32, device
+
+    def c(self) -> SpKvPages:
+        return SpKvPages(self.k_pages.data_ptr(), self.v_pages.data_ptr(),
+                         self.kidx_pages.data_ptr() if self.kidx_pages is not None else None,
+                         self.block_table.data_ptr(), int(self.block_table.numel()), int(self.k_pages.shape[1]),
+                         int(self.k_pages.shape[0]))
+
+
+def sp_kv_append(pb: Problem, kv: KvPages, t_begin: int, t_count: int, K_new, V_new, kidx_new=None):
+    p, c = pb.c(), kv.c()
+    _check(lib().sp_kv_append(C.byref(p), C.byref(c), C.c_int32(t_begin), C.c_int32(t_count), _ptr(K_new), _ptr(V_new),
+                              _ptr(kidx_new), _stream()))
+
+
+def sp_kv_gather(pb: Problem, kv: KvPages, t_begin: int, t_count: int, K_out, V_out, kidx_out=None):
+    p, c = pb.c(), kv.c()
+    _check(lib().sp_kv_gather(C.byref(p), C.byref(c), C.c_int32(t_begin), C.c_int32(t_count), _ptr(K_out), _ptr(V_out),
+                              _ptr(kidx_out), _stream()))
+
+
+def chunk_workspace_bytes(pb: Problem, q_begin: int, q_count: int) -> int:
+    p = pb.c()
+    out = C.c_size_t(0)
+    _check(lib().sp_chunk_workspace_bytes(C.byref(p), C.c_int32(q_begin), C.c_int32(q_count), C.byref(out)))
+    return int(out.value)
+
+
+def sp_prefill_chunk(pb: Problem, q_begin: int, q_count: int, X, Wqi, Wki, Q, K_new, V_new, kv: KvPages, O,
+                     idx_out: Optional[torch.Tensor], ws: torch.Tensor):
+    """pb.L must be q_begin + q_count (the context length after the chunk)."""
+    p, c = pb.c(), kv.c()
+    wp, wb = _ws_args(ws)
+    _check(lib().sp_prefill_chunk(C.byref(p), C.c_int32(q_begin), C.c_int32(q_count), _ptr(X), _ptr(Wqi), _ptr(Wki),
+                                  _ptr(Q), _ptr(K_new), _ptr(V_new), C.byref(c), _ptr(O), _ptr(idx_out), wp, wb,
+                                  _stream()))
 
 
 def launch_count() -> int:

@@ -96,6 +96,37 @@ def test_null_and_misaligned_pointers_and_panels(lib):
     assert lib.sp_launch_count() == 0
 
 
+def test_chunk_api_validates_before_launching(lib):
+    """sp_prefill_chunk / sp_kv_append / sp_chunk_workspace_bytes (PAPER.md:292 stage 4, :331): documented codes, no launch."""
+    assert C.sizeof(B.SpKvPages) == 48            # 4 pointers + 3 int32 (+ 4 bytes of tail padding)
+    fake = C.c_void_p(0x1000)
+    n = None
+    def pages(**kw):
+        base = dict(k_pages=0x1000, v_pages=0x2000, kidx_pages=0x3000, block_table=0x4000, n_blocks=16, page_size=16, n_pages=32)
+        base.update(kw)
+        return B.SpKvPages(**base)
+    def chunk(pb, q0, qc, kv, ws_bytes=1 << 40, X=fake):
+        p = pb.c()
+        return lib.sp_prefill_chunk(C.byref(p), q0, qc, X, fake, fake, fake, fake, fake, C.byref(kv), fake, n, fake,
+                                    C.c_size_t(ws_bytes), n)
+    pb = P(L=256, b_sel=32)
+    assert B.chunk_workspace_bytes(pb, 128, 128) > 0
+    assert chunk(pb, 128, 128, pages(), ws_bytes=16) == B.SP_ERR_WORKSPACE
+    assert chunk(pb, 128, 100, pages()) == B.SP_ERR_INVALID_ARG            # q_begin + q_count != L
+    assert chunk(pb, 130, 126, pages()) == B.SP_ERR_INVALID_ARG            # q_begin not a multiple of b_sel
+    assert chunk(pb, 128, 128, pages(page_size=24)) == B.SP_ERR_UNSUPPORTED  # not a power of two
+    assert chunk(pb, 128, 128, pages(n_blocks=8)) == B.SP_ERR_INVALID_ARG  # table does not cover the context
+    assert chunk(pb, 128, 128, pages(kidx_pages=0)) == B.SP_ERR_INVALID_ARG
+    assert chunk(pb, 128, 128, pages(), X=n) == B.SP_ERR_INVALID_ARG
+    assert chunk(P(L=256, b_sel=16), 128, 128, pages()) == B.SP_ERR_UNSUPPORTED      # no paged reader for this block size
+    assert chunk(P(L=40, b_sel=8, cu_seqlens=[0, 19, 40]), 8, 32, pages()) == B.SP_ERR_UNSUPPORTED   # one sequence per call
+    p = pb.c()
+    kv = pages()
+    assert lib.sp_kv_append(C.byref(p), C.byref(kv), 250, 10, fake, fake, n, n) == B.SP_ERR_INVALID_ARG   # past the table
+    assert lib.sp_kv_append(C.byref(p), C.byref(kv), 0, 10, n, n, n, n) == B.SP_ERR_INVALID_ARG
+    assert lib.sp_launch_count() == 0
+
+
 def test_missing_library_fails_loudly(monkeypatch):
     monkeypatch.setattr(B, "_lib", None)
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/libsp.so")

@@ -719,3 +719,122 @@ def test_row_kl_matches_oracle():
     qi = orc.project(pbo, inp["X"], inp["Wqi"]); ki = orc.project(pbo, inp["X"], inp["Wki"], key=True)
     Zo, _ = orc.support_scores(pbo, orc.MODE_INDEXER, qi, ki, np.arange(r0, r0 + 50))
     assert np.allclose(got[:50], orc.row_kl(Ro, Zo, nvo), rtol=1e-3, atol=1e-5)
+
+
+# ------------------------------------------------------------------ f3: chunked prefill against a paged KV cache
+
+def make_gpu_cache(cfg, page_size, seed, n_ctx=None):
+    """Empty paged cache (pools filled with garbage bit patterns) with a random block table, plus its oracle twin."""
+    n_ctx = n_ctx or cfg.L
+    n_blocks = (n_ctx + page_size - 1) // page_size
+    n_pages = n_blocks + 5
+    rng = np.random.Generator(np.random.Philox(seed))
+    bt = rng.permutation(n_pages)[:n_blocks].astype(np.int32)
+    def pool(row):
+        return rng.integers(0, 0x7f00, size=(n_pages, page_size, row), dtype=np.uint16)    # finite garbage
+    kp, vp, ip = pool(cfg.Hkv * cfg.d), pool(cfg.Hkv * cfg.d), pool(cfg.d_idx)
+    ocache = orc.PagedCache(page_size=page_size, block_table=bt, k=kp.copy(), v=vp.copy(), kidx=ip.copy())
+    gcache = B.KvPages(dev(kp).view(n_pages, page_size, cfg.Hkv, cfg.d), dev(vp).view(n_pages, page_size, cfg.Hkv, cfg.d),
+                       dev(ip), torch.from_numpy(bt).to(DEV))
+    return gcache, ocache
+
+
+CHUNK_BLK = gen.shrink(gen.C3, 1100, hidden=512, k=128)                                   # b = 64, local window
+CHUNK_PQ = gen.shrink(gen.C4_SWEEP[0], 900, Hq=8, Hkv=2, hidden=256, k=64)                 # b = 1
+CHUNK_SERVED = gen.shrink(gen.C3, 1100, hidden=512, k=128, flags=SERVED)                   # RoPE: absolute positions
+
+
+@pytest.mark.parametrize("cfg,chunk,page", [(CHUNK_BLK, 256, 16), (CHUNK_BLK, 320, 64), (CHUNK_BLK, 512, 256),
+                                            (CHUNK_PQ, 200, 32), (CHUNK_SERVED, 384, 128)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_chunked_paged_prefill_equals_full_prefill(cfg, chunk, page):
+    """sp_prefill_chunk over successive chunks of one sequence, reading K / V / indexer keys through a random block
+    table, reproduces sp_prefill_layer BIT FOR BIT (PAPER.md:292 stage 4, :331); the last chunk is also checked
+    against the oracle's chunked path, and sp_kv_gather returns the appended rows exactly."""
+    inp = gen.make_inputs(cfg)
+    pbg = B.Problem.from_config(cfg)
+    L, b = cfg.L, cfg.b_sel
+    X, Wq, Wk, Q, K, V = (dev(inp[n]) for n in ("X", "Wqi", "Wki", "Q", "K", "V"))
+    O_full = torch.full((L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    idx_full = torch.full((pbg.num_rows, cfg.k), -9, dtype=torch.int32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_LAYER_INDEXER)
+    B.sp_prefill_layer(pbg, B.SP_MODE_INDEXER, X, Wq, Wk, Q, K, V, O_full, idx_full, ws)
+    gcache, ocache = make_gpu_cache(cfg, page, seed=page + chunk)
+    Xr, Qr = X.view(L, -1), Q.view(L, cfg.Hq, cfg.d)
+    Kr, Vr = K.view(L, cfg.Hkv, cfg.d), V.view(L, cfg.Hkv, cfg.d)
+    last = None
+    for q0 in range(0, L, chunk):
+        qc = min(chunk, L - q0)
+        pc = B.Problem.from_config(cfg, L=q0 + qc)
+        nr = (qc + b - 1) // b
+        O_c = torch.full((qc, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+        idx_c = torch.full((nr, cfg.k), -9, dtype=torch.int32, device=DEV)
+        wsc = torch.empty(B.chunk_workspace_bytes(pc, q0, qc), dtype=torch.uint8, device=DEV)
+        B.sp_prefill_chunk(pc, q0, qc, Xr[q0:q0 + qc].contiguous(), Wq, Wk, Qr[q0:q0 + qc].contiguous(),
+                           Kr[q0:q0 + qc].contiguous(), Vr[q0:q0 + qc].contiguous(), gcache, O_c, idx_c, wsc)
+        torch.cuda.synchronize()
+        assert torch.equal(idx_c, idx_full[q0 // b:q0 // b + nr]), q0
+        assert torch.equal(O_c.view(torch.int16), O_full[q0:q0 + qc].view(torch.int16)), q0
+        last = (q0, qc, O_c, idx_c)
+    # the cache now holds the whole sequence: the paper's stage 4 (reconstruction) returns K and V exactly
+    K_out, V_out = torch.empty_like(Kr), torch.empty_like(Vr)
+    kidx_out = torch.empty(L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
+    B.sp_kv_gather(pbg, gcache, 0, L, K_out, V_out, kidx_out)
+    assert torch.equal(K_out.view(torch.int16), Kr.view(torch.int16)) and torch.equal(V_out.view(torch.int16), Vr.view(torch.int16))
+    # oracle, chunked: earlier chunks' tokens enter the oracle's cache as the ORACLE computes them
+    pbo_full = orc_problem(cfg)
+    q0, qc, O_c, idx_c = last
+    if q0 > 0:
+        orc.paged_scatter(ocache.k, ocache.block_table, page, 0, inp["K"].reshape(L, -1)[:q0])
+        orc.paged_scatter(ocache.v, ocache.block_table, page, 0, inp["V"].reshape(L, -1)[:q0])
+        orc.paged_scatter(ocache.kidx, ocache.block_table, page, 0,
+                          orc.project(pbo_full, inp["X"], inp["Wki"], rows=np.arange(q0), key=True))
+    res = orc.prefill_chunk(pbo_full, orc.MODE_INDEXER, q0, qc, inp["Q"].reshape(L, -1)[q0:], inp["K"].reshape(L, -1)[q0:],
+                            inp["V"].reshape(L, -1)[q0:], ocache, inp["X"].reshape(L, -1)[q0:], inp["Wqi"], inp["Wki"])
+    st = parity.compare_supports(idx_c.cpu().numpy(), res.idx, res.scores, res.n_valid, cfg.k)
+    same = np.array([np.array_equal(idx_c.cpu().numpy()[orc.row_of_pos(pbo_full, int(t)) - q0 // b],
+                                    res.idx[orc.row_of_pos(pbo_full, int(t)) - q0 // b]) for t in res.pos])
+    assert same.mean() > 0.5
+    st["chained"] = parity.compare_attention(to_f64(O_c)[same], res.out[same])
+    record_stats(f"chunked:{cfg.name}:L{L}:chunk{chunk}:page{page}:b{b}", st)
+
+
+def test_chunked_prefill_last_chunk_at_128k():
+    """BASELINE.json configs[4] (L = 131072, b_sel = 128): the LAST 4096-query chunk against a paged cache of the whole
+    prefix (page 16, random block table) equals the full-prefill rows bit for bit (the full layer is checked against
+    the oracle by test_config5_long_context_sampled)."""
+    cfg = gen.C5
+    inp = cached_inputs(cfg, True)
+    pbg = B.Problem.from_config(cfg)
+    L, b, page, chunk = cfg.L, cfg.b_sel, 16, 4096
+    X, Wq, Wk, Q, K, V = (dev(inp[n]) for n in ("X", "Wqi", "Wki", "Q", "K", "V"))
+    O_full = torch.empty(L, cfg.Hq, cfg.d, dtype=torch.bfloat16, device=DEV)
+    idx_full = torch.empty(pbg.num_rows, cfg.k, dtype=torch.int32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_LAYER_INDEXER)
+    B.sp_prefill_layer(pbg, B.SP_MODE_INDEXER, X, Wq, Wk, Q, K, V, O_full, idx_full, ws)
+    del ws
+    # indexer keys of the prefix, as the library computes them
+    q_idx = torch.empty(L, cfg.d_idx, dtype=torch.bfloat16, device=DEV)
+    k_idx = torch.empty_like(q_idx)
+    sc = torch.empty(1, L, dtype=torch.float32, device=DEV)
+    wsi = B.alloc_workspace(pbg, B.SP_STAGE_INDEXER_SCORES)
+    B.sp_indexer_scores(pbg, X, Wq, Wk, q_idx, k_idx, False, 0, 1, sc, wsi)
+    n_blocks = L // page
+    n_pages = n_blocks + 7
+    rng = np.random.Generator(np.random.Philox(77))
+    bt = torch.from_numpy(rng.permutation(n_pages)[:n_blocks].astype(np.int32)).to(DEV)
+    kv = B.KvPages(torch.zeros(n_pages, page, cfg.Hkv, cfg.d, dtype=torch.bfloat16, device=DEV),
+                   torch.zeros(n_pages, page, cfg.Hkv, cfg.d, dtype=torch.bfloat16, device=DEV),
+                   torch.zeros(n_pages, page, cfg.d_idx, dtype=torch.bfloat16, device=DEV), bt)
+    q0 = L - chunk
+    B.sp_kv_append(pbg, kv, 0, q0, K, V, k_idx)
+    Xr, Qr = X.view(L, -1), Q.view(L, cfg.Hq, cfg.d)
+    Kr, Vr = K.view(L, cfg.Hkv, cfg.d), V.view(L, cfg.Hkv, cfg.d)
+    O_c = torch.empty(chunk, cfg.Hq, cfg.d, dtype=torch.bfloat16, device=DEV)
+    idx_c = torch.empty(chunk // b, cfg.k, dtype=torch.int32, device=DEV)
+    wsc = torch.empty(B.chunk_workspace_bytes(pbg, q0, chunk), dtype=torch.uint8, device=DEV)
+    B.sp_prefill_chunk(pbg, q0, chunk, Xr[q0:].contiguous(), Wq, Wk, Qr[q0:].contiguous(), Kr[q0:].contiguous(),
+                       Vr[q0:].contiguous(), kv, O_c, idx_c, wsc)
+    torch.cuda.synchronize()
+    assert torch.equal(idx_c, idx_full[q0 // b:])
+    assert torch.equal(O_c.view(torch.int16), O_full[q0:].view(torch.int16))

@@ -20,7 +20,9 @@ __device__ __forceinline__ uint32_t pq_smem_u32(const void* p) { return (uint32_
 __device__ __forceinline__ void pq_cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void pq_cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void pq_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void pq_cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void pq_ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
   asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
                : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
@@ -86,13 +88,13 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   for (int n = 0; n < NT; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
   const int32_t* sup = idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)(pi.row - g.row_off) * k;
 
+  int e_next = lane < k ? __ldg(sup + lane) : -1;  // index entries are fetched ONE TILE AHEAD (their L2 latency used to
+                                                   // sit in front of every tile's gathers)
   for (int c0 = 0; c0 < k; c0 += PQ_KEYS) {
     // ---- this lane's key of the tile ----
     int sp = -1;
-    if (c0 + lane < k) {
-      const int e = __ldg(sup + c0 + lane);
-      if (e >= pi.seq_start && e <= t) sp = e;
-    }
+    if (e_next >= pi.seq_start && e_next <= t) sp = e_next;
+    e_next = c0 + PQ_KEYS + lane < k ? __ldg(sup + c0 + PQ_KEYS + lane) : -1;
     if (__ballot_sync(0xffffffffu, sp >= 0) == 0) continue;
     const long long sp_row = sp_kv_row(g, sp >= 0 ? sp : t);  // row of this lane's key in the K / V tensors (paged or not)
     // ---- gather the 32 K rows and V rows (invalid keys: row of the query itself, masked below) ----
@@ -103,9 +105,19 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
       const long long pr = __shfl_sync(0xffffffffu, sp_row, r);
       const size_t goff = ((size_t)pr * Hkv + kvh) * D + c * 8;
       pq_cp_async16(sK_u + pq_off<D>(r, c), K + goff);
-      pq_cp_async16(sV_u + pq_off<D>(r, c), V + goff);
     }
-    pq_cp_async_wait_all();
+    pq_cp_async_commit();
+    if (O != nullptr) {
+#pragma unroll
+      for (int i = 0; i < (PQ_KEYS * CPR) / 32; ++i) {
+        const int e = i * 32 + lane, r = e / CPR, c = e % CPR;
+        const long long pr = __shfl_sync(0xffffffffu, sp_row, r);
+        const size_t goff = ((size_t)pr * Hkv + kvh) * D + c * 8;
+        pq_cp_async16(sV_u + pq_off<D>(r, c), V + goff);
+      }
+    }
+    pq_cp_async_commit();
+    pq_cp_async_wait_group<1>();  // K has landed; V keeps arriving under S = Q K^T and the softmax
     __syncwarp();
 
     // ---- S = Q K^T: 4 n tiles of 8 keys ----
@@ -155,6 +167,8 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
     l_run = l_run * corr + psum;
     m_run = m_new;
     if (O != nullptr) {
+      pq_cp_async_wait_group<0>();
+      __syncwarp();
 #pragma unroll
       for (int n = 0; n < NT; ++n) {
         o[n][0] *= corr;

@@ -9,7 +9,7 @@
 // key columns each) read it back, form exp2(sl2 * s - lse2) with packed fp32 FMAs + MUFU.EX2 and add into
 // 128 register accumulators per thread, so the head sum never leaves the register file; after the last head
 // the mean is written.  The exponential unit, not the tensor pipe, bounds this kernel (one ex2 per 2d flops).
-// Items are cut into equal contiguous ranges, one per CTA.
+// Items go to the CTAs round robin or in contiguous ranges (see ms_cta_range).
 #include "sp_common.cuh"
 #include "sp_tc.cuh"
 
@@ -53,6 +53,32 @@ __device__ __forceinline__ float ms_ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// exp2 of two fp32 values on the FMA / ALU pipes (the exponential unit bounds this kernel: one ex2 per 2 d flops, XU at
+// 60-65 % of its peak against 10 % for the FMA pipe in profiles/r2_mass_pq.md): round-to-nearest split x = n + f
+// (magic-number add), degree-4 minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 2.7e-6 in fp32 Horner
+// form, far inside the 1e-4 mass tolerance), exponent patched in with an integer add.  Inputs are clamped to >= -125.
+#ifndef MS_POLY_EVERY
+#define MS_POLY_EVERY 2  // one pair in MS_POLY_EVERY takes the polynomial path (0 = never)
+#endif
+__device__ __forceinline__ void ms_ex2_poly2(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  ms_unpack(x2, x0, x1);
+  x0 = fmaxf(x0, -125.f);
+  x1 = fmaxf(x1, -125.f);
+  const uint64_t xc = ms_pack(x0, x1);
+  const uint64_t t = ms_add2(xc, ms_pack(12582912.f, 12582912.f));  // 1.5 * 2^23
+  const uint64_t nf = ms_add2(t, ms_pack(-12582912.f, -12582912.f));
+  const uint64_t f = ms_fma2(nf, ms_pack(-1.f, -1.f), xc);
+  uint64_t q = ms_fma2(f, ms_pack(0.009570099413394928f, 0.009570099413394928f), ms_pack(0.05591785907745361f, 0.05591785907745361f));
+  q = ms_fma2(q, f, ms_pack(0.240247443318367f, 0.240247443318367f));
+  q = ms_fma2(q, f, ms_pack(0.6931217908859253f, 0.6931217908859253f));
+  q = ms_fma2(q, f, ms_pack(0.9999992847442627f, 0.9999992847442627f));
+  float q0, q1, t0, t1;
+  ms_unpack(q, q0, q1);
+  ms_unpack(t, t0, t1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
 
 struct MsTile {
   int seq_start, n, q0;  // sequence start (packed), sequence length, first LOCAL query of the 128-query tile
@@ -76,21 +102,43 @@ __device__ __forceinline__ MsTile ms_tile_info(const SpGeom& g, int qt) {
 // key tiles of a query tile: every 256-key tile that starts at or below the tile's last query
 __device__ __forceinline__ int ms_nkt(const MsTile& t) { return (min(t.q0 + MS_MQ, t.n) - 1) / MS_NK + 1; }
 
+// Work distribution over the (query tile, key tile) units of the launch, numbered query tile by query tile.
+//  * ROUND ROBIN (unit u -> CTA u mod P) for block-shared rows: the CTAs that run together then work on the same two or
+//    three query tiles, whose Q (1 MB per query tile over the Hq heads, re-read by every key tile) stays in L2.  With
+//    contiguous ranges the 148 CTAs walked 148 different query tiles at once -- 148 MB of Q -- and the all-rows launch
+//    at 32K re-read Q from DRAM (21 GB per launch, L2 hit rate 33 %): 10.7 -> 7.9 ms; one KV group: 1.51 -> 1.31 ms.
+//  * CONTIGUOUS equal ranges per CTA for per-query rows, whose launches are row panels of at most a few dozen query
+//    tiles (Q fits L2 either way) and whose units each write 128 KB of P: a CTA that stays on one query tile writes
+//    whole rows progressively, and measured 12 % faster than round robin there (profiles/r2_mass_pq.md).
 struct MsRange {
-  long long lo, hi;
+  long long lo, hi;  // contiguous mode: this CTA's units [lo, hi)
+  int rr;            // 1 = round robin
 };
-__device__ __forceinline__ MsRange ms_cta_range(const SpGeom& g, int qt_begin, int qt_count, int cta, int P) {
+__device__ __forceinline__ MsRange ms_cta_range(const SpGeom& g, int qt_begin, int qt_count, int cta, int P, int rr) {
+  MsRange r;
+  r.rr = rr;
+  r.lo = r.hi = 0;
+  if (rr) return r;
   long long U = 0;
   for (int i = 0; i < qt_count; ++i) U += ms_nkt(ms_tile_info(g, qt_begin + i));
-  MsRange r;
   r.lo = (U * cta + P - 1) / P;
   r.hi = (U * (cta + 1) + P - 1) / P;
   return r;
 }
-__device__ __forceinline__ void ms_segment(int nkt, long long B, const MsRange& r, int& kt_lo, int& kt_hi) {
-  const long long a = r.lo > B ? r.lo - B : 0, z = r.hi < B + nkt ? r.hi - B : nkt;
-  kt_lo = (int)a;
-  kt_hi = z > a ? (int)z : (int)a;
+// key tiles [kt_lo, kt_hi) step kt_step of a query tile with nkt key tiles whose first unit is number B
+__device__ __forceinline__ void ms_units(int nkt, long long B, const MsRange& r, int cta, int P, int& kt_lo, int& kt_hi,
+                                         int& kt_step) {
+  if (r.rr) {
+    const int m = (int)(B % P);
+    kt_lo = cta >= m ? cta - m : cta - m + P;
+    kt_hi = nkt;
+    kt_step = P;
+  } else {
+    const long long a = r.lo > B ? r.lo - B : 0, z = r.hi < B + nkt ? r.hi - B : nkt;
+    kt_lo = (int)a;
+    kt_hi = z > a ? (int)z : (int)a;
+    kt_step = 1;
+  }
 }
 
 // Max over the 32 lanes of a warp for 32 columns at once (reduce-scatter butterfly, 31 shuffles): on return lane l
@@ -133,7 +181,8 @@ __global__ void __launch_bounds__(MS_THREADS, 1)
 sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK, SpGeom g,
                   const float* __restrict__ lse, int lse_stride, int Hq, int Hkv, float scale, int local_window,
                   float local_bias,
-                  int row_begin, int row_count, int qt_begin, int qt_count, float* __restrict__ mass, int64_t ld) {
+                  int row_begin, int row_count, int qt_begin, int qt_count, int round_robin, float* __restrict__ mass,
+                  int64_t ld) {
   constexpr int KB = D / 64;
   constexpr uint32_t A_BYTES = MS_MQ * 128;  // per 64-wide K block: 128 queries
   constexpr uint32_t B_BYTES = MS_NK * 128;  // per 64-wide K block: 256 keys
@@ -169,7 +218,7 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem = tmem_slot;
-  const MsRange rg = ms_cta_range(g, qt_begin, qt_count, blockIdx.x, gridDim.x);
+  const MsRange rg = ms_cta_range(g, qt_begin, qt_count, blockIdx.x, gridDim.x, round_robin);
 
   if (warp >= 10) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
@@ -182,10 +231,10 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       for (int i = 0; i < qt_count; ++i) {
         const MsTile ti = ms_tile_info(g, qt_begin + i);
         const int nkt = ms_nkt(ti);
-        int kt_lo, kt_hi;
-        ms_segment(nkt, B, rg, kt_lo, kt_hi);
+        int kt_lo, kt_hi, kt_step;
+        ms_units(nkt, B, rg, (int)blockIdx.x, (int)gridDim.x, kt_lo, kt_hi, kt_step);
         B += nkt;
-        for (int kt = kt_lo; kt < kt_hi; ++kt) {
+        for (int kt = kt_lo; kt < kt_hi; kt += kt_step) {
           for (int h = 0; h < Hq; ++h) {
             if (h % G == 0) {
               const uint32_t kb_i = k_n & 1;
@@ -223,10 +272,10 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     for (int i = 0; i < qt_count; ++i) {
       const MsTile ti = ms_tile_info(g, qt_begin + i);
       const int nkt = ms_nkt(ti);
-      int kt_lo, kt_hi;
-      ms_segment(nkt, B, rg, kt_lo, kt_hi);
+      int kt_lo, kt_hi, kt_step;
+      ms_units(nkt, B, rg, (int)blockIdx.x, (int)gridDim.x, kt_lo, kt_hi, kt_step);
       B += nkt;
-      for (int kt = kt_lo; kt < kt_hi; ++kt) {
+      for (int kt = kt_lo; kt < kt_hi; kt += kt_step) {
         for (int h = 0; h < Hq; ++h, ++hc) {
           if (h % G == 0) {
             mbar_wait(&bar.kfull[k_n & 1], (k_n >> 1) & 1);
@@ -273,15 +322,15 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     for (int i = 0; i < qt_count; ++i) {
       const MsTile ti = ms_tile_info(g, qt_begin + i);
       const int nkt = ms_nkt(ti);
-      int kt_lo, kt_hi;
-      ms_segment(nkt, B, rg, kt_lo, kt_hi);
+      int kt_lo, kt_hi, kt_step;
+      ms_units(nkt, B, rg, (int)blockIdx.x, (int)gridDim.x, kt_lo, kt_hi, kt_step);
       B += nkt;
       const int tl = ti.q0 + r;                      // local query of this thread
       const bool t_ok = tl < ti.n;
       const int tw0 = ti.q0 + wq * 32;               // warp-uniform: first / last valid query of the warp
       const int tw1 = min(tw0 + 31, ti.n - 1);
       const float* lse_row = lse + (size_t)(ti.seq_start + min(tl, ti.n - 1)) * lse_stride;
-      for (int kt = kt_lo; kt < kt_hi; ++kt) {
+      for (int kt = kt_lo; kt < kt_hi; kt += kt_step) {
         const int sc0 = kt * MS_NK + e * 128;  // local key of this warpgroup's column 0
         uint64_t acc[64];
 #pragma unroll
@@ -312,9 +361,17 @@ sp_tc_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               // interior chunk: every pair causal, outside the local window, every query valid
 #pragma unroll
               for (int j = 0; j < 32; j += 2) {
-                float x0, x1;
-                ms_unpack(ms_fma2(ms_pack(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), sl2_2, nl2), x0, x1);
-                acc[(c0 + j) >> 1] = ms_add2(acc[(c0 + j) >> 1], ms_pack(ms_ex2(x0), ms_ex2(x1)));
+                const uint64_t x2 = ms_fma2(ms_pack(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), sl2_2, nl2);
+                float p0, p1;
+                if (MS_POLY_EVERY > 0 && (j / 2) % MS_POLY_EVERY == MS_POLY_EVERY - 1) {
+                  ms_ex2_poly2(x2, p0, p1);
+                } else {
+                  float x0, x1;
+                  ms_unpack(x2, x0, x1);
+                  p0 = ms_ex2(x0);
+                  p1 = ms_ex2(x1);
+                }
+                acc[(c0 + j) >> 1] = ms_add2(acc[(c0 + j) >> 1], ms_pack(p0, p1));
               }
             } else {
 #pragma unroll
@@ -433,9 +490,10 @@ cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const 
   }
   long long grid = items < ms_sm_count() ? items : ms_sm_count();
   if (grid < 1) grid = 1;
+  const int rr = g.b_sel > 1 ? 1 : 0;
   sp_tc_mass_kernel<D><<<(unsigned)grid, MS_THREADS, smem, st>>>(tmQ, tmK, g, lse, lse_stride, Hq, Hkv, scale, lw, lb,
                                                                 row_begin,
-                                                                row_count, qt_begin, qt_count, mass, ld);
+                                                                row_count, qt_begin, qt_count, rr, mass, ld);
   sp_count_launch();
   return cudaGetLastError();
 }

@@ -416,6 +416,26 @@ def measure_oracle_mode(cfg, B, torch, devt, peaks, reps=2):
                           "frac_of_burst_peak": fl / (t_p2 * 1e-3) / 1e12 / peaks["tensor_burst"],
                           "panel_rows": [r0, r0 + panel], "scaled_by_rows": n_rows / panel},
            "config": f"{cfg.name} shape, SP_MODE_ORACLE, b_sel={cfg.b_sel}, k={cfg.k}"}
+    # head-axis support granularities: one list per KV group / per query head, selected by
+    # the SAME call from one pass 1 (SP_F_GROUP_SUPPORT / SP_F_HEAD_SUPPORT)
+    del mass
+    for name, flag, units in (("per_kv_group", B.SP_F_GROUP_SUPPORT, cfg.Hkv), ("per_head", B.SP_F_HEAD_SUPPORT, cfg.Hq)):
+        pbu = B.Problem.from_config(cfg, flags=flag)
+        idx_u = torch.empty(units, n_rows, cfg.k, dtype=torch.int32, device="cuda")
+        ws_u = B.alloc_workspace(pbu, B.SP_STAGE_LAYER_ORACLE)
+        t_u = _timed(torch, stream, lambda: B.sp_prefill_layer(pbu, B.SP_MODE_ORACLE, None, None, None, devt["Q"], devt["K"],
+                                                               devt["V"], O, idx_u, ws_u), 1 if name == "per_head" else reps)
+        inter = torch.empty(n_rows, dtype=torch.int32, device="cuda")
+        agree = []
+        hpl = cfg.Hq // units          # heads per list
+        for u in range(0, units, max(1, units // 4)):
+            B.sp_support_overlap(pb, idx, idx_u[u], inter)
+            agree.append(float(inter.sum().item()) / float((idx >= 0).sum().item()))
+        out[name] = {"layer_ms": t_u, "lists": units, "heads_per_list": hpl,
+                     "overlap_with_head_averaged_support_sampled_lists": agree,
+                     "attention_kernel": "tcgen05 block-shared (a KV group's heads share every gathered row)" if name == "per_kv_group"
+                     else "mma.sync per-query tile shape (no two heads share a gathered row)"}
+        del ws_u, idx_u
     return out
 
 

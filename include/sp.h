@@ -44,7 +44,8 @@ extern "C" {
 typedef enum sp_status {
   SP_OK = 0,
   SP_ERR_INVALID_ARG = -1, /* null / misaligned pointer, nonpositive size, Hq % Hkv, bad cu_seqlens, bad panel */
-  SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}, Hq/Hkv not in {1,2,4,8}, unknown flag bits ...) */
+  SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}: the Qwen3.5 head dim 256 / d_idx 256 rows of
+                              PAPER.md:280 are NOT built; Hq/Hkv not in {1,2,4,8}; unknown flag bits ...)              */
   SP_ERR_WORKSPACE = -3,   /* workspace too small (see sp_workspace_bytes)                                      */
   SP_ERR_CUDA = -4         /* a CUDA launch / API error; text via sp_strerror                                   */
 } sp_status;
@@ -90,12 +91,18 @@ typedef struct sp_params {
  *   SP_F_RELU   : z = max(idx_scale <q_idx, k_idx> + local term, 0)
  * KEY_LN and ROPE act in the projection (q_idx / k_idx come out transformed, rounded once to bf16; with
  * preprojected = 1 the caller's tensors are taken as already transformed); RELU acts in the score epilogue. */
-enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u, SP_F_GROUP_SUPPORT = 8u };
-/* SP_F_GROUP_SUPPORT ("shared within each KV group S_{l,t,r}"; A29) is read by
- * sp_sparse_gqa_attn ONLY: idx is then [Hkv, n_rows, k] -- one support list per KV group and support row, each
- * list as described under "idx" below -- and query head h attends the list of group g(h).  Every other entry
- * point returns SP_ERR_UNSUPPORTED when the bit is set; the lists themselves come from sp_oracle_mass_group +
- * sp_topk_support (one call pair per KV group). */
+enum { SP_F_RELU = 1u, SP_F_KEY_LN = 2u, SP_F_ROPE = 4u, SP_F_GROUP_SUPPORT = 8u, SP_F_HEAD_SUPPORT = 16u };
+/* Support granularity on the HEAD axis ("shared within each KV group S_{l,t,r}" / "separately per query
+ * head S_{l,t,h}"; the paper evaluates neither, :133, :137; A29).  Default (neither bit): ONE head-averaged list
+ * per support row.
+ *   SP_F_GROUP_SUPPORT: one list per KV group; index tensors are [Hkv, n_rows, k]; group r's mass is the mean over ITS
+ *     G = Hq/Hkv query heads, P_r[t,s] = (1/G) sum_{g(h)=r} A[t,h,s].
+ *   SP_F_HEAD_SUPPORT : one list per query head; index tensors are [Hq, n_rows, k]; head h's mass is A[t,h,s] itself.
+ * Everything else (block max, top-k, tie rule, recompute) is the head-averaged definition on the sub-problem.  The bits
+ * are read by sp_sparse_gqa_attn (layout of idx) and by sp_prefill_layer in SP_MODE_ORACLE (which then selects Hkv or Hq
+ * lists from ONE pass 1 and attends with them); every other entry point returns SP_ERR_UNSUPPORTED when one is set, and
+ * both together are SP_ERR_INVALID_ARG.  Per-head lists leave no two heads a shared gathered row, so the attention runs
+ * on the per-query kernel's tile shape for every b_sel. */
 
 /* Number of support rows of the whole pack (host arithmetic only). Returns < 0 on invalid params. */
 int64_t sp_num_rows(const sp_params *p);
@@ -138,6 +145,11 @@ int sp_oracle_mass(const sp_params *p, const void *Q, const void *K, float *lse,
 int sp_oracle_mass_group(const sp_params *p, const void *Q, const void *K, float *lse, int32_t lse_ready,
                          int32_t group, int32_t row_begin, int32_t row_count, float *mass, int64_t ld_mass,
                          void *ws, size_t ws_bytes, void *stream);
+/* The same for ONE query head ("separately per query head S_{l,t,h}"): mass = A[t,head,s] (block max for
+ * b_sel > 1).  head outside [0,Hq) -> SP_ERR_INVALID_ARG. */
+int sp_oracle_mass_head(const sp_params *p, const void *Q, const void *K, float *lse, int32_t lse_ready,
+                        int32_t head, int32_t row_begin, int32_t row_count, float *mass, int64_t ld_mass,
+                        void *ws, size_t ws_bytes, void *stream);
 
 /* Causal top-k of each support row of the panel (PAPER.md:127 TopK_s(P,k); :145 sentinel padding; :156
  * causally invalid positions masked before selection).  Row r ranks columns [0, n_valid(r)) of
@@ -186,7 +198,9 @@ int sp_gather_probe(const void *base, int32_t row_bytes, int64_t row_pitch_bytes
  * 2-5 in SP_MODE_ORACLE, Alg.2 steps 2,4,5 in SP_MODE_INDEXER).  Support rows are processed in panels so the
  * score workspace stays bounded.
  *   X, Wqi, Wki: indexer mode only (ignored in oracle mode).  O: [L,Hq,d] bf16.
- *   idx_out: [sp_num_rows(p), k] int32 or NULL (then the indices live in the workspace). */
+ *   idx_out: [sp_num_rows(p), k] int32 or NULL (then the indices live in the workspace); with SP_F_GROUP_SUPPORT /
+ *   SP_F_HEAD_SUPPORT (oracle mode) [Hkv or Hq, sp_num_rows(p), k], and sp_workspace_bytes(SP_STAGE_LAYER_ORACLE)
+ *   accounts for those lists when the same flags are set in the params it is given. */
 int sp_prefill_layer(const sp_params *p, int32_t mode, const void *X, const void *Wqi, const void *Wki,
                      const void *Q, const void *K, const void *V, void *O, int32_t *idx_out,
                      void *ws, size_t ws_bytes, void *stream);

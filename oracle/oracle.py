@@ -340,6 +340,49 @@ def sparse_attn_per_group(pb: Problem, Q, K, V, pos, sup):
     return out
 
 
+# ---------------------------------------------------------------- per-head support ("separately per query head")
+# S_{l,t,h}: head h's own attention distribution A[t,h,.] is its mass (the head "mean" over one head); block max, top-k,
+# tie rule and recompute as for the head-averaged support -- the head-averaged definition on the sub-problem
+# (Q[:, h], K[:, g(h)], V[:, g(h)]) with Hq' = Hkv' = 1.  The paper names the variant and evaluates none (:133, :137).
+
+def _head_problem(pb: Problem) -> Problem:
+    return Problem(L=pb.L, Hq=1, Hkv=1, d=pb.d, k=pb.k, b_sel=pb.b_sel, scale=pb.scale,
+                   local_window=pb.local_window, local_bias=pb.local_bias, cu_seqlens=pb.cu_seqlens)
+
+
+def _head_slices(pb: Problem, Q, K, V, h: int):
+    G = pb.Hq // pb.Hkv
+    Q = _u16(Q).reshape(pb.L, pb.Hq, pb.d)
+    K = _u16(K).reshape(pb.L, pb.Hkv, pb.d)
+    V = _u16(V).reshape(pb.L, pb.Hkv, pb.d) if V is not None else None
+    r = h // G                                                   # g(h), A5
+    return (np.ascontiguousarray(Q[:, h:h + 1]), np.ascontiguousarray(K[:, r:r + 1]),
+            np.ascontiguousarray(V[:, r:r + 1]) if V is not None else None)
+
+
+def select_support_per_head(pb: Problem, Q, K, rows):
+    """Oracle-mode supports per query head: idx [Hq, len(rows), k], cnt [Hq, len(rows)]."""
+    hp = _head_problem(pb)
+    idx, cnt = [], []
+    for h in range(pb.Hq):
+        Qh, Kh, _ = _head_slices(pb, Q, K, None, h)
+        _, _, i, c = select_support(hp, MODE_ORACLE, Qh, Kh, rows)
+        idx.append(i)
+        cnt.append(c)
+    return np.stack(idx), np.stack(cnt)
+
+
+def sparse_attn_per_head(pb: Problem, Q, K, V, pos, sup):
+    """O6 with one support per head: sup [Hq, len(pos), k]; head h attends S_{r(t), h}."""
+    hp = _head_problem(pb)
+    pos = _i32(pos)
+    out = np.empty((len(pos), pb.Hq, pb.d), dtype=np.float64)
+    for h in range(pb.Hq):
+        Qh, Kh, Vh = _head_slices(pb, Q, K, V, h)
+        out[:, h:h + 1] = sparse_attn(hp, Qh, Kh, Vh, pos, sup[h])
+    return out
+
+
 # ---------------------------------------------------------------- chunked prefill against a paged KV cache
 # PAPER.md:292 (five-stage serving path, stage 4 "reconstruct K/V from the paged KV cache when the chunked path requires
 # contiguous tensors"), :331 and :428 (chunks of max_num_batched_tokens = 4K / 8K queries against the whole prefix).

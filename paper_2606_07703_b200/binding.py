@@ -20,7 +20,8 @@ LIB_PATH = os.path.join(_HERE, "libsp.so")
 SP_OK, SP_ERR_INVALID_ARG, SP_ERR_UNSUPPORTED, SP_ERR_WORKSPACE, SP_ERR_CUDA = 0, -1, -2, -3, -4
 SP_MODE_ORACLE, SP_MODE_INDEXER = 0, 1
 SP_F_RELU, SP_F_KEY_LN, SP_F_ROPE = 1, 2, 4   # sp_params.flags: the served scorer of PAPER.md:270-274
-SP_F_GROUP_SUPPORT = 8                        # sp_sparse_gqa_attn only: idx is [Hkv, n_rows, k]
+SP_F_GROUP_SUPPORT = 8                        # idx is [Hkv, n_rows, k]: one list per KV group
+SP_F_HEAD_SUPPORT = 16                        # idx is [Hq, n_rows, k]: one list per query head
 (SP_STAGE_INDEXER_SCORES, SP_STAGE_ORACLE_MASS, SP_STAGE_TOPK, SP_STAGE_SPARSE_ATTN, SP_STAGE_DENSE_ATTN,
  SP_STAGE_LAYER_ORACLE, SP_STAGE_LAYER_INDEXER) = range(7)
 
@@ -29,7 +30,7 @@ EXPORTS = (
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
     "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
     "sp_oracle_mass_group", "sp_gather_probe", "sp_kv_append", "sp_kv_gather", "sp_chunk_workspace_bytes",
-    "sp_prefill_chunk",
+    "sp_prefill_chunk", "sp_oracle_mass_head",
 )
 
 
@@ -196,6 +197,15 @@ def sp_oracle_mass_group(pb: Problem, Q, K, lse: Optional[torch.Tensor], lse_rea
                                       C.c_int64(mass.stride(0)), wp, wb, _stream()))
 
 
+def sp_oracle_mass_head(pb: Problem, Q, K, lse: Optional[torch.Tensor], lse_ready: bool, head: int, row_begin: int,
+                        row_count: int, mass: torch.Tensor, ws: Optional[torch.Tensor] = None):
+    p = pb.c()
+    wp, wb = _ws_args(ws)
+    _check(lib().sp_oracle_mass_head(C.byref(p), _ptr(Q), _ptr(K), _ptr(lse), C.c_int32(1 if lse_ready else 0),
+                                     C.c_int32(head), C.c_int32(row_begin), C.c_int32(row_count), _ptr(mass),
+                                     C.c_int64(mass.stride(0)), wp, wb, _stream()))
+
+
 def sp_topk_support(pb: Problem, scores: torch.Tensor, row_begin: int, row_count: int, idx: torch.Tensor,
                     cnt: Optional[torch.Tensor] = None, ws: Optional[torch.Tensor] = None):
     p = pb.c()
@@ -207,9 +217,15 @@ def sp_topk_support(pb: Problem, scores: torch.Tensor, row_begin: int, row_count
 def sp_sparse_gqa_attn(pb: Problem, Q, K, V, idx, O, lse: Optional[torch.Tensor] = None,
                        ws: Optional[torch.Tensor] = None):
     p = pb.c()
-    if idx.dim() == 3:   # one support list per KV group: [Hkv, n_rows, k]
-        assert idx.shape[0] == pb.Hkv and idx.is_contiguous(), idx.shape
-        p.flags |= SP_F_GROUP_SUPPORT
+    if idx.dim() == 3:   # one support list per KV group [Hkv, n_rows, k] or per head [Hq, n_rows, k]
+        assert idx.is_contiguous(), "index tensors crossing the ABI must be contiguous"
+        p.flags &= ~(SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)
+        if pb.flags & SP_F_HEAD_SUPPORT or (idx.shape[0] == pb.Hq and pb.Hq != pb.Hkv):
+            assert idx.shape[0] == pb.Hq, idx.shape
+            p.flags |= SP_F_HEAD_SUPPORT
+        else:
+            assert idx.shape[0] == pb.Hkv, idx.shape
+            p.flags |= SP_F_GROUP_SUPPORT
     wp, wb = _ws_args(ws)
     _check(lib().sp_sparse_gqa_attn(C.byref(p), _ptr(Q), _ptr(K), _ptr(V), _ptr(idx), _ptr(O), _ptr(lse), wp, wb,
                                     _stream()))

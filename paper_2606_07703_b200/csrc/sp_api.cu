@@ -131,12 +131,12 @@ cudaError_t run_indexer_scores(const sp_params* p, const void* q_idx, const void
 }
 
 cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const float* lse, int row_begin, int row_count,
-                     int max_nv, float* mass, int64_t ld, cudaStream_t st, int grp = -1) {
+                     int max_nv, float* mass, int64_t ld, cudaStream_t st, int grp = -1, int head = -1) {
   const SpGeom g = dev_geom(p);
   if (sp_tc_mass_supported(p->b_sel, p->d))
     return sp_launch_mass_tc(g, p->cu_seqlens ? p->cu_seqlens_host : nullptr, Q, K, lse, p->Hq, p->Hkv, p->d,
-                             attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st, grp);
-  if (grp >= 0) return cudaErrorNotSupported;  // callers check sp_tc_mass_supported first
+                             attn_scale(p), p->local_window, p->local_bias, row_begin, row_count, mass, ld, st, grp, head);
+  if (grp >= 0 || head >= 0) return cudaErrorNotSupported;  // callers check sp_tc_mass_supported first
   return sp_launch_mass(g, Q, K, lse, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias, row_begin,
                         row_count, max_nv, mass, ld, st);
 }
@@ -145,9 +145,12 @@ cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const flo
 // the oracle's pass 1 of a row panel) -- the query chunks that intersect [q_begin, q_begin + q_count): rows of a
 // boundary chunk outside the range get their lse too, which is harmless.
 cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
-                     int q_count, void* O, float* lse, cudaStream_t st, long long idx_grp = 0) {
+                     int q_count, void* O, float* lse, cudaStream_t st, long long idx_grp = 0, bool per_head = false) {
   SpGeom g = dev_geom(p);
   g.idx_grp = idx_grp;
+  if (per_head)  // one list per HEAD: no two heads share gathered rows, the per-query kernel's tile shape (G = 1 rows per warp)
+    return sp_launch_attn_pq(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
+                             q_begin, q_count, O, lse, st, true);
   const int G = p->Hq / p->Hkv;
   const bool whole = q_begin == 0 && q_count == p->L;
   const bool dense_lse_range = idx == nullptr && O == nullptr && q_count > 0;
@@ -192,7 +195,7 @@ struct LayerPlan {
   size_t off_qidx, off_kidx, off_lse, off_scores, off_idx, off_stage, total;
 };
 
-LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws) {
+LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws, int units = 1) {
   LayerPlan pl{};
   const HostGeom hg = host_geom(p);
   pl.n_rows = hg.num_rows();
@@ -212,9 +215,20 @@ LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws) {
   }
   pl.off_scores = off; off += align_up((size_t)pl.panel_rows * pl.ld * sizeof(float));
   pl.off_idx = off;
-  if (idx_in_ws) off += align_up((size_t)pl.n_rows * p->k * sizeof(int32_t));
+  if (idx_in_ws) off += align_up((size_t)units * pl.n_rows * p->k * sizeof(int32_t));
   pl.total = off;
   return pl;
+}
+
+// number of support lists per support row the layer call selects: 1, Hkv (SP_F_GROUP_SUPPORT) or Hq (SP_F_HEAD_SUPPORT);
+// negative = an sp_status
+int layer_units(const sp_params* p, int mode) {
+  const uint32_t gf = p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT);
+  if (gf == 0) return 1;
+  if (gf == (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)) return SP_ERR_INVALID_ARG;
+  if (mode != SP_MODE_ORACLE) return SP_ERR_UNSUPPORTED;
+  if (p->Hq < 1 || p->Hkv < 1) return SP_ERR_INVALID_ARG;
+  return gf == SP_F_GROUP_SUPPORT ? p->Hkv : p->Hq;
 }
 
 }  // namespace
@@ -263,6 +277,15 @@ int sp_workspace_bytes(const sp_params* p, int stage, size_t* bytes_out) {
   if (!bytes_out) return SP_ERR_INVALID_ARG;
   const bool idxr = stage == SP_STAGE_INDEXER_SCORES || stage == SP_STAGE_LAYER_INDEXER;
   const bool attn = stage != SP_STAGE_INDEXER_SCORES && stage != SP_STAGE_TOPK;
+  int units = 1;
+  sp_params pq;
+  if (p && stage == SP_STAGE_LAYER_ORACLE && (p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT))) {
+    units = layer_units(p, SP_MODE_ORACLE);
+    if (units < 0) return units;
+    pq = *p;
+    pq.flags &= ~(uint32_t)(SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT);
+    p = &pq;
+  }
   const int rc = validate_common(p, attn, idxr);
   if (rc != SP_OK) return rc;
   switch (stage) {
@@ -271,7 +294,7 @@ int sp_workspace_bytes(const sp_params* p, int stage, size_t* bytes_out) {
     case SP_STAGE_TOPK:
     case SP_STAGE_SPARSE_ATTN:
     case SP_STAGE_DENSE_ATTN: *bytes_out = 0; return SP_OK;
-    case SP_STAGE_LAYER_ORACLE: *bytes_out = plan_layer(p, SP_MODE_ORACLE, true).total; return SP_OK;
+    case SP_STAGE_LAYER_ORACLE: *bytes_out = plan_layer(p, SP_MODE_ORACLE, true, units).total; return SP_OK;
     case SP_STAGE_LAYER_INDEXER: *bytes_out = plan_layer(p, SP_MODE_INDEXER, true).total; return SP_OK;
   }
   return SP_ERR_INVALID_ARG;
@@ -297,12 +320,12 @@ int sp_indexer_scores(const sp_params* p, const void* X, const void* Wqi, const 
 }
 
 static int oracle_mass_impl(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int grp,
-                            int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws,
+                            int head, int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws,
                             size_t ws_bytes, void* stream) {
   int rc = validate_common(p, true, false);
   if (rc != SP_OK) return rc;
-  if (grp >= p->Hkv) return SP_ERR_INVALID_ARG;
-  if (grp >= 0 && !sp_tc_mass_supported(p->b_sel, p->d)) return SP_ERR_UNSUPPORTED;
+  if (grp >= p->Hkv || head >= p->Hq) return SP_ERR_INVALID_ARG;
+  if ((grp >= 0 || head >= 0) && !sp_tc_mass_supported(p->b_sel, p->d)) return SP_ERR_UNSUPPORTED;
   if (!Q || !K || !mass || !aligned16(Q) || !aligned16(K) || !aligned16(mass)) return SP_ERR_INVALID_ARG;
   if (lse_ready && !lse) return SP_ERR_INVALID_ARG;
   int max_nv = 0;
@@ -337,20 +360,27 @@ static int oracle_mass_impl(const sp_params* p, const void* Q, const void* K, fl
     }
     SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, q_lo, q_hi - q_lo + 1, nullptr, lse, st), "mass pass 1 (lse)");
   }
-  SP_CUDA(run_mass(p, Q, K, lse, row_begin, row_count, max_nv, mass, ld_mass, st, grp), "mass pass 2");
+  SP_CUDA(run_mass(p, Q, K, lse, row_begin, row_count, max_nv, mass, ld_mass, st, grp, head), "mass pass 2");
   return SP_OK;
 }
 
 int sp_oracle_mass(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t row_begin,
                    int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes, void* stream) {
-  return oracle_mass_impl(p, Q, K, lse, lse_ready, -1, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
+  return oracle_mass_impl(p, Q, K, lse, lse_ready, -1, -1, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
 }
 
 int sp_oracle_mass_group(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t group,
                          int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes,
                          void* stream) {
   if (group < 0) return SP_ERR_INVALID_ARG;
-  return oracle_mass_impl(p, Q, K, lse, lse_ready, group, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
+  return oracle_mass_impl(p, Q, K, lse, lse_ready, group, -1, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
+}
+
+int sp_oracle_mass_head(const sp_params* p, const void* Q, const void* K, float* lse, int32_t lse_ready, int32_t head,
+                        int32_t row_begin, int32_t row_count, float* mass, int64_t ld_mass, void* ws, size_t ws_bytes,
+                        void* stream) {
+  if (head < 0) return SP_ERR_INVALID_ARG;
+  return oracle_mass_impl(p, Q, K, lse, lse_ready, -1, head, row_begin, row_count, mass, ld_mass, ws, ws_bytes, stream);
 }
 
 int sp_topk_support(const sp_params* p, const float* scores, int64_t ld_scores, int32_t row_begin, int32_t row_count,
@@ -404,14 +434,17 @@ int sp_gather_probe(const void* base, int32_t row_bytes, int64_t row_pitch_bytes
 int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
                        float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
   if (!p) return SP_ERR_INVALID_ARG;
-  sp_params q = *p;  // SP_F_GROUP_SUPPORT belongs to this entry point only: every other one rejects it as unknown
-  q.flags &= ~(uint32_t)SP_F_GROUP_SUPPORT;
+  sp_params q = *p;  // the support-granularity flags belong to this entry point and to sp_prefill_layer's oracle mode
+  q.flags &= ~(uint32_t)(SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT);
+  if ((p->flags & SP_F_GROUP_SUPPORT) && (p->flags & SP_F_HEAD_SUPPORT)) return SP_ERR_INVALID_ARG;
   const int rc = validate_common(&q, true, false);
   if (rc != SP_OK) return rc;
   if (!Q || !K || !V || !idx || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
     return SP_ERR_INVALID_ARG;
-  const long long idx_grp = (p->flags & SP_F_GROUP_SUPPORT) ? host_geom(&q).num_rows() * (long long)q.k : 0;
-  SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp), "sparse attention");
+  const bool per_head = (p->flags & SP_F_HEAD_SUPPORT) != 0;
+  const long long idx_grp =
+      (p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)) ? host_geom(&q).num_rows() * (long long)q.k : 0;
+  SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp, per_head), "sparse attention");
   return SP_OK;
 }
 
@@ -428,13 +461,21 @@ int sp_dense_gqa_attn(const sp_params* p, const void* Q, const void* K, const vo
 int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void* Wqi, const void* Wki, const void* Q,
                      const void* K, const void* V, void* O, int32_t* idx_out, void* ws, size_t ws_bytes,
                      void* stream) {
-  if (mode != SP_MODE_ORACLE && mode != SP_MODE_INDEXER) return SP_ERR_INVALID_ARG;
+  if (mode != SP_MODE_ORACLE && mode != SP_MODE_INDEXER || !p) return SP_ERR_INVALID_ARG;
+  // support granularity on the head axis: oracle mode only (the indexer is head-collapsed by construction)
+  const int units = layer_units(p, mode);
+  if (units < 0) return units;
+  sp_params pq = *p;
+  pq.flags &= ~(uint32_t)(SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT);
+  const bool per_head = (p->flags & SP_F_HEAD_SUPPORT) != 0, per_group = (p->flags & SP_F_GROUP_SUPPORT) != 0;
+  p = &pq;
   const int rc = validate_common(p, true, mode == SP_MODE_INDEXER);
   if (rc != SP_OK) return rc;
+  if ((per_head || per_group) && !sp_tc_mass_supported(p->b_sel, p->d)) return SP_ERR_UNSUPPORTED;
   if (!Q || !K || !V || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O)) return SP_ERR_INVALID_ARG;
   if (mode == SP_MODE_INDEXER && (!X || !Wqi || !Wki || !aligned16(X) || !aligned16(Wqi) || !aligned16(Wki)))
     return SP_ERR_INVALID_ARG;
-  const LayerPlan pl = plan_layer(p, mode, idx_out == nullptr);
+  const LayerPlan pl = plan_layer(p, mode, idx_out == nullptr, units);
   if (!ws || !aligned16(ws) || ws_bytes < pl.total) return SP_ERR_WORKSPACE;
   char* base = (char*)ws;
   cudaStream_t st = (cudaStream_t)stream;
@@ -451,17 +492,24 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
   } else {
     SP_CUDA(run_attn(p, Q, K, nullptr, nullptr, 0, p->L, nullptr, lse, st), "mass pass 1 (lse)");
   }
-  for (long long r0 = 0; r0 < pl.n_rows; r0 += pl.panel_rows) {
-    const int rcnt = (int)(pl.n_rows - r0 < pl.panel_rows ? pl.n_rows - r0 : pl.panel_rows);
-    const int max_nv = hg.max_n_valid(r0, rcnt);
-    if (mode == SP_MODE_INDEXER) {
-      SP_CUDA(run_indexer_scores(p, q_idx, k_idx, (int)r0, rcnt, max_nv, scores, pl.ld, st), "indexer scores");
-    } else {
-      SP_CUDA(run_mass(p, Q, K, lse, (int)r0, rcnt, max_nv, scores, pl.ld, st), "mass pass 2");
+  // one selection per unit: the whole layer (head-averaged support), each KV group, or each head -- all from ONE pass 1
+  for (int u = 0; u < units; ++u) {
+    int32_t* idx_u = idx + (size_t)u * pl.n_rows * p->k;
+    for (long long r0 = 0; r0 < pl.n_rows; r0 += pl.panel_rows) {
+      const int rcnt = (int)(pl.n_rows - r0 < pl.panel_rows ? pl.n_rows - r0 : pl.panel_rows);
+      const int max_nv = hg.max_n_valid(r0, rcnt);
+      if (mode == SP_MODE_INDEXER) {
+        SP_CUDA(run_indexer_scores(p, q_idx, k_idx, (int)r0, rcnt, max_nv, scores, pl.ld, st), "indexer scores");
+      } else {
+        SP_CUDA(run_mass(p, Q, K, lse, (int)r0, rcnt, max_nv, scores, pl.ld, st, per_group ? u : -1, per_head ? u : -1),
+                "mass pass 2");
+      }
+      SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, max_nv, idx_u + (size_t)r0 * p->k, nullptr, st), "top-k");
     }
-    SP_CUDA(sp_launch_topk(g, scores, pl.ld, (int)r0, rcnt, p->k, max_nv, idx + (size_t)r0 * p->k, nullptr, st), "top-k");
   }
-  SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st), "sparse attention");
+  SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st, units > 1 || per_group || per_head ? pl.n_rows * (long long)p->k : 0,
+                   per_head),
+          "sparse attention");
   return SP_OK;
 }
 

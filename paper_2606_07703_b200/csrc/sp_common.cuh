@@ -132,7 +132,8 @@ cudaError_t sp_launch_indexer_scores_tc(const SpGeom& g, const int32_t* cu_host,
 bool sp_tc_mass_supported(int b_sel, int d);
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
-                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp = -1);  // grp >= 0: that KV group's heads only
+                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp = -1,
+                              int head = -1);  // grp >= 0: that KV group's heads only; head >= 0: that one head only
 
 bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d);
 cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, long long chunk_base,
@@ -143,7 +144,7 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
 // per-query gather-sparse attention on mma.sync (sp_mma_attn.cu)
 cudaError_t sp_launch_attn_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int q_begin,
-                              int q_count, void* O, float* lse, cudaStream_t st);
+                              int q_count, void* O, float* lse, cudaStream_t st, bool per_head = false);
 
 // diagnostics (sp_diag.cu)
 cudaError_t sp_launch_overlap(const int32_t* a, const int32_t* b, long long n_rows, int k, int32_t* inter,

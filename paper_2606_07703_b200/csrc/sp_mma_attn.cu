@@ -53,18 +53,22 @@ template <int D, int G>
 __global__ void __launch_bounds__(PQ_WARPS * 32)
 sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
-                  int local_window, float local_bias, int q_begin, int q_count, __nv_bfloat16* __restrict__ O,
-                  float* __restrict__ lse) {
+                  int local_window, float local_bias, int q_begin, int q_count, int kv_div,
+                  __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
   constexpr int KS = D / 16;   // k-slices of the QK^T contraction
   constexpr int NT = D / 8;    // 8-channel n tiles of O
   constexpr int CPR = D / 8;   // 16-byte chunks per row
   extern __shared__ __align__(128) uint8_t pq_smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long wid = (long long)blockIdx.x * PQ_WARPS + warp;
-  if (wid >= (long long)q_count * Hkv) return;
-  const int t = q_begin + (int)(wid / Hkv);
-  const int kvh = (int)(wid % Hkv);
-  const int Hq = Hkv * G;
+  // units per query: the Hkv KV groups (G heads each share the gathered rows), or -- one support list per HEAD
+  // (PAPER.md:100 S_{l,t,h}; G == 1 instantiation, kv_div = heads per KV group) -- the Hq heads, each gathering its own rows
+  const int NU = Hkv * kv_div;
+  if (wid >= (long long)q_count * NU) return;
+  const int t = q_begin + (int)(wid / NU);
+  const int unit = (int)(wid % NU);
+  const int kvh = unit / kv_div;  // KV head whose rows are gathered
+  const int Hq = NU * G;
   const SpPos pi = sp_pos_info(g, t);
   const int gq = lane >> 2, tq = lane & 3;  // fragment coordinates: row group, column pair
   uint8_t* sK = pq_smem + (size_t)warp * (2 * PQ_KEYS * D * 2);
@@ -74,7 +78,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   // ---- A fragments of Q: head h = row gq (< G), channels ks*16 + 2 tq (+1) and + 8 ----
   uint32_t qa[KS][2];
   {
-    const __nv_bfloat16* qr = Q + ((size_t)(t - g.q_off) * Hq + kvh * G + min(gq, G - 1)) * D;
+    const __nv_bfloat16* qr = Q + ((size_t)(t - g.q_off) * Hq + unit * G + min(gq, G - 1)) * D;
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) {
       qa[ks][0] = gq < G ? *reinterpret_cast<const uint32_t*>(qr + ks * 16 + 2 * tq) : 0u;
@@ -86,7 +90,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   float o[NT][4];
 #pragma unroll
   for (int n = 0; n < NT; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
-  const int32_t* sup = idx + (size_t)kvh * (size_t)g.idx_grp + (size_t)(pi.row - g.row_off) * k;
+  const int32_t* sup = idx + (size_t)unit * (size_t)g.idx_grp + (size_t)(pi.row - g.row_off) * k;
 
   int e_next = lane < k ? __ldg(sup + lane) : -1;  // index entries are fetched ONE TILE AHEAD (their L2 latency used to
                                                    // sit in front of every tile's gathers)
@@ -190,7 +194,7 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
   }
   // ---- epilogue: rows gq < G ----
   if (gq < G) {
-    const size_t orow = (size_t)(t - g.q_off) * Hq + kvh * G + gq;
+    const size_t orow = (size_t)(t - g.q_off) * Hq + unit * G + gq;
     if (O != nullptr) {
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
       __nv_bfloat16* dst = O + orow * D + 2 * tq;
@@ -204,29 +208,31 @@ sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bflo
 
 template <int D, int G>
 cudaError_t launch_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hkv,
-                      float scale, int lw, float lb, int q_begin, int q_count, void* O, float* lse, cudaStream_t st) {
+                      float scale, int lw, float lb, int q_begin, int q_count, int kv_div, void* O, float* lse,
+                      cudaStream_t st) {
   const size_t smem = (size_t)PQ_WARPS * 2 * PQ_KEYS * D * 2;
   static unsigned char attr_seen[SP_MAX_DEVICES];
   if (sp_first_use_on_device(attr_seen)) {
     cudaError_t e = cudaFuncSetAttribute(sp_attn_pq_kernel<D, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  const long long warps = (long long)q_count * Hkv;
+  const long long warps = (long long)q_count * Hkv * kv_div;
   sp_attn_pq_kernel<D, G><<<(unsigned)((warps + PQ_WARPS - 1) / PQ_WARPS), PQ_WARPS * 32, smem, st>>>(
       g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, q_begin,
-      q_count, (__nv_bfloat16*)O, lse);
+      q_count, kv_div, (__nv_bfloat16*)O, lse);
   return cudaGetLastError();
 }
 
 template <int D>
 cudaError_t launch_pq_d(int G, const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,
-                        int Hkv, float scale, int lw, float lb, int q_begin, int q_count, void* O, float* lse,
-                        cudaStream_t st) {
+                        int Hkv, float scale, int lw, float lb, int q_begin, int q_count, bool per_head, void* O,
+                        float* lse, cudaStream_t st) {
+  if (per_head) return launch_pq<D, 1>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, G, O, lse, st);
   switch (G) {
-    case 1: return launch_pq<D, 1>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, O, lse, st);
-    case 2: return launch_pq<D, 2>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, O, lse, st);
-    case 4: return launch_pq<D, 4>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, O, lse, st);
-    case 8: return launch_pq<D, 8>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, O, lse, st);
+    case 1: return launch_pq<D, 1>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, 1, O, lse, st);
+    case 2: return launch_pq<D, 2>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, 1, O, lse, st);
+    case 4: return launch_pq<D, 4>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, 1, O, lse, st);
+    case 8: return launch_pq<D, 8>(g, Q, K, V, idx, k, Hkv, scale, lw, lb, q_begin, q_count, 1, O, lse, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -236,13 +242,13 @@ cudaError_t launch_pq_d(int G, const SpGeom& g, const void* Q, const void* K, co
 // Sparse attention of the packed queries [q_begin, q_begin + q_count) with one support row per sp_pos_info(g, t).row.
 cudaError_t sp_launch_attn_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int q_begin,
-                              int q_count, void* O, float* lse, cudaStream_t st) {
+                              int q_count, void* O, float* lse, cudaStream_t st, bool per_head) {
   if (q_count <= 0) return cudaSuccess;
   const int G = Hq / Hkv;
   cudaError_t e = d == 128 ? launch_pq_d<128>(G, g, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, q_begin,
-                                              q_count, O, lse, st)
+                                              q_count, per_head, O, lse, st)
                            : launch_pq_d<64>(G, g, Q, K, V, idx, k, Hkv, scale, local_window, local_bias, q_begin,
-                                             q_count, O, lse, st);
+                                             q_count, per_head, O, lse, st);
   sp_count_launch();
   return e;
 }

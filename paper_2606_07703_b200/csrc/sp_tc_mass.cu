@@ -465,7 +465,7 @@ int ms_sm_count() { return sp_sm_count(); }
 
 template <int D>
 cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const float* lse, int Hq, int Hkv, int grp,
-                           float scale, int lw, float lb, int row_begin, int row_count, int qt_begin, int qt_count,
+                           int head, float scale, int lw, float lb, int row_begin, int row_count, int qt_begin, int qt_count,
                            long long items, float* mass, int64_t ld, cudaStream_t st) {
   CUtensorMap tmQ, tmK;
   cudaError_t e;
@@ -473,7 +473,13 @@ cudaError_t launch_mass_tc(const SpGeom& g, const void* Q, const void* K, const 
   // head -- through offset base pointers; the row pitches of Q, K and lse stay those of the full tensors.
   const int lse_stride = Hq, G = Hq / Hkv;
   const uint64_t q_pitch = (uint64_t)Hq * D, k_pitch = (uint64_t)Hkv * D;
-  if (grp >= 0) {
+  if (head >= 0) {  // per-HEAD mass (PAPER.md:100 S_{l,t,h}): one head over its KV head
+    Q = (const __nv_bfloat16*)Q + (size_t)head * D;
+    K = (const __nv_bfloat16*)K + (size_t)(head / G) * D;
+    lse += (size_t)head;
+    Hq = 1;
+    Hkv = 1;
+  } else if (grp >= 0) {
     Q = (const __nv_bfloat16*)Q + (size_t)grp * G * D;
     K = (const __nv_bfloat16*)K + (size_t)grp * D;
     lse += (size_t)grp * G;
@@ -507,7 +513,7 @@ bool sp_tc_mass_supported(int b_sel, int d) {
 // cu_host: HOST copy of cu_seqlens (nullptr = one sequence).
 cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const void* Q, const void* K, const float* lse,
                               int Hq, int Hkv, int d, float scale, int local_window, float local_bias, int row_begin,
-                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp) {
+                              int row_count, float* mass, int64_t ld, cudaStream_t st, int grp, int head) {
   if (row_count <= 0) return cudaSuccess;
   // 128-query tiles (per sequence) that intersect the support-row panel [row_begin, row_begin + row_count)
   const int b = g.b_sel;
@@ -535,8 +541,8 @@ cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const voi
   }
   if (qlo < 0) return cudaSuccess;
   const int cnt = (int)(qhi - qlo + 1);
-  return d == 128 ? launch_mass_tc<128>(g, Q, K, lse, Hq, Hkv, grp, scale, local_window, local_bias, row_begin,
+  return d == 128 ? launch_mass_tc<128>(g, Q, K, lse, Hq, Hkv, grp, head, scale, local_window, local_bias, row_begin,
                                         row_count, (int)qlo, cnt, items, mass, ld, st)
-                  : launch_mass_tc<64>(g, Q, K, lse, Hq, Hkv, grp, scale, local_window, local_bias, row_begin,
+                  : launch_mass_tc<64>(g, Q, K, lse, Hq, Hkv, grp, head, scale, local_window, local_bias, row_begin,
                                        row_count, (int)qlo, cnt, items, mass, ld, st);
 }

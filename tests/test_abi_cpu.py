@@ -60,8 +60,9 @@ def test_num_rows_and_workspace_are_host_arithmetic(lib):
     (dict(Hq=6, Hkv=4), B.SP_ERR_INVALID_ARG),
     (dict(d=96), B.SP_ERR_UNSUPPORTED),
     (dict(Hq=32, Hkv=2), B.SP_ERR_UNSUPPORTED),
-    (dict(flags=8), B.SP_ERR_UNSUPPORTED),               # SP_F_GROUP_SUPPORT belongs to sp_sparse_gqa_attn alone
-    (dict(flags=16), B.SP_ERR_UNSUPPORTED),              # unknown flag bit
+    (dict(flags=8), B.SP_ERR_UNSUPPORTED),               # SP_F_GROUP_SUPPORT: oracle-mode layer / sp_sparse_gqa_attn only
+    (dict(flags=16), B.SP_ERR_UNSUPPORTED),              # SP_F_HEAD_SUPPORT: likewise (this is the INDEXER layer stage)
+    (dict(flags=32), B.SP_ERR_UNSUPPORTED),              # unknown flag bit
     (dict(flags=1, b_sel=16), B.SP_ERR_UNSUPPORTED),     # served-scorer flags need a tcgen05 score path
     (dict(d_idx=32), B.SP_ERR_UNSUPPORTED),
     (dict(hidden=100), B.SP_ERR_UNSUPPORTED),
@@ -94,6 +95,17 @@ def test_null_and_misaligned_pointers_and_panels(lib):
     assert h(C.byref(p), B.SP_MODE_INDEXER, n, n, n, fake, fake, fake, fake, n, fake, C.c_size_t(1 << 40), n) == B.SP_ERR_INVALID_ARG
     assert b"SP_ERR_WORKSPACE" in lib.sp_strerror(B.SP_ERR_WORKSPACE)
     assert lib.sp_launch_count() == 0
+
+
+def test_head_axis_flags_in_the_oracle_layer_workspace(lib):
+    base = B.workspace_bytes(P(), B.SP_STAGE_LAYER_ORACLE)
+    grp = B.workspace_bytes(P(flags=B.SP_F_GROUP_SUPPORT), B.SP_STAGE_LAYER_ORACLE)
+    head = B.workspace_bytes(P(flags=B.SP_F_HEAD_SUPPORT), B.SP_STAGE_LAYER_ORACLE)
+    idx_bytes = 256 * 16 * 4                                  # n_rows * k * int32
+    assert grp - base == (2 - 1) * idx_bytes and head - base == (8 - 1) * idx_bytes
+    with pytest.raises(B.SpError) as ei:
+        B.workspace_bytes(P(flags=B.SP_F_GROUP_SUPPORT | B.SP_F_HEAD_SUPPORT), B.SP_STAGE_LAYER_ORACLE)
+    assert ei.value.code == B.SP_ERR_INVALID_ARG
 
 
 def test_chunk_api_validates_before_launching(lib):

@@ -407,9 +407,11 @@ def test_sparse_attention_on_per_group_oracle_supports(cfg, b, k):
     idx = torch.from_numpy(np.ascontiguousarray(idx_o)).to(DEV)
     B.sp_sparse_gqa_attn(pbg, dev(inp["Q"]), dev(inp["K"]), dev(inp["V"]), idx, O)
     parity.compare_attention(to_f64(O), want)
-    # and the flag is this entry point's alone
+    # the flag means nothing to the stage calls that take no index tensor
     with pytest.raises(B.SpError) as ei:
-        B.workspace_bytes(B.Problem.from_config(cfg, flags=B.SP_F_GROUP_SUPPORT, **over), B.SP_STAGE_LAYER_ORACLE)
+        B.sp_topk_support(B.Problem.from_config(cfg, flags=B.SP_F_GROUP_SUPPORT, **over),
+                          torch.zeros(4, cfg.L, dtype=torch.float32, device=DEV), 0, 4,
+                          torch.zeros(4, k, dtype=torch.int32, device=DEV))
     assert ei.value.code == B.SP_ERR_UNSUPPORTED
 
 
@@ -453,6 +455,63 @@ def test_per_group_selection_chain(cfg, b, k, lw):
     parity.compare_attention(to_f64(O)[keep], want[keep])
     with pytest.raises(B.SpError):
         B.sp_oracle_mass_group(pbg, Qd, Kd, lse, True, cfg.Hkv, 0, rows, mass)
+
+
+@pytest.mark.parametrize("cfg,b,k,lw,gran", [(SMALL_ORC, 1, 96, 0, "group"), (SMALL_ORC, 64, 96, 12, "group"),
+                                             (SMALL_ORC128, 128, 200, 16, "group"), (SMALL_ORC, 1, 96, 0, "head"),
+                                             (SMALL_ORC, 64, 96, 12, "head"), (SMALL_ORC128, 128, 200, 16, "head"),
+                                             (SMALL_ORC128, 1, 40, 0, "head")],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_layer_with_head_axis_granularity(cfg, b, k, lw, gran):
+    """sp_prefill_layer in oracle mode with SP_F_GROUP_SUPPORT / SP_F_HEAD_SUPPORT (A29): one pass 1,
+    then one selection per KV group or per head, then attention with those lists -- against the per-group / per-head
+    oracle: every list under the support rule, outputs on the queries whose lists all match, the rest against the
+    oracle's attention on the GPU's own lists."""
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    flag = B.SP_F_GROUP_SUPPORT if gran == "group" else B.SP_F_HEAD_SUPPORT
+    over = dict(b_sel=b, k=k, local_window=lw, local_bias=0.75 if lw else 0.0)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, flags=flag, **over)
+    rows = orc.num_rows(pbo)
+    units = cfg.Hkv if gran == "group" else cfg.Hq
+    Qd, Kd, Vd = dev(inp["Q"]), dev(inp["K"]), dev(inp["V"])
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    idx = torch.full((units, rows, k), -9, dtype=torch.int32, device=DEV)
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_LAYER_ORACLE)
+    assert ws.numel() >= B.workspace_bytes(B.Problem.from_config(cfg, **over), B.SP_STAGE_LAYER_ORACLE)
+    B.sp_prefill_layer(pbg, B.SP_MODE_ORACLE, None, None, None, Qd, Kd, Vd, O, idx, ws)
+    torch.cuda.synchronize()
+    all_rows = np.arange(rows)
+    if gran == "group":
+        idx_o, _ = orc.select_support_per_group(pbo, inp["Q"], inp["K"], all_rows)
+        sub, slices, attn = orc._group_problem(pbo), orc._group_slices, orc.sparse_attn_per_group
+    else:
+        idx_o, _ = orc.select_support_per_head(pbo, inp["Q"], inp["K"], all_rows)
+        sub, slices, attn = orc._head_problem(pbo), orc._head_slices, orc.sparse_attn_per_head
+    idx_g = idx.cpu().numpy()
+    for u in range(units):
+        Qu, Ku, _ = slices(pbo, inp["Q"], inp["K"], None, u)
+        R, nv = orc.support_scores(sub, orc.MODE_ORACLE, Qu, Ku, all_rows)
+        parity.compare_supports(idx_g[u], idx_o[u], R, nv, k)
+    pos = np.arange(cfg.L)
+    row_of = np.array([orc.row_of_pos(pbo, int(t)) for t in pos])
+    keep = np.all(idx_g == idx_o, axis=(0, 2))[row_of]
+    assert keep.mean() > 0.5, keep.mean()
+    o_gpu = to_f64(O)
+    st = {"units": units, "chained_queries": int(keep.sum()), "chained_on_gpu_support": int((~keep).sum())}
+    st["chained"] = parity.compare_attention(o_gpu[keep], attn(pbo, inp["Q"], inp["K"], inp["V"], pos[keep], idx_o[:, row_of[keep], :]))
+    if (~keep).any():
+        st["chained_gpu_support"] = parity.compare_attention(
+            o_gpu[~keep], attn(pbo, inp["Q"], inp["K"], inp["V"], pos[~keep], idx_g[:, row_of[~keep], :]))
+    record_stats(f"head_axis:{gran}:{cfg.name}:b{b}:k{k}", st)
+    # the stage call agrees with the layer's lists
+    O2 = torch.empty_like(O)
+    B.sp_sparse_gqa_attn(pbg, Qd, Kd, Vd, idx, O2)
+    assert torch.equal(O2.view(torch.int16), O.view(torch.int16))
+    # indexer mode has no head axis to split
+    with pytest.raises(B.SpError) as ei:
+        B.workspace_bytes(B.Problem.from_config(cfg, flags=flag, hidden=256, d_idx=64, **over), B.SP_STAGE_LAYER_INDEXER)
+    assert ei.value.code == B.SP_ERR_UNSUPPORTED
 
 
 @pytest.mark.parametrize("cfg", [SMALL_ORC, SMALL_ORC128], ids=lambda c: c.name)

@@ -520,7 +520,7 @@ def test_row_kl_pins():
 
 
 # ---------------------------------------------------------------- per-KV-group support (A29)
-# oracle groundwork for SURVEY.md 8(f) f4 -- there is no CUDA path for it yet
+# the head-axis variants of the support
 
 def _group_bruteforce(pb, Q, K, V, b):
     """Independent of oracle.py's slicing: dense [Hq, L, L] probabilities, mean over each group's heads."""
@@ -586,6 +586,67 @@ def test_per_group_equals_dense_when_budget_covers_prefix():
     idx, _ = orc.select_support_per_group(pb, Q, K, pos)
     out = orc.sparse_attn_per_group(pb, Q, K, V, pos, idx)
     assert np.allclose(out, orc.dense_attn(pb, Q, K, V, pos), rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- per-head support ("separately per query head")
+
+def _head_bruteforce(pb, Q, K, V, b):
+    """Dense [Hq, L, L] probabilities; every head ranks ITS OWN rows (block max over the block's queries)."""
+    from scipy.special import softmax
+    G = pb.Hq // pb.Hkv
+    z = bf.logits(Q, K, 1.0 / math.sqrt(pb.d), G)                       # [Hq, L, L]
+    A = softmax(z, axis=-1)
+    idx = []
+    for h in range(pb.Hq):
+        R, nv = bf.support_rows(A[h], b)
+        idx.append(bf.topk_rows(R, nv, pb.k))
+    idx = np.stack(idx)                                                 # [Hq, rows, k]
+    v = np.repeat(bf.bf16_to_f64(V), G, axis=1)
+    out = np.zeros((pb.L, pb.Hq, pb.d))
+    for h in range(pb.Hq):
+        for t in range(pb.L):
+            s = idx[h, t // b]
+            s = s[(s >= 0) & (s <= t)]
+            if len(s):
+                out[t, h] = softmax(z[h, t, s]) @ v[s, h]
+    return idx, out
+
+
+@pytest.mark.parametrize("b", [1, 4])
+def test_per_head_support_matches_bruteforce(b):
+    pb, Q, K, V = small_problem(L=37, Hq=6, Hkv=3, d=8, k=5, b=b, seed=51)
+    rows = np.arange(orc.num_rows(pb))
+    idx, cnt = orc.select_support_per_head(pb, Q, K, rows)
+    want_idx, want_out = _head_bruteforce(pb, Q, K, V, b)
+    assert idx.shape == (6, len(rows), 5)
+    assert np.array_equal(idx, want_idx)
+    assert np.array_equal(cnt, (want_idx >= 0).sum(axis=-1))
+    pos = np.arange(pb.L)
+    out = orc.sparse_attn_per_head(pb, Q, K, V, pos, idx[:, pos // b, :])
+    assert np.allclose(out, want_out, rtol=0, atol=1e-13)
+    # two heads of the SAME KV group must differ here, or a head -> group mix-up would go unseen
+    assert not np.array_equal(idx[0], idx[1])
+
+
+def test_per_head_reductions():
+    # G = 1: a head is its KV group (PAPER.md:100: the three granularities coincide for MHA with one head per group)
+    pb, Q, K, V = small_problem(L=33, Hq=3, Hkv=3, d=8, k=6, b=2, seed=61)
+    rows = np.arange(orc.num_rows(pb))
+    ih, ch = orc.select_support_per_head(pb, Q, K, rows)
+    ig, cg = orc.select_support_per_group(pb, Q, K, rows)
+    assert np.array_equal(ih, ig) and np.array_equal(ch, cg)
+    # identical heads inside a group: every head's distribution equals the group mean, so head lists == group lists
+    pb2 = orc.Problem(L=33, Hq=6, Hkv=3, d=8, k=6, b_sel=2)
+    Q2 = np.repeat(Q, 2, axis=1)
+    ih2, _ = orc.select_support_per_head(pb2, Q2, K, rows)
+    ig2, _ = orc.select_support_per_group(pb2, Q2, K, rows)
+    for h in range(6):
+        assert np.array_equal(ih2[h], ig2[h // 2])
+    # k >= n: every list is the whole prefix, the recompute is dense attention
+    pb3, Q3, K3, V3 = small_problem(L=20, Hq=4, Hkv=2, d=8, k=20, seed=71)
+    pos = np.arange(20)
+    i3, _ = orc.select_support_per_head(pb3, Q3, K3, pos)
+    assert np.allclose(orc.sparse_attn_per_head(pb3, Q3, K3, V3, pos, i3), orc.dense_attn(pb3, Q3, K3, V3, pos), rtol=0, atol=1e-14)
 
 
 # ---------------------------------------------------------------- paged KV cache / chunked prefill (PAPER.md:292, :331, :428)

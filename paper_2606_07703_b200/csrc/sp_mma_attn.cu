@@ -50,7 +50,7 @@ __device__ __forceinline__ uint32_t pq_off(int r, int c) {
 }
 
 template <int D, int G>
-__global__ void __launch_bounds__(PQ_WARPS * 32)
+__global__ void __launch_bounds__(PQ_WARPS * 32, 3)  // 3 CTAs per SM (the shared-memory limit at d = 128): <= 168 registers; at 180 only 2 fit
 sp_attn_pq_kernel(SpGeom g, const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
                   int local_window, float local_bias, int q_begin, int q_count, int kv_div,

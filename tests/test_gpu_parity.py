@@ -18,13 +18,15 @@ pytestmark = pytest.mark.gpu
 DEV = "cuda"
 
 # chained parity: at least this fraction of the sampled support rows BEYOND the budget must carry the oracle's exact
-# index list (rows with near-tied k-th scores may swap keys within the overlap rule; measured fractions are recorded
-# by record_stats and kept under profiles/)
+# index list (rows with near-tied k-th scores may swap keys within the overlap rule).  Measured (profiles/r2_parity.json):
+# c2 109/112, c3 29/33, c4 22..28 of 28, c5 14/22 -- the floor sits under the smallest; every query of a row that
+# differs is still compared end to end, against the oracle's attention on the GPU's own list.
 CHAINED_IDENTICAL_FLOOR = 0.5
-# fraction of projected bf16 elements allowed to differ (by one ulp) from the oracle's fp64-sum rounding; set from the
-# measured rates
-PROJ_MISMATCH_RATE = 5e-3
-PROJ_SERVED_MISMATCH_RATE = 1e-2
+# fraction of projected bf16 elements allowed to differ (by one ulp) from the oracle's fp64-sum rounding: ~3x the measured
+# rates (profiles/r2_parity.json: 2.3e-4 .. 5.8e-4 plain, 2.3e-4 .. 6.7e-4 with the key LayerNorm / RoPE epilogue);
+# DESIGN.md "Arithmetic and tolerances"
+PROJ_MISMATCH_RATE = 2e-3
+PROJ_SERVED_MISMATCH_RATE = 2e-3
 STATS_PATH = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out", "parity_stats.json")
 _STATS = {}
 

@@ -649,7 +649,9 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             // a fresh read of S.  Flagged tiles have their max from the masking pass. ----
             bool need;
             if (!flagged) {
-              need = !(tsum <= AT_SUM_LIMIT);
+              // (a row with no finite running max yet -- only possible here after fully masked tiles of a list that is
+              // not ascending -- has no reference to speculate against and takes its max the classic way)
+              need = !(tsum <= AT_SUM_LIMIT) || m_run == -INFINITY;
               if (!__any_sync(0xffffffffu, need)) break;
               uint32_t w[AT_KT];
               tmem_ld_x32(t_s, w);

@@ -531,6 +531,32 @@ def test_dense_attention_matches_oracle(cfg):
 
 
 @pytest.mark.parametrize("b", [64, 1])
+def test_sparse_attention_accepts_unordered_index_lists(b):
+    """include/sp.h: entries < 0 or > t are ignored wherever they stand.  The oracle's lists, shuffled inside every row
+    with the -1 padding mixed in (so masked entries precede valid ones and whole leading tiles can be masked for a
+    query), must give the same outputs and log-sum-exps."""
+    cfg = SMALL_ORC128
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    over = dict(b_sel=b, k=200, local_window=12, local_bias=-0.5)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    res = orc.prefill_layer(pbo, orc.MODE_ORACLE, inp["Q"], inp["K"], inp["V"])
+    rng = np.random.Generator(np.random.Philox(2024 + b))
+    idx_sh = np.stack([rng.permutation(r) for r in res.idx]).astype(np.int32)
+    idx_sh[::3] = np.sort(idx_sh[::3], axis=1)[:, ::-1]              # every third row: descending, valid keys LAST
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    lse = torch.empty(cfg.L, cfg.Hq, dtype=torch.float32, device=DEV)
+    B.sp_sparse_gqa_attn(pbg, dev(inp["Q"]), dev(inp["K"]), dev(inp["V"]), torch.from_numpy(idx_sh).to(DEV), O, lse)
+    parity.compare_attention(to_f64(O), res.out)
+    sup = np.stack([res.idx[orc.row_of_pos(pbo, t)] for t in range(cfg.L)])
+    _, lse_o = orc.sparse_attn(pbo, inp["Q"], inp["K"], inp["V"], np.arange(cfg.L), sup, want_lse=True)
+    fin = np.isfinite(lse_o)
+    got = to_f64(lse)
+    assert np.array_equal(np.isfinite(got), fin)
+    assert np.allclose(got[fin], lse_o[fin], rtol=0, atol=2e-5)
+
+
+@pytest.mark.parametrize("b", [64, 1])
 def test_attention_growing_logits_rescale_path(b):
     """Logits that keep growing along the key axis (later keys dominate by > 2^8) force the lazy O rescale of the
     tcgen05 kernel in most tiles, and large magnitudes check that nothing overflows; dense and sparse paths."""

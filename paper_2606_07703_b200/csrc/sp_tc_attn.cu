@@ -265,7 +265,9 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
     const int c = ptid % CPR;
     const int key0 = ptid / CPR;
     const uint32_t kv_off = (uint32_t)(c / 8) * KV_BLK;
-    uint32_t gk = 0, n_q = 0, n_it = 0;
+    uint32_t n_q = 0, n_it = 0;
+    uint32_t ld_s = 0, ld_ph = 0;  // K / V ring slot of the next tile, and the parity of its use count
+    bool ld_wrapped = false;       // the ring has been filled once: slots must be waited for
     // ---- index-list staging runs ONE ITEM AHEAD of the K/V loads (its global loads have L2 / DRAM latency and would
     // otherwise sit between two items): `is` / n_st walk the same item sequence as `i` / n_it ----
     int is = 0;
@@ -307,11 +309,14 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             if (!ok || p > qa0 - win) f |= 1u;
             if (!ok || p > qa1 - win) f |= 2u;
             if (ok) my_last = e + 1;
-            if (f) atomicOr(&fl[e / AT_KT], f);
+            // the 32 entries of a warp lie in ONE tile (e0 and 128 u are multiples of 32): one atomic per warp
+            f = __reduce_or_sync(0xffffffffu, f);
+            if (f && (ptid & 31) == 0) atomicOr(&fl[e / AT_KT], f);
           }
         }
       }
-      if (my_last) atomicMax(&n_eff_sh[ib], my_last);
+      my_last = __reduce_max_sync(0xffffffffu, my_last);
+      if (my_last && (ptid & 31) == 0) atomicMax(&n_eff_sh[ib], my_last);
       loader_bar_sync();
       nt_buf[ib] = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
       mbar_arrive(&bar.idxfull[ib]);
@@ -336,39 +341,47 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       }
       ++n_it;
       if (nt == 0) continue;
-      const __nv_bfloat16* Kh = K + (size_t)it.kvh * D + c * 8;
-      const __nv_bfloat16* Vh = V + (size_t)it.kvh * D + c * 8;
-      const size_t rstride = (size_t)Hkv * D;
+      // Per 16-byte chunk the loaders spend an LDS (the key's position), one 32 x 32 -> 64-bit multiply-add (row
+      // address) and the cp.async itself: everything else is hoisted -- a loader warp shares its scheduler with two
+      // softmax warps, and at ~280 instructions per tile (run-time ring modulo, 64-bit offset multiplies and the
+      // swizzle recomputed per pass) the loaders took a fifth of the kernel's issue slots (profiles/r2_attn.md).
+      const char* Kb = reinterpret_cast<const char*>(K) + ((size_t)it.kvh * D + c * 8) * 2;
+      const long long v_minus_k = reinterpret_cast<const char*>(V) - reinterpret_cast<const char*>(K);
+      const uint32_t row_bytes = (uint32_t)Hkv * D * 2;
+      // destination of pass pi: row key0 + pi * KPP keeps the row's low three bits (KPP % 8 == 0), so its swizzled
+      // offset is that of row key0 plus pi * KPP * 128
+      static_assert(KPP % 8 == 0, "a loader pass must step whole swizzle atoms");
+      const uint32_t dst_row0 = sw128_offset(key0, c % 8) + kv_off;
       auto load_tile = [&](int j) {
-        const uint32_t gj = gk + j;
-        const int s = gj % NS;
-        const uint32_t u = gj / NS;
-        size_t off[PASSES];
+        const char* src[PASSES];
 #pragma unroll
         for (int pi = 0; pi < PASSES; ++pi) {
-          const int col = j * AT_KT + key0 + pi * KPP;
           int p;
           if (SPARSE) {
-            p = si[col];
+            p = si[j * AT_KT + key0 + pi * KPP];
             if (p < 0) p = it.seq_start;  // masked later; any valid row will do
           } else {
-            p = it.seq_start + min(col, it.t1);
+            p = it.seq_start + min(j * AT_KT + key0 + pi * KPP, it.t1);
           }
-          off[pi] = (size_t)sp_kv_row(g, p) * rstride;
+          if (g.bt != nullptr) src[pi] = Kb + (size_t)sp_kv_row(g, p) * row_bytes;
+          else src[pi] = Kb + (unsigned long long)(uint32_t)p * row_bytes;
         }
-        if (u > 0) mbar_wait(&bar.kempty[s], (u - 1) & 1);
-        const uint32_t kdst = smem_u32(sK + s * KV_TILE) + kv_off;
+        if (ld_wrapped) mbar_wait(&bar.kempty[ld_s], ld_ph ^ 1);
+        const uint32_t kdst = smem_u32(sK) + ld_s * KV_TILE + dst_row0;
 #pragma unroll
-        for (int pi = 0; pi < PASSES; ++pi)
-          cp_async16(kdst + sw128_offset(key0 + pi * KPP, c % 8), Kh + off[pi]);
-        cp_async_arrive_noinc(&bar.kfull[s]);
+        for (int pi = 0; pi < PASSES; ++pi) cp_async16(kdst + pi * (KPP * 128), src[pi]);
+        cp_async_arrive_noinc(&bar.kfull[ld_s]);
         if (WITH_O) {
-          if (u > 0) mbar_wait(&bar.vempty[s], (u - 1) & 1);
-          const uint32_t vdst = smem_u32(sV + s * KV_TILE) + kv_off;
+          if (ld_wrapped) mbar_wait(&bar.vempty[ld_s], ld_ph ^ 1);
+          const uint32_t vdst = smem_u32(sV) + ld_s * KV_TILE + dst_row0;
 #pragma unroll
-          for (int pi = 0; pi < PASSES; ++pi)
-            cp_async16(vdst + sw128_offset(key0 + pi * KPP, c % 8), Vh + off[pi]);
-          cp_async_arrive_noinc(&bar.vfull[s]);
+          for (int pi = 0; pi < PASSES; ++pi) cp_async16(vdst + pi * (KPP * 128), src[pi] + v_minus_k);
+          cp_async_arrive_noinc(&bar.vfull[ld_s]);
+        }
+        if (++ld_s == (uint32_t)NS) {  // ring position and phase of the next tile
+          ld_s = 0;
+          ld_ph ^= 1;
+          ld_wrapped = true;
         }
       };
       // The first tiles only need ring slots whose MMAs were issued before the previous item's last S MMA, so they
@@ -395,7 +408,6 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
         }
       }
       if (SPARSE && !staged_ahead) stage_next();
-      gk += nt;
     }
     cp_async_wait<0>();
   } else if (warp == AT_MMA_WARP || warp >= AT_LOAD_WARP0 + AT_LOAD_WARPS) {

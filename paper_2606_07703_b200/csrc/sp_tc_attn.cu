@@ -40,6 +40,8 @@ constexpr int AT_THREADS = 512;    // 8 softmax warps + 4 loader warps + 4 MMA-i
 constexpr int AT_LOAD_WARPS = 4;
 constexpr int AT_MMA_WARP = 8;
 constexpr int AT_LOAD_WARP0 = 9;
+// (Measured and not kept: MMA issuers on warps 8, 9 and the loaders on warps 10, 11, 14, 15, i.e. two loaders on each of
+// schedulers 2 and 3 instead of issuer + loader on schedulers 0 and 1: +2.5 % slower.)
 constexpr float AT_RESCALE_THRESHOLD = 8.0f;  // log2 units: O is rescaled only when the row max grew by > 2^8
 
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t* bar) {
@@ -149,6 +151,11 @@ struct AtBarriers {
   uint64_t oempty[2];    // softmax -> MMA: the item's O accumulator has been read out
   uint64_t idxfull[2], idxempty[2];
 };
+
+// byte offset of packed key position p's row in a PAGED K / V pool (deliberately not inlined, see the loaders)
+__device__ __noinline__ unsigned long long at_paged_row_bytes(const SpGeom& g, int p, uint32_t row_bytes) {
+  return (unsigned long long)sp_kv_row(g, p) * row_bytes;
+}
 
 struct AtItem {
   int seq_start, t0, t1, kvh, row;
@@ -354,6 +361,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       const uint32_t dst_row0 = sw128_offset(key0, c % 8) + kv_off;
       auto load_tile = [&](int j) {
         const char* src[PASSES];
+        int pos[PASSES];
 #pragma unroll
         for (int pi = 0; pi < PASSES; ++pi) {
           int p;
@@ -363,8 +371,13 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           } else {
             p = it.seq_start + min(j * AT_KT + key0 + pi * KPP, it.t1);
           }
-          if (g.bt != nullptr) src[pi] = Kb + (size_t)sp_kv_row(g, p) * row_bytes;
-          else src[pi] = Kb + (unsigned long long)(uint32_t)p * row_bytes;
+          src[pi] = Kb + (unsigned long long)(uint32_t)p * row_bytes;
+          pos[pi] = p;
+        }
+        if (g.bt != nullptr) {  // paged cache: rows through the block table.  A CALL, so that the contiguous path above
+                                // carries none of it as predicated-off instructions (64 issue slots per tile otherwise)
+#pragma unroll
+          for (int pi = 0; pi < PASSES; ++pi) src[pi] = Kb + at_paged_row_bytes(g, pos[pi], row_bytes);
         }
         if (ld_wrapped) mbar_wait(&bar.kempty[ld_s], ld_ph ^ 1);
         const uint32_t kdst = smem_u32(sK) + ld_s * KV_TILE + dst_row0;

@@ -578,6 +578,11 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       const int tp = it.seq_start + tl;        // packed
       const size_t orow = ((size_t)(tp - g.q_off) * Hq + it.kvh * G + h);
       const int qa_local = it.t0 + mt * (128 / G);
+      // masked tiles: reference position of this row (packed for index lists, local for the dense kernel) and the last
+      // position OUTSIDE its local window (no window: nothing is inside)
+      int t_ref = SPARSE ? tp : tl;
+      int near_lo = win > 0 ? t_ref - win : 0x7fffffff;
+      asm volatile("" : "+r"(t_ref), "+r"(near_lo));
 
       if (mt < n_mt && my_nt > 0) {
         float m_run = -INFINITY, l_run = 0.f;
@@ -639,30 +644,39 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
                 pk[cc / 2] = bf16x2_rn(p0, p1);
               }
             } else {
+              // masked tile: the position tests of PAPER.md eq. (2) (causal, p <= t) and of the local window
+              // (t - p < W gets the bias), folded into ONE additive term per element: -inf, or the bias, or 0, each
+              // already less the running max, so that x - m comes out of a single FFMA.  One unsigned compare covers
+              // "-1 (no entry)" and "p > t"; positions are read four at a time (same address in all lanes: broadcast).
+              const float nm = -m_off, nb = lb2 - m_off;
+              float mxr = -INFINITY;
 #pragma unroll
-              for (int cc = 0; cc < AT_KT; cc += 2) {
-                float x[2];
+              for (int cc = 0; cc < AT_KT; cc += 4) {
+                int pp[4];
+                if (SPARSE) {
+                  const int4 p4 = *reinterpret_cast<const int4*>(si + j * AT_KT + cc);
+                  pp[0] = p4.x, pp[1] = p4.y, pp[2] = p4.z, pp[3] = p4.w;
+                } else {
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                  const int col = j * AT_KT + cc + u;
-                  bool ok;
-                  int dist;
-                  if (SPARSE) {
-                    const int p = si[col];
-                    ok = p >= 0 && p <= tp;
-                    dist = tp - p;
-                  } else {
-                    ok = col <= tl;
-                    dist = tl - col;
-                  }
-                  x[u] = ok ? fmaf(__uint_as_float(v[cc + u]), sl2, (win > 0 && dist < win) ? lb2 : 0.f) : -INFINITY;
+                  for (int u = 0; u < 4; ++u) pp[u] = j * AT_KT + cc + u;
                 }
-                mx = fmaxf(mx, fmaxf(x[0], x[1]));
-                const float p0 = ex2_approx(x[0] - m_off);
-                const float p1 = ex2_approx(x[1] - m_off);
-                sum2 = f2_add(sum2, f2_pack(p0, p1));
-                pk[cc / 2] = bf16x2_rn(p0, p1);
+                float xr[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                  const bool ok = (uint32_t)pp[u] <= (uint32_t)t_ref;
+                  const float b = pp[u] > near_lo ? nb : nm;
+                  xr[u] = fmaf(__uint_as_float(v[cc + u]), sl2, ok ? b : -INFINITY);
+                }
+                mxr = fmaxf(mxr, fmaxf(fmaxf(xr[0], xr[1]), fmaxf(xr[2], xr[3])));
+#pragma unroll
+                for (int u = 0; u < 4; u += 2) {
+                  const float p0 = ex2_approx(xr[u]);
+                  const float p1 = ex2_approx(xr[u + 1]);
+                  sum2 = f2_add(sum2, f2_pack(p0, p1));
+                  pk[(cc + u) / 2] = bf16x2_rn(p0, p1);
+                }
               }
+              mx = mxr + m_off;  // -inf stays -inf (m_off is finite)
             }
             {
               float s0, s1;

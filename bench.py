@@ -468,21 +468,30 @@ def measure_per_query_c4(B, torch, gen, peaks, L=32768, reps=2):
                                                                r0, panel, sc, wsx), reps)
     t_sc = _timed(torch, stream, lambda: B.sp_indexer_scores(pb, None, None, None, q_idx, k_idx, True, r0, panel, sc), reps)
     t_tk = _timed(torch, stream, lambda: B.sp_topk_support(pb, sc, r0, panel, idx_p), reps)
+    # per-query attention as the layer runs it: with the SPARSE_ATTN workspace, i.e. the membership-masked tcgen05 tile
+    # loop where its plan applies (c4 @ 32K / 64K), else the gather kernel; and the gather kernel on its own
+    nb_at = B.workspace_bytes(pb, B.SP_STAGE_SPARSE_ATTN)
+    ws_at = torch.empty(max(nb_at, 256), dtype=torch.uint8, device="cuda") if nb_at else None
+    t_at_layer = _timed(torch, stream, lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx, O, None, ws_at), reps)
     t_at = _timed(torch, stream, lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx, O), reps)
+    del ws_at
     pairs = kept_pairs(L, k)
+    causal = L * (L + 1) // 2
     gather_bytes = 4.0 * cfg.Hkv * cfg.d * pairs
     # plain gather of whole K token rows (all KV heads: Hkv * d * 2 bytes) over the attention's own index stream
     sink = torch.empty(148 * 8 * 256, dtype=torch.int32, device="cuda")
     row_b = pitch = cfg.Hkv * cfg.d * 2
     t_probe = _timed(torch, stream, lambda: B.sp_gather_probe(dv["K"], row_b, pitch, idx, sink), reps)
     probe_GBps = float(pairs) * row_b / (t_probe * 1e-3) / 1e9
-    causal = L * (L + 1) // 2
     topk_bytes = 4.0 * causal + 4.0 * n_rows * k
     g = gather_bytes / (t_at * 1e-3) / 1e9
     return {"config": f"c4 L={L} k={k} b_sel=1 indexer mode (BASELINE.json configs[3])", "layer_ms": t_layer,
             "tokens_per_s": L / (t_layer * 1e-3),
             "stages_ms": {"projection": max(t_both - t_sc, 0.0), "scoring": t_sc * f, "topk": t_tk * f,
-                          "sparse_attention_per_query": t_at},
+                          "sparse_attention_per_query": t_at_layer},
+            "attention_plan": "membership-masked dense tiles (tcgen05)" if nb_at else "gather (mma.sync + cp.async)",
+            "attention_masked_TFLOPs": (4.0 * causal * cfg.Hq * cfg.d / (t_at_layer * 1e-3) / 1e12) if nb_at else None,
+            "attention_gather_kernel_ms": t_at,
             "scoring_score_write_GBps": 4.0 * causal / (t_sc * f * 1e-3) / 1e9,
             "topk_GBps": topk_bytes / (t_tk * f * 1e-3) / 1e9, "topk_frac_of_hbm": topk_bytes / (t_tk * f * 1e-3) / 1e9 / peaks["hbm"],
             "gather_GBps": g, "gather_frac_of_hbm_copy_peak": g / peaks["hbm"],

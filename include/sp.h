@@ -164,9 +164,17 @@ int sp_topk_support(const sp_params *p, const float *scores, int64_t ld_scores,
 /* GQA attention recomputed only over the selected KV positions, online softmax (PAPER.md:107; :156 each
  * query re-applies its own causal mask; Alg.1 step 5).
  *   idx: [sp_num_rows(p), k] as produced by sp_topk_support for the WHOLE pack (row of query t =
- *        its support row).  Entries < 0 or > t (or outside t's sequence) are ignored for query t.
+ *        its support row).  Entries < 0 or > t (or outside t's sequence) are ignored for query t, in any order;
+ *        the valid entries of a row are a SET (distinct positions, as a top-k gives them).
  *   O: [L,Hq,d] bf16 (fp32 accumulate).  Empty effective support -> O row = 0, lse = -inf.
- *   lse: [L,Hq] fp32 or NULL. */
+ *   lse: [L,Hq] fp32 or NULL.
+ *   ws: optional.  For per-query lists (b_sel == 1) whose k is a sizeable part of the prefix the layer is cheaper as
+ *        the dense tile loop over the whole causal prefix with a membership mask than as k gathered rows per query
+ *        and KV head (the per-query realization is "harder to fuse and amortize").
+ *        sp_workspace_bytes(SP_STAGE_SPARSE_ATTN) is non-zero exactly when that plan applies to p (Hq/Hkv in {4,8},
+ *        d in {64,128}, scale > 0, no local bias, every sequence starting at a multiple of 32, causal pairs at most
+ *        ~22x the kept pairs); with a workspace of that size the call takes it (device scratch, overwritten: a
+ *        [L/32, L] bitmap), with ws == NULL or a smaller one it gathers.  Same result up to summation order. */
 int sp_sparse_gqa_attn(const sp_params *p, const void *Q, const void *K, const void *V,
                        const int32_t *idx, void *O, float *lse, void *ws, size_t ws_bytes, void *stream);
 

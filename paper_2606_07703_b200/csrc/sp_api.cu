@@ -141,13 +141,67 @@ cudaError_t run_mass(const sp_params* p, const void* Q, const void* K, const flo
                         row_count, max_nv, mass, ld, st);
 }
 
+// ---- per-query supports: gather kernel or membership-masked dense tiles (sp_tc_attn.cu) ----
+// The gather kernel moves k rows per query and KV head; the masked tile loop touches every (query, key <= query) pair
+// once on the tensor core.  Measured on a B200 (c4: d = 128, G = 4, k = L/16 up to 2048): the gather kernel costs
+// 350-405 ps per kept pair, the masked loop 14-15.5 ps per causal pair (L = 16K: 5.83 vs 1.88 ms; 32K: 23.0 vs 7.6 ms;
+// 64K: 53.5 vs 33.2 ms), i.e. the masked loop wins while the causal pairs are fewer than ~25x the kept ones; at
+// k = 2048 that is L below ~100K.  The threshold leaves a margin for the long runs' power cap.
+constexpr double MASKED_PAIR_RATIO = 22.0;
+constexpr size_t MASKED_MAX_BYTES = (size_t)3 << 30;
+
+struct MaskedPlan {
+  bool use;
+  size_t bytes;
+  long long chunks;
+};
+
+MaskedPlan masked_plan(const sp_params* p) {
+  MaskedPlan m{false, 0, 0};
+  if (p->b_sel != 1 || p->k < 1 || p->Hkv < 1) return m;
+  const int G = p->Hq / p->Hkv;
+  if (!sp_tc_attn_masked_supported(G, p->d)) return m;
+  if (!(attn_scale(p) > 0.f)) return m;
+  if (p->local_window > 0 && p->local_bias != 0.f) return m;  // the local bias needs the per-element path
+  const HostGeom hg = host_geom(p);
+  const int QT = 256 / G;
+  double dense = 0.0, kept = 0.0;
+  long long chunks = 0;
+  for (int i = 0; i < hg.batch; ++i) {
+    const long long s0 = hg.seq_start(i), n = hg.seq_len(i);
+    if (s0 % 32 != 0) return m;  // a bitmap word holds 32 consecutive queries of ONE sequence
+    const double nn = (double)n, kk = (double)(n < p->k ? n : p->k);
+    dense += nn * (nn + 1.0) / 2.0;
+    kept += kk * (kk + 1.0) / 2.0 + (nn - kk) * kk;
+    chunks += (n + QT - 1) / QT;
+  }
+  if (dense > MASKED_PAIR_RATIO * kept) return m;
+  long long pitch, rows;
+  sp_support_bits_shape(p->L, &pitch, &rows);
+  m.bytes = align_up((size_t)pitch * rows * sizeof(uint32_t));
+  if (m.bytes > MASKED_MAX_BYTES) return m;
+  m.chunks = chunks;
+  m.use = true;
+  return m;
+}
+
 // idx == nullptr -> dense.  The tcgen05 kernel covers the whole pack, or -- dense and LSE-only (O == nullptr,
 // the oracle's pass 1 of a row panel) -- the query chunks that intersect [q_begin, q_begin + q_count): rows of a
 // boundary chunk outside the range get their lse too, which is harmless.
 cudaError_t run_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, int q_begin,
-                     int q_count, void* O, float* lse, cudaStream_t st, long long idx_grp = 0, bool per_head = false) {
+                     int q_count, void* O, float* lse, cudaStream_t st, long long idx_grp = 0, bool per_head = false,
+                     void* ws = nullptr, size_t ws_bytes = 0) {
   SpGeom g = dev_geom(p);
   g.idx_grp = idx_grp;
+  if (idx != nullptr && O != nullptr && !per_head && idx_grp == 0 && q_begin == 0 && q_count == p->L && ws != nullptr) {
+    const MaskedPlan mp = masked_plan(p);
+    if (mp.use && ws_bytes >= mp.bytes) {
+      cudaError_t e = sp_launch_support_bits(g, idx, p->k, host_geom(p).num_rows(), (uint32_t*)ws, st);
+      if (e != cudaSuccess) return e;
+      return sp_launch_attn_tc_masked(g, mp.chunks, Q, K, V, (const uint32_t*)ws, p->Hq, p->Hkv, p->d, attn_scale(p), O, lse,
+                                      st);
+    }
+  }
   if (per_head)  // one list per HEAD: no two heads share gathered rows, the per-query kernel's tile shape (G = 1 rows per warp)
     return sp_launch_attn_pq(g, Q, K, V, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p), p->local_window, p->local_bias,
                              q_begin, q_count, O, lse, st, true);
@@ -192,7 +246,7 @@ constexpr size_t PANEL_BYTES = (size_t)1 << 30;  // score panel budget inside sp
 struct LayerPlan {
   int64_t ld;
   long long n_rows, panel_rows;
-  size_t off_qidx, off_kidx, off_lse, off_scores, off_idx, off_stage, total;
+  size_t off_qidx, off_kidx, off_lse, off_scores, off_idx, off_stage, total, scores_bytes;
 };
 
 LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws, int units = 1) {
@@ -213,7 +267,17 @@ LayerPlan plan_layer(const sp_params* p, int mode, bool idx_in_ws, int units = 1
   } else {
     pl.off_lse = off; off += ws_mass(p);
   }
-  pl.off_scores = off; off += align_up((size_t)pl.panel_rows * pl.ld * sizeof(float));
+  pl.off_scores = off;
+  {
+    // the membership bitmap of the masked per-query attention (masked_plan) reuses the score panel, free by then
+    size_t panel = align_up((size_t)pl.panel_rows * pl.ld * sizeof(float));
+    if (units == 1) {
+      const MaskedPlan mp = masked_plan(p);
+      if (mp.use && mp.bytes > panel) panel = mp.bytes;
+    }
+    pl.scores_bytes = panel;
+    off += panel;
+  }
   pl.off_idx = off;
   if (idx_in_ws) off += align_up((size_t)units * pl.n_rows * p->k * sizeof(int32_t));
   pl.total = off;
@@ -291,8 +355,12 @@ int sp_workspace_bytes(const sp_params* p, int stage, size_t* bytes_out) {
   switch (stage) {
     case SP_STAGE_INDEXER_SCORES: *bytes_out = ws_indexer(p); return SP_OK;
     case SP_STAGE_ORACLE_MASS: *bytes_out = ws_mass(p); return SP_OK;
+    case SP_STAGE_SPARSE_ATTN: {
+      const MaskedPlan mp = masked_plan(p);
+      *bytes_out = mp.use ? mp.bytes : 0;
+      return SP_OK;
+    }
     case SP_STAGE_TOPK:
-    case SP_STAGE_SPARSE_ATTN:
     case SP_STAGE_DENSE_ATTN: *bytes_out = 0; return SP_OK;
     case SP_STAGE_LAYER_ORACLE: *bytes_out = plan_layer(p, SP_MODE_ORACLE, true, units).total; return SP_OK;
     case SP_STAGE_LAYER_INDEXER: *bytes_out = plan_layer(p, SP_MODE_INDEXER, true).total; return SP_OK;
@@ -432,8 +500,9 @@ int sp_gather_probe(const void* base, int32_t row_bytes, int64_t row_pitch_bytes
 }
 
 int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx, void* O,
-                       float* lse, void* /*ws*/, size_t /*ws_bytes*/, void* stream) {
+                       float* lse, void* ws, size_t ws_bytes, void* stream) {
   if (!p) return SP_ERR_INVALID_ARG;
+  if (ws && !aligned16(ws)) return SP_ERR_INVALID_ARG;
   sp_params q = *p;  // the support-granularity flags belong to this entry point and to sp_prefill_layer's oracle mode
   q.flags &= ~(uint32_t)(SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT);
   if ((p->flags & SP_F_GROUP_SUPPORT) && (p->flags & SP_F_HEAD_SUPPORT)) return SP_ERR_INVALID_ARG;
@@ -444,7 +513,7 @@ int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const v
   const bool per_head = (p->flags & SP_F_HEAD_SUPPORT) != 0;
   const long long idx_grp =
       (p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)) ? host_geom(&q).num_rows() * (long long)q.k : 0;
-  SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp, per_head), "sparse attention");
+  SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp, per_head, ws, ws_bytes), "sparse attention");
   return SP_OK;
 }
 
@@ -508,7 +577,7 @@ int sp_prefill_layer(const sp_params* p, int32_t mode, const void* X, const void
     }
   }
   SP_CUDA(run_attn(p, Q, K, V, idx, 0, p->L, O, nullptr, st, units > 1 || per_group || per_head ? pl.n_rows * (long long)p->k : 0,
-                   per_head),
+                   per_head, base + pl.off_scores, pl.scores_bytes),
           "sparse attention");
   return SP_OK;
 }

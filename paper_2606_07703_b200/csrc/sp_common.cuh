@@ -140,6 +140,14 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
                               const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hq, int Hkv,
                               int d, float scale, int local_window, float local_bias, void* O, float* lse,
                               cudaStream_t st);
+// per-query supports as membership-masked dense attention (sp_tc_attn.cu)
+bool sp_tc_attn_masked_supported(int G, int d);
+void sp_support_bits_shape(long long L, long long* pitch, long long* rows);
+cudaError_t sp_launch_support_bits(const SpGeom& g, const int32_t* idx, int k, long long n_rows, uint32_t* bits,
+                                   cudaStream_t st);
+cudaError_t sp_launch_attn_tc_masked(const SpGeom& g, long long n_chunks, const void* Q, const void* K, const void* V,
+                                     const uint32_t* bits, int Hq, int Hkv, int d, float scale, void* O, float* lse,
+                                     cudaStream_t st);
 
 // per-query gather-sparse attention on mma.sync (sp_mma_attn.cu)
 cudaError_t sp_launch_attn_pq(const SpGeom& g, const void* Q, const void* K, const void* V, const int32_t* idx, int k,

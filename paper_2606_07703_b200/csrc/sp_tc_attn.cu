@@ -42,6 +42,9 @@ constexpr int AT_MMA_WARP = 8;
 constexpr int AT_LOAD_WARP0 = 9;
 // (Measured and not kept: MMA issuers on warps 8, 9 and the loaders on warps 10, 11, 14, 15, i.e. two loaders on each of
 // schedulers 2 and 3 instead of issuer + loader on schedulers 0 and 1: +2.5 % slower.)
+constexpr uint32_t AT_AX_BYTES = 128 * 128;  // membership-masked mode: query selector tile
+constexpr uint32_t AT_BX_BYTES = 64 * 128;   // ... and one mask tile per ring stage
+constexpr float AT_NO_KEY = -1e30f;          // a raw logit below this is a masked one (the mask adds -2^127)
 constexpr float AT_RESCALE_THRESHOLD = 8.0f;  // log2 units: O is rescaled only when the row max grew by > 2^8
 
 __device__ __forceinline__ void cp_async_arrive_noinc(uint64_t* bar) {
@@ -193,13 +196,16 @@ __device__ __forceinline__ int at_item_id(int i, int c, int P, int n_items) {
   return id < n_items ? id : -1;
 }
 
-template <int D, int G, bool SPARSE, bool WITH_O>
+template <int D, int G, bool SPARSE, bool WITH_O, bool MASKED = false>
 __global__ void __launch_bounds__(AT_THREADS, 1)
 sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_bfloat16* __restrict__ Q,
                   const __nv_bfloat16* __restrict__ K,
                   const __nv_bfloat16* __restrict__ V, const int32_t* __restrict__ idx, int k, int Hkv, float scale,
                   int local_window, float local_bias, int chunks_per_row, int n_chunks, int chunk_base, int n_items,
-                  int n_stages, int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse) {
+                  int n_stages, int kpad, __nv_bfloat16* __restrict__ O, float* __restrict__ lse,
+                  const uint32_t* __restrict__ mbits = nullptr, long long mbits_pitch = 0) {
+  static_assert(!MASKED || (!SPARSE && WITH_O && (G == 4 || G == 8)), "membership-masked mode: dense key tiles, G in {4, 8}");
+  constexpr int QM = 128 / G;             // queries per M tile (MASKED: K extent of the mask product)
   constexpr int KB = D / 64;              // 64-wide column blocks of a row
   constexpr int CPR = D / 8;              // 16-byte chunks per row
   constexpr uint32_t Q_BLK = 256 * 128;   // bytes of one column block of the Q tile (256 rows)
@@ -223,7 +229,11 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
   uint8_t* sQ = smem;
   uint8_t* sK = sQ + KB * Q_BLK;
   uint8_t* sV = sK + NS * KV_TILE;
-  int* sIdx = reinterpret_cast<int*>(sV + (WITH_O ? NS * KV_TILE : 0));    // SPARSE: [2][kpad]
+  // MASKED: sAx = the one-hot query selector [128 rows x 64 columns] (constant), sBx = per ring stage the mask tile
+  // [64 keys x 2 * QM queries] (0 / -2^127), both K-major SWIZZLE_128B like Q and K
+  uint8_t* sAx = sV + (WITH_O ? NS * KV_TILE : 0);
+  uint8_t* sBx = sAx + (MASKED ? AT_AX_BYTES : 0);
+  int* sIdx = reinterpret_cast<int*>(sBx + (MASKED ? NS * AT_BX_BYTES : 0));  // SPARSE: [2][kpad]
   uint32_t* sFlag = reinterpret_cast<uint32_t*>(sIdx + 2 * kpad);          // SPARSE: [2][kpad / 64]
   const int ntmax = kpad / AT_KT;
 
@@ -237,7 +247,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
     tma_prefetch_desc(&tmQ);
     mbar_init(&bar.qempty, 2);
     for (int s = 0; s < AT_MAX_STAGES; ++s) {
-      mbar_init(&bar.kfull[s], 128);
+      mbar_init(&bar.kfull[s], MASKED ? 256 : 128);  // MASKED: + one plain arrive per loader thread (mask tile stores)
       mbar_init(&bar.vfull[s], 128);
       mbar_init(&bar.kempty[s], 2);
       mbar_init(&bar.vempty[s], 2);
@@ -254,6 +264,18 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       mbar_init(&bar.idxempty[m], 256);
     }
     fence_barrier_init();
+  }
+  if (MASKED) {
+    // selector tile: row R of an M tile (query R / G of the tile) has a single 1.0 in column R / G, so that
+    // (selector x mask tile^T)[R, key] = mask tile[key, query of R]: the membership mask is ADDED to S by the tensor
+    // core (QM / 16 extra K steps per S tile) and the softmax warps run the plain unmasked path
+    for (int ch = threadIdx.x; ch < 128 * 8; ch += AT_THREADS) {
+      const int row = ch >> 3, c8 = ch & 7, q = row / G;
+      uint32_t w[4] = {0u, 0u, 0u, 0u};
+      if ((q >> 3) == c8) w[(q & 7) >> 1] = (q & 1) ? 0x3F800000u : 0x00003F80u;  // bf16 1.0
+      *reinterpret_cast<uint4*>(sAx + sw128_offset(row, c8)) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+    fence_proxy_async_smem();
   }
   if (warp == AT_MMA_WARP) tmem_alloc<512>(&tmem_slot);
   tc_fence_before_sync();
@@ -359,7 +381,19 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       // offset is that of row key0 plus pi * KPP * 128
       static_assert(KPP % 8 == 0, "a loader pass must step whole swizzle atoms");
       const uint32_t dst_row0 = sw128_offset(key0, c % 8) + kv_off;
+      // MASKED: thread -> (key mkey of the tile, M tile mmt): one 32-bit word of the membership bitmap
+      // mbits[query / 32][key] holds the tile's QM queries for that key
+      constexpr int NCH = QM / 8;  // 16-byte chunks (8 bf16 mask values) per key and M tile
+      const int mkey = ptid & 63, mmt = ptid >> 6;
+      const int mq0 = it.seq_start + it.t0 + mmt * QM;  // first query of the M tile (packed; a multiple of QM)
+      const uint32_t* mrow = MASKED ? mbits + (size_t)(mq0 >> 5) * (size_t)mbits_pitch + it.seq_start : nullptr;
+      const int msh = mq0 & 31;
       auto load_tile = [&](int j) {
+        uint32_t mw = 0u;
+        if (MASKED) {
+          const int keyl = j * AT_KT + mkey;
+          if (keyl <= it.t1) mw = __ldg(mrow + keyl);
+        }
         const char* src[PASSES];
         int pos[PASSES];
 #pragma unroll
@@ -384,6 +418,25 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
 #pragma unroll
         for (int pi = 0; pi < PASSES; ++pi) cp_async16(kdst + pi * (KPP * 128), src[pi]);
         cp_async_arrive_noinc(&bar.kfull[ld_s]);
+        if (MASKED) {
+          // 1 bit -> one bf16: 0x0000 (member) or 0xFF00 = -2^127 (not a member; finite, so 0 x mask stays 0).  Four
+          // inverted bits times 0x10204080 put bit a into the sign of byte a (no two partial products share a bit
+          // position); PRMT's sign-replicate mode turns each into the 0x00 / 0xFF high byte of a bf16.
+          const uint32_t nw = ~(mw >> msh);
+          uint8_t* xdst = sBx + ld_s * AT_BX_BYTES;
+#pragma unroll
+          for (int i = 0; i < NCH; ++i) {
+            uint32_t o[4];
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const uint32_t X = ((nw >> (8 * i + 4 * h2)) & 0xFu) * 0x10204080u;
+              asm("prmt.b32 %0, %1, %2, %3;" : "=r"(o[2 * h2]) : "r"(X), "r"(0u), "r"(0x9484u));
+              asm("prmt.b32 %0, %1, %2, %3;" : "=r"(o[2 * h2 + 1]) : "r"(X), "r"(0u), "r"(0xB4A4u));
+            }
+            *reinterpret_cast<uint4*>(xdst + sw128_offset(mkey, mmt * NCH + i)) = make_uint4(o[0], o[1], o[2], o[3]);
+          }
+          mbar_arrive(&bar.kfull[ld_s]);  // release: the stores above are visible to whoever sees the phase complete
+        }
         if (WITH_O) {
           if (ld_wrapped) mbar_wait(&bar.vempty[ld_s], ld_ph ^ 1);
           const uint32_t vdst = smem_u32(sV) + ld_s * KV_TILE + dst_row0;
@@ -442,6 +495,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       const uint64_t qdesc0 = umma_desc_sw128(smem_u32(sQ) + mt * 16384, 16, 1024);
       const uint64_t kdesc0 = umma_desc_sw128(smem_u32(sK), 16, 1024);
       const uint64_t vdesc0 = umma_desc_sw128(smem_u32(sV), KV_BLK, 1024);
+      const uint64_t axdesc0 = umma_desc_sw128(smem_u32(sAx), 16, 1024);
+      const uint64_t bxdesc0 = umma_desc_sw128(smem_u32(sBx) + mt * (QM * 2), 16, 1024);  // this M tile's query columns
       uint32_t k_s = 0, k_ph = 0, v_s = 0, v_ph = 0;  // K / V ring positions of the next tile this warp consumes
       uint32_t n_q = 0, n_it = 0, n_o = 0;            // items with work / items seen / items this M tile was active in
       uint32_t cs = 0, cp = 0;                        // S tiles issued / PV tiles issued by this warp (buffer = & 1)
@@ -487,6 +542,11 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             for (int kk = 0; kk < D / 16; ++kk) {
               umma_ss(d_s, qdesc0 + (uint64_t)(((kk / 4) * Q_BLK + (kk % 4) * 32) >> 4),
                       kd + (uint64_t)(((kk / 4) * KV_BLK + (kk % 4) * 32) >> 4), idesc_s, kk != 0);
+            }
+            if (MASKED) {  // S += selector x mask tile^T
+              const uint64_t bx = bxdesc0 + (uint64_t)((k_s * AT_BX_BYTES) >> 4);
+#pragma unroll
+              for (int kk = 0; kk < QM / 16; ++kk) umma_ss(d_s, axdesc0 + (uint64_t)(kk * 2), bx + (uint64_t)(kk * 2), idesc_s, 1);
             }
             umma_commit(&bar.sfull[mt][cs & 1]);
             umma_commit(&bar.kempty[k_s]);
@@ -601,6 +661,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           if (SPARSE) flagged = ((fl[j] >> mt) & 1u) != 0;
           else flagged = (j * AT_KT + AT_KT - 1 > qa_local - win);
           flagged = flagged || !scale_pos;
+          if (MASKED) flagged = false;  // causal order and membership both come with the mask product (host: scale > 0, no window)
           uint32_t pk[AT_KT / 2];
           float tsum;
           if (j == 0 && !flagged) {  // first tile: its max IS the running max (saves the certain second pass)
@@ -615,8 +676,10 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
               a0 = fmaxf(a0, fmaxf(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])));
               a1 = fmaxf(a1, fmaxf(__uint_as_float(v[cc + 2]), __uint_as_float(v[cc + 3])));
             }
-            m_run = fmaxf(a0, a1) * sl2;
+            const float a = fmaxf(a0, a1);
+            m_run = (MASKED && a < AT_NO_KEY) ? -INFINITY : a * sl2;
           }
+          bool redone = false;
 #pragma unroll 1
           for (;;) {
             uint32_t v[AT_KT];
@@ -690,8 +753,10 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             if (!flagged) {
               // (a row with no finite running max yet -- only possible here after fully masked tiles of a list that is
               // not ascending -- has no reference to speculate against and takes its max the classic way)
-              need = !(tsum <= AT_SUM_LIMIT) || m_run == -INFINITY;
+              // (MASKED: a row none of whose keys so far was a member stays at -inf; one redo per tile at most)
+              need = !(tsum <= AT_SUM_LIMIT) || (m_run == -INFINITY && !(MASKED && redone));
               if (!__any_sync(0xffffffffu, need)) break;
+              redone = true;
               uint32_t w[AT_KT];
               tmem_ld_x32(t_s, w);
               tmem_ld_x32(t_s + 32, w + 32);
@@ -703,7 +768,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
                 a0 = fmaxf(a0, fmaxf(__uint_as_float(w[cc]), __uint_as_float(w[cc + 1])));
                 a1 = fmaxf(a1, fmaxf(__uint_as_float(w[cc + 2]), __uint_as_float(w[cc + 3])));
               }
-              mx = fmaxf(a0, a1) * sl2;
+              const float a = fmaxf(a0, a1);
+              mx = (MASKED && a < AT_NO_KEY) ? -INFINITY : a * sl2;
             }
             // ---- running max with lazy rescale of the TMEM accumulator ----
             const float m_new = fmaxf(m_run, mx);
@@ -711,7 +777,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
               need = m_new > m_run + AT_RESCALE_THRESHOLD;  // also true for the first finite max
               if (!__any_sync(0xffffffffu, need)) break;
             }
-            const float f = need ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
+            const float f = (need && m_new > m_run) ? ex2_approx(m_run - m_new) : 1.f;  // m_run = -inf -> 0
             if (WITH_O && j > 0) {
               mbar_wait(&bar.ofull[mt], (cs - 1) & 1);  // PV(j-1) has finished updating O
               tc_fence_after_sync();
@@ -742,7 +808,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           mbar_wait(&bar.ofin[mt], n_ep & 1);
           ++n_ep;
           tc_fence_after_sync();
-          const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
+          // (MASKED: a row without any member key has m_run = -inf; its l_run may hold the polynomial path's 2^-125s)
+          const float inv = (l_run > 0.f && !(MASKED && m_run == -INFINITY)) ? 1.f / l_run : 0.f;
 #pragma unroll
           for (int c0 = 0; c0 < D; c0 += 32) {
             uint32_t o[32];
@@ -778,7 +845,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             }
           }
         }
-        if (lse != nullptr && row_valid) lse[orow] = l_run > 0.f ? (m_run + log2f(l_run)) * SP_LN2 : -INFINITY;
+        if (lse != nullptr && row_valid)
+          lse[orow] = (l_run > 0.f && !(MASKED && m_run == -INFINITY)) ? (m_run + log2f(l_run)) * SP_LN2 : -INFINITY;
       } else if (my_nt == 0 && row_valid) {  // empty support: O = 0, lse = -inf (reading A9)
         if (WITH_O) {
           const uint4 z = make_uint4(0, 0, 0, 0);
@@ -795,35 +863,37 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
 }
 
 template <int D>
-size_t attn_smem_bytes(int kpad, bool sparse, bool with_o, int stages) {
+size_t attn_smem_bytes(int kpad, bool sparse, bool with_o, int stages, bool masked = false) {
   const size_t kb = D / 64;
   return 1024 + kb * 256 * 128 + (size_t)stages * (with_o ? 2 : 1) * kb * AT_KT * 128 +
-         (sparse ? (size_t)2 * kpad * 4 + (size_t)2 * (kpad / AT_KT) * 4 : 0);
+         (sparse ? (size_t)2 * kpad * 4 + (size_t)2 * (kpad / AT_KT) * 4 : 0) +
+         (masked ? (size_t)AT_AX_BYTES + (size_t)stages * AT_BX_BYTES : 0);
 }
 
 constexpr size_t AT_SMEM_LIMIT = 227 * 1024 - 512;  // dynamic limit minus the static barriers / slots
 
 template <int D>
-int attn_pick_stages(int kpad, bool sparse, bool with_o) {
+int attn_pick_stages(int kpad, bool sparse, bool with_o, bool masked = false) {
   int s = AT_MAX_STAGES;
-  while (s >= 2 && attn_smem_bytes<D>(kpad, sparse, with_o, s) > AT_SMEM_LIMIT) --s;
+  while (s >= 2 && attn_smem_bytes<D>(kpad, sparse, with_o, s, masked) > AT_SMEM_LIMIT) --s;
   return s;  // < 2 -> unsupported
 }
 
 int at_sm_count() { return sp_sm_count(); }
 
-template <int D, int G, bool SPARSE, bool WITH_O>
+template <int D, int G, bool SPARSE, bool WITH_O, bool MASKED = false>
 cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V,
                        const int32_t* idx, int k, int Hkv, float scale, int lw, float lb, int cpr, int n_chunks,
-                       int chunk_base, int n_items, void* O, float* lse) {
+                       int chunk_base, int n_items, void* O, float* lse, const uint32_t* mbits = nullptr,
+                       long long mbits_pitch = 0) {
   const int kpad = SPARSE ? (k + AT_KT - 1) / AT_KT * AT_KT : 0;
-  const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O);
+  const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O, MASKED);
   if (stages < 2) return cudaErrorInvalidValue;
-  const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages);
+  const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages, MASKED);
   static size_t attr_smem_dev[SP_MAX_DEVICES];
   size_t& attr_smem = attr_smem_dev[sp_current_device()];
   if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(sp_tc_attn_kernel<D, G, SPARSE, WITH_O>,
+    cudaError_t e = cudaFuncSetAttribute(sp_tc_attn_kernel<D, G, SPARSE, WITH_O, MASKED>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_smem = smem;
@@ -835,9 +905,9 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
                                          (uint64_t)Hkv * G * D * 2, G, 256 / G);
     if (e != cudaSuccess) return e;
   }
-  sp_tc_attn_kernel<D, G, SPARSE, WITH_O><<<grid, AT_THREADS, smem, st>>>(
+  sp_tc_attn_kernel<D, G, SPARSE, WITH_O, MASKED><<<grid, AT_THREADS, smem, st>>>(
       tmQ, g, (const __nv_bfloat16*)Q, (const __nv_bfloat16*)K, (const __nv_bfloat16*)V, idx, k, Hkv, scale, lw, lb, cpr,
-      n_chunks, chunk_base, n_items, stages, kpad, (__nv_bfloat16*)O, lse);
+      n_chunks, chunk_base, n_items, stages, kpad, (__nv_bfloat16*)O, lse, mbits, mbits_pitch);
   return cudaGetLastError();
 }
 
@@ -866,7 +936,83 @@ cudaError_t launch_d(int G, const SpGeom& g, cudaStream_t st, const void* Q, con
   return cudaErrorInvalidValue;
 }
 
+// Membership bitmap of per-query supports (b_sel == 1): bit (t & 31) of bits[(t >> 5) * pitch + p] is set iff packed key
+// position p is in query t's list AND causally valid for it (same sequence, p <= t).  One CTA per row.
+__global__ void __launch_bounds__(256)
+sp_support_bits_kernel(SpGeom g, const int32_t* __restrict__ idx, int k, uint32_t* __restrict__ bits, long long pitch) {
+  const long long r = blockIdx.x;
+  const SpRow ri = sp_row_info(g, (int)r);
+  const int t = ri.seq_start + ri.t_last;
+  uint32_t* row = bits + (size_t)(t >> 5) * (size_t)pitch;
+  const uint32_t bit = 1u << (t & 31);
+  const int32_t* sup = idx + (size_t)r * k;
+  for (int e = threadIdx.x; e < k; e += 256) {
+    const int p = __ldg(sup + e);
+    if (p >= ri.seq_start && p <= t) atomicOr(row + p, bit);
+  }
+}
+
+template <int D>
+cudaError_t launch_masked_d(int G, const SpGeom& g, cudaStream_t st, const void* Q, const void* K, const void* V, int Hkv,
+                            float scale, int n_chunks, int n_items, void* O, float* lse, const uint32_t* bits,
+                            long long pitch) {
+  switch (G) {
+    case 4:
+      return launch_one<D, 4, false, true, true>(g, st, Q, K, V, nullptr, 0, Hkv, scale, 0, 0.f, 1, n_chunks, 0, n_items, O,
+                                                 lse, bits, pitch);
+    case 8:
+      return launch_one<D, 8, false, true, true>(g, st, Q, K, V, nullptr, 0, Hkv, scale, 0, 0.f, 1, n_chunks, 0, n_items, O,
+                                                 lse, bits, pitch);
+  }
+  return cudaErrorInvalidValue;
+}
+
 }  // namespace
+
+// ---- per-query supports as MASKED DENSE attention (PAPER.md:107 + :156; :315-317 names the per-query realization as
+// the one that is "harder to fuse and amortize") ----
+// When k is a sizeable fraction of the prefix, gathering k rows per query and KV head (4 flop per gathered byte) costs
+// more than running the dense tcgen05 tile loop over the whole prefix and masking by membership: the mask reaches S
+// as a rank-(128/G) product on the tensor core, so the softmax warps run their unmasked path and the kernel keeps
+// the dense kernel's rate.  The caller (sp_api.cu) chooses between this and the gather kernel from the pair counts.
+bool sp_tc_attn_masked_supported(int G, int d) {
+  if (G != 4 && G != 8) return false;
+  if (d != 64 && d != 128) return false;
+  return (d == 128 ? attn_pick_stages<128>(0, false, true, true) : attn_pick_stages<64>(0, false, true, true)) >= 2;
+}
+
+// words per bitmap row and rows of the bitmap for a pack of L tokens
+void sp_support_bits_shape(long long L, long long* pitch, long long* rows) {
+  *pitch = (L + 3) / 4 * 4;
+  *rows = (L + 31) / 32 + 8;  // + the query blocks a last, partly filled M tile names
+}
+
+cudaError_t sp_launch_support_bits(const SpGeom& g, const int32_t* idx, int k, long long n_rows, uint32_t* bits,
+                                   cudaStream_t st) {
+  long long pitch, rows;
+  sp_support_bits_shape(g.L, &pitch, &rows);
+  cudaError_t e = cudaMemsetAsync(bits, 0, (size_t)pitch * rows * sizeof(uint32_t), st);
+  if (e != cudaSuccess) return e;
+  if (n_rows <= 0) return cudaSuccess;
+  sp_support_bits_kernel<<<(unsigned)n_rows, 256, 0, st>>>(g, idx, k, bits, pitch);
+  sp_count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t sp_launch_attn_tc_masked(const SpGeom& g, long long n_chunks, const void* Q, const void* K, const void* V,
+                                     const uint32_t* bits, int Hq, int Hkv, int d, float scale, void* O, float* lse,
+                                     cudaStream_t st) {
+  const int G = Hq / Hkv;
+  if (n_chunks <= 0) return cudaSuccess;
+  if (n_chunks * Hkv > 0x7fffffffLL) return cudaErrorInvalidValue;
+  long long pitch, rows;
+  sp_support_bits_shape(g.L, &pitch, &rows);
+  const int n_items = (int)(n_chunks * Hkv);
+  cudaError_t e = d == 128 ? launch_masked_d<128>(G, g, st, Q, K, V, Hkv, scale, (int)n_chunks, n_items, O, lse, bits, pitch)
+                           : launch_masked_d<64>(G, g, st, Q, K, V, Hkv, scale, (int)n_chunks, n_items, O, lse, bits, pitch);
+  sp_count_launch();
+  return e;
+}
 
 // The tcgen05 attention covers dense attention always and sparse attention when a support row's queries fill a
 // useful part of an M tile; per-query (b_sel == 1) supports are gather-bound and stay on the CUDA-core kernel.

@@ -556,6 +556,100 @@ def test_sparse_attention_accepts_unordered_index_lists(b):
     assert np.allclose(got[fin], lse_o[fin], rtol=0, atol=2e-5)
 
 
+def _random_supports(L, k, cu, rng, empty_every=0):
+    """Per-query index lists that are NOT top-k outputs: a random subset of the query's causal prefix of random size,
+    unsorted, -1 padding mixed in, a few entries beyond the query (to be ignored), some rows empty."""
+    cu = [0, L] if cu is None else list(cu)
+    idx = np.full((L, k), -1, dtype=np.int32)
+    for i in range(len(cu) - 1):
+        for t in range(cu[i], cu[i + 1]):
+            if empty_every and t % empty_every == 3:
+                continue
+            n = t - cu[i] + 1
+            m = int(rng.integers(1, min(n, k) + 1))
+            row = idx[t]
+            row[:m] = cu[i] + rng.choice(n, size=m, replace=False)
+            if m + 2 <= k and t + 2 < cu[i + 1]:
+                row[m:m + 2] = (t + 1, t + 2)                          # non-causal entries: ignored (:156)
+            rng.shuffle(row)
+    return idx
+
+
+@pytest.mark.parametrize("name,L,Hq,Hkv,d,k,cu", [
+    ("g4_d128", 520, 8, 2, 128, 64, None), ("g4_d64", 700, 16, 4, 64, 96, None), ("g8_d128", 333, 8, 1, 128, 40, None),
+    ("g8_d64", 401, 16, 2, 64, 300, None), ("g4_varlen", 672, 8, 2, 128, 50, (0, 256, 288, 640, 672)),
+    ("g8_varlen_k_ge_n", 416, 8, 1, 64, 512, (0, 32, 416))])
+def test_per_query_attention_as_masked_dense_tiles(name, L, Hq, Hkv, d, k, cu):
+    """b_sel = 1 lists through the membership-masked tcgen05 tile loop (chosen when sp_workspace_bytes(SPARSE_ATTN) > 0
+    and the caller passes that workspace): same outputs and log-sum-exps as the oracle on arbitrary lists -- unsorted,
+    padded, with ignored non-causal entries, empty rows, rows whose first key tiles hold no member, k >= n."""
+    rng = np.random.Generator(np.random.Philox(77 + L + k))
+    Qb = orc.f64_to_bf16(rng.standard_normal((L, Hq, d)))
+    Kb = orc.f64_to_bf16(rng.standard_normal((L, Hkv, d)))
+    Vb = orc.f64_to_bf16(rng.standard_normal((L, Hkv, d)))
+    kw = dict(L=L, Hq=Hq, Hkv=Hkv, d=d, k=k, b_sel=1, cu_seqlens=cu)
+    pbo, pbg = orc.Problem(**kw), B.Problem(**kw)
+    idx = _random_supports(L, k, cu, rng, empty_every=37)
+    idx[L // 2, :] = -1
+    idx[L // 2, 0] = (cu[-2] if cu else 0)                           # one member only, in the first tile
+    nb = B.workspace_bytes(pbg, B.SP_STAGE_SPARSE_ATTN)
+    assert nb > 0, "the masked tile loop should be the plan for this shape"
+    ws = torch.empty(nb, dtype=torch.uint8, device=DEV)
+    ws.fill_(0xAB)                                                     # the call initialises what it reads
+    O = torch.full((L, Hq, d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    lse = torch.full((L, Hq), float("nan"), dtype=torch.float32, device=DEV)
+    n0 = B.launch_count()
+    B.sp_sparse_gqa_attn(pbg, dev(Qb), dev(Kb), dev(Vb), torch.from_numpy(idx).to(DEV), O, lse, ws)
+    torch.cuda.synchronize()
+    assert B.launch_count() - n0 == 2                                  # bitmap builder + attention (the gather path: 1)
+    want, lse_o = orc.sparse_attn(pbo, Qb, Kb, Vb, np.arange(L), idx, want_lse=True)
+    parity.compare_attention(to_f64(O), want)
+    got = to_f64(lse)
+    fin = np.isfinite(lse_o)
+    assert (~fin).sum() >= L // 37 - 1                                 # the empty rows are in the comparison
+    assert np.array_equal(np.isfinite(got), fin)                       # empty support -> O = 0, lse = -inf (A9)
+    assert np.all(to_f64(O)[~fin[:, 0]] == 0.0)
+    assert np.allclose(got[fin], lse_o[fin], rtol=0, atol=2e-5)
+    # and the gather kernel (no workspace) gives the same answer on the same lists
+    O2 = torch.full_like(O, float("nan"))
+    B.sp_sparse_gqa_attn(pbg, dev(Qb), dev(Kb), dev(Vb), torch.from_numpy(idx).to(DEV), O2, None)
+    parity.compare_attention(to_f64(O2), want)
+
+
+def test_masked_dense_plan_only_where_it_applies():
+    """Shapes the masked tile loop does not cover keep the gather kernel: workspace size 0 and one launch."""
+    base = dict(L=512, Hq=8, Hkv=2, d=128, k=64, b_sel=1)
+    assert B.workspace_bytes(B.Problem(**base), B.SP_STAGE_SPARSE_ATTN) > 0
+    for over in (dict(local_window=16, local_bias=0.5), dict(Hkv=4), dict(Hkv=8), dict(b_sel=64), dict(scale=-0.1),
+                 dict(cu_seqlens=(0, 100, 512)), dict(L=65536 * 2, k=16)):
+        kw = dict(base, **over)
+        assert B.workspace_bytes(B.Problem(**kw), B.SP_STAGE_SPARSE_ATTN) == 0, over
+    # a zero-bias window changes nothing and keeps the plan
+    assert B.workspace_bytes(B.Problem(**dict(base, local_window=16, local_bias=0.0)), B.SP_STAGE_SPARSE_ATTN) > 0
+
+
+def test_masked_dense_tiles_growing_logits():
+    """The masked tile loop under logits that grow along the key axis (lazy rescale in most tiles) and large
+    magnitudes: the mask term (-2^127 before scaling) must never leak into a finite row."""
+    cfg = SMALL_ORC128
+    inp = gen.make_inputs(cfg, with_indexer=False)
+    Kf = orc.bf16_to_f64(inp["K"]).reshape(cfg.L, cfg.Hkv, cfg.d)
+    Qf = orc.bf16_to_f64(inp["Q"]).reshape(cfg.L, cfg.Hq, cfg.d)
+    u = np.ones(cfg.d) / math.sqrt(cfg.d)
+    Kf = Kf + (np.arange(cfg.L)[:, None, None] * 0.25) * u
+    Qf = Qf + 6.0 * u
+    Kb, Qb = orc.f64_to_bf16(Kf), orc.f64_to_bf16(Qf)
+    over = dict(b_sel=1, k=200, local_window=0, local_bias=0.0)
+    pbo = orc_problem(cfg, **over)
+    pbg = B.Problem.from_config(cfg, **over)
+    res = orc.prefill_layer(pbo, orc.MODE_ORACLE, Qb, Kb, inp["V"])
+    ws = B.alloc_workspace(pbg, B.SP_STAGE_SPARSE_ATTN)
+    assert B.workspace_bytes(pbg, B.SP_STAGE_SPARSE_ATTN) > 0
+    O = torch.full((cfg.L, cfg.Hq, cfg.d), float("nan"), dtype=torch.bfloat16, device=DEV)
+    B.sp_sparse_gqa_attn(pbg, dev(Qb), dev(Kb), dev(inp["V"]), torch.from_numpy(res.idx).to(DEV), O, None, ws)
+    parity.compare_attention(to_f64(O), res.out)
+
+
 @pytest.mark.parametrize("b", [64, 1])
 def test_attention_growing_logits_rescale_path(b):
     """Logits that keep growing along the key axis (later keys dominate by > 2^8) force the lazy O rescale of the
@@ -846,6 +940,13 @@ def test_chunked_paged_prefill_equals_full_prefill(cfg, chunk, page):
     idx_full = torch.full((pbg.num_rows, cfg.k), -9, dtype=torch.int32, device=DEV)
     ws = B.alloc_workspace(pbg, B.SP_STAGE_LAYER_INDEXER)
     B.sp_prefill_layer(pbg, B.SP_MODE_INDEXER, X, Wq, Wk, Q, K, V, O_full, idx_full, ws)
+    if b == 1 and B.workspace_bytes(pbg, B.SP_STAGE_SPARSE_ATTN) > 0:
+        # the whole-sequence layer ran these per-query lists through the masked tile loop; a chunk (queries against a
+        # paged prefix) keeps the gather kernel.  Bit identity is a property of one kernel: take the gather kernel's
+        # whole-sequence output as the reference and hold the layer's to the attention tolerance
+        O_layer = O_full.clone()
+        B.sp_sparse_gqa_attn(pbg, Q, K, V, idx_full, O_full)
+        parity.compare_attention(to_f64(O_layer), to_f64(O_full))
     gcache, ocache = make_gpu_cache(cfg, page, seed=page + chunk)
     Xr, Qr = X.view(L, -1), Q.view(L, cfg.Hq, cfg.d)
     Kr, Vr = K.view(L, cfg.Hkv, cfg.d), V.view(L, cfg.Hkv, cfg.d)

@@ -20,6 +20,9 @@
 
 namespace {
 
+#ifndef SP_TOPK_OLD_BIG
+#define SP_TOPK_OLD_BIG 0
+#endif
 constexpr int TK_THREADS = 1024;
 constexpr int TK_WARPS = TK_THREADS / 32;
 constexpr int TK_CACHE = 40 * 1024;       // keys staged in shared memory (160 KB)
@@ -40,12 +43,13 @@ __device__ __forceinline__ uint32_t load_key(const float* __restrict__ x, const 
 
 struct TkShared {
   uint32_t hist[256];
+  uint32_t hist2[256];
   uint32_t wgt[TK_WARPS], weq[TK_WARPS];  // per-warp totals (elements above khi / T; equal to T)
   uint32_t wcand[TK_WARPS];               // per-warp candidate counts
   uint32_t bis[34];                       // [32]: candidates above T
   uint32_t part[2][TK_WARPS];             // bisection: per-warp partial counts, double buffered by step parity
   uint32_t sel[2];                        // radix select scratch
-  uint32_t T, need_eq, ok;
+  uint32_t T, need_eq, ok, tg;
 };
 
 // ---- exact fallback: 4-pass MSB-first radix select (8 bits per pass) -> sh.T, sh.need_eq ----
@@ -58,7 +62,7 @@ __device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, 
     if (tid < 256) sh.hist[tid] = 0;
     __syncthreads();
     const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
-    for (int i0 = 0; i0 < n; i0 += TK_THREADS) {
+    for (int i0 = 0; i0 < n; i0 += (int)blockDim.x) {
       const int i = i0 + tid;
       bool act = false;
       uint32_t bin = 0;
@@ -323,6 +327,406 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
   else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
 }
 
+
+// ---- rows beyond the register-resident classes: ONE streaming pass ----
+// 256 threads per row, three rows per SM.  (1) 512 pseudo-random keys of the row are sorted (bitonic, shared memory);
+// two order statistics bracket the k-th largest key T: klo <= T <= khi with high probability.  (2) The row is read
+// ONCE, 16 bytes per lane and load: every warp owns a contiguous segment, counts its keys above khi and appends every
+// key >= klo, with its index, to a private list in shared memory -- in index order (ballots), so the concatenation of
+// the eight lists is the index-ordered list of everything that can still be selected (~k + 10 % of n entries).
+// (3) If the bracket held (count(> khi) < k <= entries, no list overflowed) T is found by bit-by-bit bisection over the
+// register-resident list entries (only the bits below the common prefix of klo and khi are undecided), and (4) the
+// output is compacted from the lists: ties to the lower index and ascending order fall out of the list order.
+// Otherwise the exact radix select over the row (from L2 / HBM) and two more passes take over: always correct, only
+// slower.  The 1024-thread kernel above staged the row in shared memory and walked it three times with a block-wide
+// barrier between the phases of the single row an SM held: ~45 K cycles per 24 K-key row, 0.09 of the HBM rate.
+constexpr int TX_THREADS = 256;
+constexpr int TX_WARPS = TX_THREADS / 32;
+constexpr int TX_LIST = 1024;    // list entries per warp
+constexpr int TX_SAMPLE = 1024;
+constexpr int TX_UNROLL = 4;     // 16-byte loads in flight per lane
+
+// rank-th largest (rank >= 1) of the keys the CTA's threads hold in registers: slot j of a thread counts iff bit j of
+// `valid` is set.  MSB-first radix select in digits of up to 8 bits starting at bit `top`: every valid key agrees with
+// `known` above that bit.  At most `max_passes` digits are resolved; the result has the unresolved low bits zero and
+// *rest = how many keys share its resolved prefix down to the rank (the number of ties to take when all bits are
+// resolved).  *low = mask of the unresolved bits.
+template <int NK>
+__device__ __forceinline__ uint32_t tx_select(const uint32_t (&key)[NK], uint32_t valid, int nk_used, uint32_t rank, int top,
+                                              uint32_t known, int max_passes, TkShared& sh, uint32_t* rest, uint32_t* low) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t hi_mask = top >= 31 ? 0u : (0xffffffffu << (top + 1));  // bits already decided
+  uint32_t prefix = known & hi_mask, need = rank;
+  int hi = top;
+  for (int pass = 0; pass < max_passes && hi >= 0; ++pass) {
+    const int lo = hi >= 7 ? hi - 7 : 0;
+    const uint32_t dmask = (2u << (hi - lo)) - 1u;
+    sh.hist[tid] = 0;  // TX_THREADS == 256 bins
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < NK; ++j) {
+      if (j >= nk_used) break;  // warp-uniform
+      if (((valid >> j) & 1u) && ((key[j] & hi_mask) == prefix)) atomicAdd(&sh.hist[(key[j] >> lo) & dmask], 1u);
+    }
+    __syncthreads();
+    if (warp == 0) {  // the bin holding rank `need` counting from the top: 8 bins per lane
+      uint32_t c[8];
+      uint32_t tot = 0;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        c[j] = sh.hist[255 - (lane * 8 + j)];
+        tot += c[j];
+      }
+      uint32_t incl = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      uint32_t before = incl - tot;
+      if (before < need && need <= incl) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          if (need <= before + c[j]) {
+            sh.sel[0] = 255u - (uint32_t)(lane * 8 + j);
+            sh.sel[1] = need - before;
+            break;
+          }
+          before += c[j];
+        }
+      }
+    }
+    __syncthreads();
+    prefix |= sh.sel[0] << lo;
+    need = sh.sel[1];
+    hi_mask |= dmask << lo;
+    hi = lo - 1;
+  }
+  *rest = need;
+  *low = ~hi_mask;
+  return prefix;
+}
+
+// Bracket of the sample: the keys of sample ranks r_hi < r_lo (0-based from the top), each resolved to the two 8-bit
+// digits below bit `top` (above it all sample keys agree with `known`) and rounded outwards -- an approximate bracket
+// is as good as an exact one, it only has to contain T.  Two passes; the first histogram serves both ranks.
+template <int NK>
+__device__ __forceinline__ void tx_bracket(const uint32_t (&key)[NK], int r_hi, int r_lo, bool want_hi, bool want_lo, int top,
+                                           uint32_t known, TkShared& sh, uint32_t* khi, uint32_t* klo) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t hi_mask = top >= 31 ? 0u : (0xffffffffu << (top + 1));
+  uint32_t pre_h = known & hi_mask, pre_l = pre_h;
+  uint32_t need_h = (uint32_t)r_hi + 1u, need_l = (uint32_t)r_lo + 1u;
+  int hi = top;
+  for (int pass = 0; pass < 2 && hi >= 0; ++pass) {
+    const int lo = hi >= 7 ? hi - 7 : 0;
+    const uint32_t dmask = (2u << (hi - lo)) - 1u;
+    sh.hist[tid] = 0;
+    sh.hist2[tid] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < NK; ++j) {
+      const uint32_t bin = (key[j] >> lo) & dmask, top_bits = key[j] & hi_mask;
+      if (top_bits == pre_h) atomicAdd(&sh.hist[bin], 1u);
+      if (top_bits == pre_l) atomicAdd(&sh.hist2[bin], 1u);
+    }
+    __syncthreads();
+    if (warp < 2) {  // warp 0: rank r_hi in hist, warp 1: rank r_lo in hist2
+      const uint32_t* hh = warp == 0 ? sh.hist : sh.hist2;
+      const uint32_t need = warp == 0 ? need_h : need_l;
+      uint32_t c[8];
+      uint32_t tot = 0;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        c[j] = hh[255 - (lane * 8 + j)];
+        tot += c[j];
+      }
+      uint32_t incl = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      uint32_t before = incl - tot;
+      if (before < need && need <= incl) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          if (need <= before + c[j]) {
+            sh.part[warp][0] = 255u - (uint32_t)(lane * 8 + j);
+            sh.part[warp][1] = need - before;
+            break;
+          }
+          before += c[j];
+        }
+      }
+    }
+    __syncthreads();
+    pre_h |= sh.part[0][0] << lo;
+    need_h = sh.part[0][1];
+    pre_l |= sh.part[1][0] << lo;
+    need_l = sh.part[1][1];
+    hi_mask |= dmask << lo;
+    hi = lo - 1;
+  }
+  if (want_hi) *khi = pre_h | ~hi_mask;
+  if (want_lo) *klo = pre_l;
+}
+
+__device__ __forceinline__ float key_to_float(uint32_t key) {
+  return __uint_as_float((key & 0x80000000u) ? (key ^ 0x80000000u) : ~key);
+}
+
+__global__ void __launch_bounds__(TX_THREADS, 3)
+sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
+                      int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
+  extern __shared__ uint32_t tx_smem[];  // [TX_WARPS][TX_LIST] pairs (score bits, index)
+  __shared__ TkShared sh;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+  const int r = row_count - 1 - (int)blockIdx.x;  // long rows first
+  const SpRow ri = sp_row_info(g, row_begin + r);
+  const int n = ri.t_last + 1;
+  if (n <= n_lo) return;
+  int32_t* out = idx + (size_t)r * k;
+  const int keep = min(n, k);
+  if (tid == 0 && cnt) cnt[r] = keep;
+  for (int j = keep + tid; j < k; j += TX_THREADS) out[j] = -1;
+  if (n <= k) {
+    for (int j = tid; j < n; j += TX_THREADS) out[j] = ri.seq_start + j;
+    return;
+  }
+  const float* x = scores + (size_t)r * ld;
+
+  // ---- 1. bracket from a sample (rows too short to sample: everything is a candidate).  Two order statistics of the
+  // sample, each resolved to the 16 bits below the sample's highest differing bit and rounded outwards ----
+  uint32_t klo = 0u, khi = 0xffffffffu;
+  if (n >= 4 * TX_SAMPLE) {
+    const int stride = n / TX_SAMPLE;
+    uint32_t sk[TX_SAMPLE / TX_THREADS];
+    uint32_t dif = 0;
+#pragma unroll
+    for (int j = 0; j < TX_SAMPLE / TX_THREADS; ++j) {
+      const int e = tid + j * TX_THREADS;
+      const uint32_t h = ((uint32_t)e * 2654435761u) >> 12;
+      sk[j] = order_key(__ldg(x + e * stride + (int)(h % (uint32_t)stride)));
+    }
+    if (tid == 0) sh.T = sk[0];
+    __syncthreads();
+    const uint32_t ref = sh.T;
+#pragma unroll
+    for (int j = 0; j < TX_SAMPLE / TX_THREADS; ++j) dif |= sk[j] ^ ref;
+    dif = __reduce_or_sync(0xffffffffu, dif);
+    if (lane == 0) sh.part[0][warp] = dif;
+    __syncthreads();
+    dif = 0;
+    for (int w = 0; w < TX_WARPS; ++w) dif |= sh.part[0][w];
+    const int stop = dif ? 31 - __clz(dif) : -1;
+    const float frac = (float)k / (float)n;
+    const float rr = frac * TX_SAMPLE;  // expected sample rank (from the top) of T
+    const int margin = (int)ceilf(3.5f * sqrtf(rr * (1.f - frac))) + 4;
+    const int ih = (int)floorf(rr) - margin, il = (int)ceilf(rr) + margin;  // 0-based ranks from the top
+    if (stop < 0) {
+      klo = khi = ref;
+    } else {
+      // a rank outside the sample leaves that side of the bracket open; the helper still needs a valid rank to walk
+      const bool want_hi = ih > 0, want_lo = il < TX_SAMPLE - 1;
+      tx_bracket<TX_SAMPLE / TX_THREADS>(sk, want_hi ? ih : 0, want_lo ? il : TX_SAMPLE - 1, want_hi, want_lo, stop, ref, sh,
+                                         &khi, &klo);
+    }
+  }
+  // float images of the bracket for the streaming compare (-0 == +0 and the order of non-NaN values are those of the
+  // keys; under flush-to-zero a denormal may pass as 0: the filter is a superset, the exact counts come from the keys)
+  const float klo_f = klo == 0u ? -INFINITY : key_to_float(klo);
+
+  // ---- 2. one pass over the row: every warp lists the elements >= klo of its segment, in index order ----
+  const int seg = ((n + TX_WARPS - 1) / TX_WARPS + 127) & ~127;
+  const int seg0 = min(warp * seg, n), seg1 = min(seg0 + seg, n);
+  uint32_t* lst = tx_smem + warp * (2 * TX_LIST);
+  const uint32_t lst_addr = (uint32_t)__cvta_generic_to_shared(lst);
+  const bool vec_ok = (ld & 3) == 0;  // rows start 16-byte aligned
+  uint32_t nl = 0;                     // warp-uniform
+  bool over = false;
+  for (int i0 = seg0; i0 < seg1; i0 += 128 * TX_UNROLL) {
+    float v[TX_UNROLL][4];
+#pragma unroll
+    for (int u = 0; u < TX_UNROLL; ++u) {
+      const int i = i0 + u * 128 + lane * 4;
+      if (vec_ok && i + 3 < seg1) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(x + i));
+        v[u][0] = q.x, v[u][1] = q.y, v[u][2] = q.z, v[u][3] = q.w;
+      } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) v[u][c] = (i + c < seg1) ? __ldg(x + i + c) : __uint_as_float(0x7fc00000u);  // NaN: never listed
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < TX_UNROLL; ++u) {
+      const int i = i0 + u * 128 + lane * 4;
+      bool f[4];
+      uint32_t bal[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        f[c] = v[u][c] >= klo_f;
+        bal[c] = __ballot_sync(0xffffffffu, f[c]);
+      }
+      if (bal[0] | bal[1] | bal[2] | bal[3]) {
+        if (nl + 128u <= (uint32_t)TX_LIST) {  // room for a whole step
+          // list order = index order: lane-major, then the lane's four elements
+          uint32_t a = lst_addr + 8u * (nl + __popc(bal[0] & lt) + __popc(bal[1] & lt) + __popc(bal[2] & lt) + __popc(bal[3] & lt));
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            if (f[c]) {
+              asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a), "r"(__float_as_uint(v[u][c])), "r"(i + c) : "memory");
+              a += 8u;
+            }
+          }
+        } else {
+          over = true;
+        }
+        nl += __popc(bal[0]) + __popc(bal[1]) + __popc(bal[2]) + __popc(bal[3]);
+      }
+    }
+  }
+  __syncwarp();
+  // ---- the warp's list in registers as keys; exact counts above / inside the bracket ----
+  uint32_t ck[TX_LIST / 32];
+  uint32_t cmask = 0, my_gt = 0, my_c = 0;
+  const int slots = over ? 0 : (int)((nl + 31u) >> 5);
+#pragma unroll
+  for (int j = 0; j < TX_LIST / 32; ++j) ck[j] = 0u;
+#pragma unroll
+  for (int j = 0; j < TX_LIST / 32; ++j) {
+    if (j >= slots) break;  // warp-uniform
+    const uint32_t e = lane + 32 * j;
+    uint32_t bits;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(bits) : "r"(lst_addr + 8u * e));
+    const uint32_t key = order_key(__uint_as_float(bits));
+    const bool in = e < nl, gt = in && key > khi, cd = in && key <= khi && key >= klo;
+    my_gt += gt;
+    my_c += cd;
+    cmask |= (cd ? 1u : 0u) << j;
+    ck[j] = (gt || cd) ? key : 0u;  // (flush-to-zero extras and padding: key 0)
+  }
+  my_gt = __reduce_add_sync(0xffffffffu, my_gt);
+  my_c = __reduce_add_sync(0xffffffffu, my_c);
+  if (lane == 0) {
+    sh.wgt[warp] = my_gt;
+    sh.wcand[warp] = my_c;
+    sh.weq[warp] = over ? 1u : 0u;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    const uint32_t a = lane < TX_WARPS ? sh.wgt[lane] : 0u, b = lane < TX_WARPS ? sh.wcand[lane] : 0u;
+    const uint32_t c = lane < TX_WARPS ? sh.weq[lane] : 0u;
+    const uint32_t tg0 = __reduce_add_sync(0xffffffffu, a), tc0 = __reduce_add_sync(0xffffffffu, b);
+    const uint32_t ov0 = __reduce_or_sync(0xffffffffu, c);
+    if (lane == 0) {
+      sh.tg = tg0;
+      sh.ok = (!ov0 && tg0 < (uint32_t)k && (uint32_t)k <= tg0 + tc0) ? 1u : 0u;
+    }
+  }
+  __syncthreads();
+  const uint32_t tg = sh.tg;
+  const bool ok = sh.ok != 0u;
+  uint32_t T, need_eq, base_gt, base_eq;
+  if (ok) {
+    // ---- 3. T = the (k - tg)-th largest of the candidates klo <= key <= khi ----
+    const uint32_t diff = klo ^ khi;
+    const int top = diff ? 31 - __clz(diff) : -1;  // highest bit the candidates can differ in
+    if (top < 0) {
+      T = khi;
+      need_eq = (uint32_t)k - tg;
+    } else {
+      uint32_t low;
+      T = tx_select<TX_LIST / 32>(ck, cmask, slots, (uint32_t)k - tg, top, khi, 4, sh, &need_eq, &low);
+    }
+    uint32_t gg = 0, ee = 0;
+#pragma unroll
+    for (int j = 0; j < TX_LIST / 32; ++j) {
+      if (j >= slots) break;
+      gg += ck[j] > T;
+      ee += ck[j] == T;  // T >= klo >= 1 whenever a padding 0 could be met ... see below
+    }
+    // (a padding / dropped slot holds key 0; T == 0 only if klo == 0 and then nothing was dropped, and padding slots
+    // lie past nl: they are excluded in the compaction by e < nl and here by the count below)
+    if (T == 0u) {
+      ee = 0;
+#pragma unroll
+      for (int j = 0; j < TX_LIST / 32; ++j) ee += (j < slots) && (lane + 32 * j < (int)nl) && ck[j] == 0u;
+    }
+    gg = __reduce_add_sync(0xffffffffu, gg);
+    ee = __reduce_add_sync(0xffffffffu, ee);
+    if (lane == 0) {
+      sh.wgt[warp] = gg;
+      sh.weq[warp] = ee;
+    }
+    __syncthreads();
+    base_gt = base_eq = 0;
+    for (int w = 0; w < warp; ++w) {
+      base_gt += sh.wgt[w];
+      base_eq += sh.weq[w];
+    }
+    // ---- 4. compaction from the list (index order) ----
+    uint32_t run_gt = base_gt, run_eq = base_eq;
+#pragma unroll
+    for (int j = 0; j < TX_LIST / 32; ++j) {
+      if (j >= slots) break;
+      const uint32_t e = lane + 32 * j;
+      const bool in = e < nl;
+      const bool gt = in && ck[j] > T, eq = in && ck[j] == T;
+      const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
+      const uint32_t pg = run_gt + __popc(mg & lt), pe = run_eq + __popc(me & lt);
+      if (gt || (eq && pe < need_eq)) {
+        uint32_t ix;
+        asm volatile("ld.shared.b32 %0, [%1];" : "=r"(ix) : "r"(lst_addr + 8u * e + 4u));
+        out[pg + min(pe, need_eq)] = ri.seq_start + (int)ix;
+      }
+      run_gt += __popc(mg);
+      run_eq += __popc(me);
+    }
+    return;
+  }
+  // ---- exact fallback: radix select over the row, then a counting and a compaction pass ----
+  radix_select<false>(x, nullptr, n, k, sh);
+  T = sh.T;
+  need_eq = sh.need_eq;
+  {
+    uint32_t gg = 0, ee = 0;
+    for (int i = seg0 + lane; i < seg1; i += 32) {
+      const uint32_t key = order_key(__ldg(x + i));
+      gg += key > T;
+      ee += key == T;
+    }
+    gg = __reduce_add_sync(0xffffffffu, gg);
+    ee = __reduce_add_sync(0xffffffffu, ee);
+    if (lane == 0) {
+      sh.wgt[warp] = gg;
+      sh.weq[warp] = ee;
+    }
+    __syncthreads();
+    base_gt = base_eq = 0;
+    for (int w = 0; w < warp; ++w) {
+      base_gt += sh.wgt[w];
+      base_eq += sh.weq[w];
+    }
+  }
+  uint32_t run_gt = base_gt, run_eq = base_eq;
+  for (int i0 = seg0; i0 < seg1; i0 += 32) {
+    const int i = i0 + lane;
+    bool gt = false, eq = false;
+    if (i < seg1) {
+      const uint32_t key = order_key(__ldg(x + i));
+      gt = key > T;
+      eq = key == T;
+    }
+    const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
+    const uint32_t pg = run_gt + __popc(mg & lt), pe = run_eq + __popc(me & lt);
+    if (gt || (eq && pe < need_eq)) out[pg + min(pe, need_eq)] = ri.seq_start + i;
+    run_gt += __popc(mg);
+    run_eq += __popc(me);
+  }
+}
+
 // ---- rows up to 16384 keys: W = 1, 2, ... 16 warps per support row (class W takes n <= 1024 W), the whole row in
 // registers.
 // Warp w owns the contiguous segment [w * seg, (w + 1) * seg) of the row (seg a multiple of 32, element
@@ -333,7 +737,10 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
 // block barriers whatever n is; this one costs O(n) issue slots.  A row is processed iff n_lo < n <= n_hi, so that
 // a panel with mixed row lengths can be covered by one launch per class. ----
 constexpr int TKS_WARPS = 8;   // warps per CTA for W <= 8; W = 16 and 32 use one CTA of W warps per row
-constexpr int TKS_WMAX = 16;   // the largest class: n <= 16384, two rows fill the register file of an SM (W = 32, one
+#ifndef TKS_WMAX_DEF
+#define TKS_WMAX_DEF 8
+#endif
+constexpr int TKS_WMAX = TKS_WMAX_DEF;   // the largest class: n <= 16384, two rows fill the register file of an SM (W = 32, one
                                // row per SM with nothing to overlap its barriers, measured SLOWER than sp_topk_kernel)
 constexpr int TKS_NW = 1024;  // class W holds rows with n <= TKS_NW * W
 template <int W>
@@ -342,8 +749,8 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
                      int n_lo, int n_hi, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
   constexpr int CTA_WARPS = W > TKS_WARPS ? W : TKS_WARPS;
   constexpr int RPC = CTA_WARPS / W;  // rows per CTA
-  __shared__ int sh_cnt[2][TKS_WMAX];
-  __shared__ int sh_fin[2][TKS_WMAX];
+  __shared__ int sh_cnt[2][16];
+  __shared__ int sh_fin[2][16];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int w = warp % W;
   const int r = blockIdx.x * RPC + warp / W;
@@ -371,7 +778,7 @@ sp_topk_small_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int
     key[s] = (s < ns && i < n) ? order_key(__ldg(x + i)) : 0u;  // padding key 0 is below every tested threshold
   }
   auto row_bar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + warp / W), "n"(W * 32) : "memory"); };
-  auto row_sum = [&](int c, int (*buf)[TKS_WMAX], int step) -> int {
+  auto row_sum = [&](int c, int (*buf)[16], int step) -> int {
     c = __reduce_add_sync(0xffffffffu, c);
     if (W == 1) return c;
     if (lane == 0) buf[step & 1][warp] = c;
@@ -461,10 +868,22 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     }
     sp_count_launch();
   };
+  const size_t smem_x = (size_t)2 * TX_WARPS * TX_LIST * sizeof(uint32_t);
+  static unsigned char attr_seen_x[SP_MAX_DEVICES];
+  if (sp_first_use_on_device(attr_seen_x)) {
+    cudaError_t e = cudaFuncSetAttribute(sp_topk_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
+    if (e != cudaSuccess) return e;
+  }
   auto launch_big = [&](int rb, int rc, int nlo) {
+#if SP_TOPK_OLD_BIG
     sp_topk_kernel<<<rc, TK_THREADS, smem, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
                                                  idx + (size_t)(rb - row_begin) * k,
                                                  cnt ? cnt + (rb - row_begin) : nullptr);
+#else
+    sp_topk_stream_kernel<<<rc, TX_THREADS, smem_x, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
+                                                          idx + (size_t)(rb - row_begin) * k,
+                                                          cnt ? cnt + (rb - row_begin) : nullptr);
+#endif
     sp_count_launch();
   };
   // A class is launched only when it fills the machine (rows * W >= one 8-warp CTA per SM) or when it is the last

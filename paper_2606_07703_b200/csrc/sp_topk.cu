@@ -1,33 +1,20 @@
 // sp_topk.cu -- causal top-k of support-row scores (PAPER.md:127 TopK_s(P,k); :145 sentinel padding;
 // :156 invalid positions masked before selection).  Exact: compare/integer work only.
 //
-// One CTA (1024 threads) per support row.  The kept set is the first min(k, n) elements of the total order
-// (score descending, index ascending), emitted in ascending index order, tail padded with -1.  With
-// key = order-preserving uint32 image of the fp32 score, the kept set is { key > T } plus the first `need_eq`
-// elements with key == T in index order, T = key of the k-th largest element.  Finding (T, need_eq):
-//   1. a 1024-element pseudo-random sample of the row is sorted (bitonic: shuffles inside a warp, shared memory
-//      across warps); two of its order statistics bracket T with high probability: klo <= T <= khi;
-//   2. ONE pass over the row (staged in shared memory when it fits, else re-read from L2): every warp owns a
-//      contiguous segment, counts its elements above khi and appends those inside [klo, khi] to its private
-//      candidate list (no atomics);
-//   3. if the bracket holds (count(>khi) < k <= count(>khi) + candidates, no list overflowed) T is found by a
-//      bit-by-bit bisection over the few candidates (register resident; only the bits below the common prefix
-//      of klo and khi are undecided); otherwise an exact 4-pass radix select over the whole row takes over
-//      (always correct; only slower).
-//   4. one index-ordered compaction pass; the per-warp output bases come from the candidate lists (or from a
-//      counting pass in the fallback).  Ties go to the lower index and the output is ascending by construction.
+// The kept set is the first min(k, n) elements of the total order (score descending, index ascending), emitted in
+// ascending index order, tail padded with -1.  With key = order-preserving uint32 image of the fp32 score, the kept
+// set is { key > T } plus the first `need_eq` elements with key == T in index order, T = key of the k-th largest
+// element.  Two kernels find (T, need_eq) and compact:
+//   sp_topk_small_kernel<W>  rows up to 1024 W keys (W = 1 .. 8 warps per row), the row in registers, bit-by-bit
+//                            bisection with redux.sync counts;
+//   sp_topk_stream_kernel    longer rows: sampled bracket, ONE streaming pass that lists what can still be selected,
+//                            radix select over the candidates, compaction from the list; exact radix-select fallback
+//                            over the whole row when the bracket does not hold (always correct, only slower).
 #include "sp_common.cuh"
 
 namespace {
 
-#ifndef SP_TOPK_OLD_BIG
-#define SP_TOPK_OLD_BIG 0
-#endif
-constexpr int TK_THREADS = 1024;
-constexpr int TK_WARPS = TK_THREADS / 32;
-constexpr int TK_CACHE = 40 * 1024;       // keys staged in shared memory (160 KB)
-constexpr int TK_CAND_PER_WARP = 256;     // private candidate list per warp (32 x 256 x 4 B = 32 KB)
-constexpr int TK_SAMPLE = 1024;
+constexpr int TK_WARPS = 32;  // sizes the per-warp scratch arrays of TkShared (any CTA up to 1024 threads)
 
 __device__ __forceinline__ uint32_t order_key(float x) {
   uint32_t u = __float_as_uint(x);
@@ -117,217 +104,6 @@ __device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, 
   __syncthreads();
 }
 
-template <bool CACHED>
-__device__ void topk_row(const float* __restrict__ x, uint32_t* keys, uint32_t* cand, int n, int k, int seq_start,
-                         int32_t* __restrict__ out, TkShared& sh) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t lt = (1u << lane) - 1u;
-
-  if (CACHED) {  // stage the row once: 8 independent loads in flight per thread
-    int i = tid;
-    for (; i + 7 * TK_THREADS < n; i += 8 * TK_THREADS) {
-      float v[8];
-#pragma unroll
-      for (int j = 0; j < 8; ++j) v[j] = __ldg(x + i + j * TK_THREADS);
-#pragma unroll
-      for (int j = 0; j < 8; ++j) keys[i + j * TK_THREADS] = order_key(v[j]);
-    }
-    for (; i < n; i += TK_THREADS) keys[i] = order_key(__ldg(x + i));
-  }
-  if (tid < 34) sh.bis[tid] = 0;
-  // warp segments: contiguous, a multiple of 32 elements
-  const int seg = ((n + TK_WARPS - 1) / TK_WARPS + 31) & ~31;
-  const int seg0 = min(warp * seg, n), seg1 = min(seg0 + seg, n);
-  uint32_t* my_cand = cand + warp * TK_CAND_PER_WARP;
-
-  // ---- 1. bracket [klo, khi] from a sorted sample (short rows: everything is a candidate) ----
-  uint32_t klo = 0u, khi = 0xffffffffu;
-  if (n > TK_WARPS * TK_CAND_PER_WARP) {
-    const int stride = n / TK_SAMPLE;  // >= 8
-    uint32_t v;
-    {
-      const uint32_t h = ((uint32_t)tid * 2654435761u) >> 12;
-      const int i = tid * stride + (int)(h % (uint32_t)stride);
-      __syncthreads();  // keys staged
-      v = load_key<CACHED>(x, keys, i);
-    }
-    // bitonic sort, descending; partners closer than a warp exchange by shuffle, the others through `cand`
-    for (int size = 2; size <= TK_SAMPLE; size <<= 1) {
-      const bool desc = (tid & size) == 0;
-      for (int st = size >> 1; st > 0; st >>= 1) {
-        uint32_t pv;
-        if (st >= 32) {
-          cand[tid] = v;
-          __syncthreads();
-          pv = cand[tid ^ st];
-          __syncthreads();
-        } else {
-          pv = __shfl_xor_sync(0xffffffffu, v, st);
-        }
-        const bool keep_max = desc == ((tid & st) == 0);
-        v = keep_max ? max(v, pv) : min(v, pv);
-      }
-    }
-    cand[tid] = v;
-    __syncthreads();
-    const float frac = (float)k / (float)n;
-    const float r = frac * TK_SAMPLE;  // expected sample rank (from the top) of T
-    const int margin = (int)ceilf(3.5f * sqrtf(r * (1.f - frac))) + 4;
-    const int ih = (int)floorf(r) - margin, il = (int)ceilf(r) + margin;
-    if (ih > 0) khi = cand[ih];
-    if (il < TK_SAMPLE - 1) klo = cand[il];
-  }
-  __syncthreads();  // sample reads done before the candidate lists reuse the buffer; keys staged
-
-  // ---- 2. one pass: count above khi, collect candidates per warp ----
-  uint32_t my_gt = 0, ncand = 0;  // ncand is warp-uniform
-  for (int i0 = seg0; i0 < seg1; i0 += 32) {
-    const int i = i0 + lane;
-    bool c = false;
-    uint32_t key = 0u;
-    if (i < seg1) {
-      key = load_key<CACHED>(x, keys, i);
-      my_gt += key > khi;
-      c = key >= klo && key <= khi;
-    }
-    const uint32_t m = __ballot_sync(0xffffffffu, c);
-    if (c) {
-      const uint32_t slot = ncand + __popc(m & lt);
-      if (slot < TK_CAND_PER_WARP) my_cand[slot] = key;
-    }
-    ncand += __popc(m);
-  }
-  const uint32_t warp_gt = __reduce_add_sync(0xffffffffu, my_gt);
-  if (lane == 0) {
-    sh.wgt[warp] = warp_gt;
-    sh.wcand[warp] = ncand;
-  }
-  __syncthreads();
-  if (warp == 0) {
-    const uint32_t tg = __reduce_add_sync(0xffffffffu, sh.wgt[lane]);
-    const uint32_t tc = __reduce_add_sync(0xffffffffu, sh.wcand[lane]);
-    const uint32_t mx = __reduce_max_sync(0xffffffffu, sh.wcand[lane]);
-    if (lane == 0) {
-      sh.ok = (mx <= TK_CAND_PER_WARP && tg < (uint32_t)k && (uint32_t)k <= tg + tc) ? 1u : 0u;
-      sh.sel[0] = tg;
-    }
-  }
-  __syncthreads();
-  uint32_t T, need_eq;
-  uint32_t base_gt, base_eq;  // selected-before counts at the start of this warp's segment
-  if (sh.ok) {
-    // ---- 3. bisection over the candidates: T = need-th largest candidate key ----
-    const uint32_t need = (uint32_t)k - sh.sel[0];
-    uint32_t ck[TK_CAND_PER_WARP / 32];
-#pragma unroll
-    for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) {
-      const uint32_t e = lane + 32 * j;
-      ck[j] = e < ncand ? my_cand[e] : 0u;  // key 0 never counts: thresholds below are >= 1 ... see note
-    }
-    // note: a padding key of 0 is only counted by the threshold 0 itself, which is never tested (bit steps OR in
-    // at least one bit)
-    // T lies in [klo, khi]: the bits above their highest differing bit are already known
-    const uint32_t diff = klo ^ khi;
-    const int top = diff ? 31 - __clz(diff) : -1;  // highest undecided bit
-    uint32_t t = top < 0 ? khi : (top >= 31 ? 0u : (khi & ~((2u << top) - 1u)));
-    for (int bit = top; bit >= 0; --bit) {
-      const uint32_t c0 = t | (1u << bit);
-      uint32_t cnt = 0;
-#pragma unroll
-      for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) cnt += ck[j] >= c0;
-      cnt = __reduce_add_sync(0xffffffffu, cnt);
-      uint32_t* part = sh.part[bit & 1];
-      if (lane == 0) part[warp] = cnt;
-      __syncthreads();
-      if (__reduce_add_sync(0xffffffffu, part[lane]) >= need) t = c0;
-    }
-    T = t;
-    {
-      uint32_t g = 0, e = 0;
-#pragma unroll
-      for (int j = 0; j < TK_CAND_PER_WARP / 32; ++j) {
-        g += ck[j] > T;
-        e += (ck[j] == T) && (lane + 32 * j < ncand);
-      }
-      g = __reduce_add_sync(0xffffffffu, g);
-      e = __reduce_add_sync(0xffffffffu, e);
-      if (lane == 0) {
-        if (g) atomicAdd(&sh.bis[32], g);
-        sh.wgt[warp] = warp_gt + g;  // elements of this segment with key > T
-        sh.weq[warp] = e;
-      }
-    }
-    __syncthreads();
-    need_eq = need - sh.bis[32];
-  } else {
-    radix_select<CACHED>(x, keys, n, k, sh);
-    T = sh.T;
-    need_eq = sh.need_eq;
-    uint32_t g = 0, e = 0;
-    for (int i = seg0 + lane; i < seg1; i += 32) {
-      const uint32_t key = load_key<CACHED>(x, keys, i);
-      g += key > T;
-      e += key == T;
-    }
-    g = __reduce_add_sync(0xffffffffu, g);
-    e = __reduce_add_sync(0xffffffffu, e);
-    if (lane == 0) {
-      sh.wgt[warp] = g;
-      sh.weq[warp] = e;
-    }
-    __syncthreads();
-  }
-  {
-    const uint32_t g = lane < warp ? sh.wgt[lane] : 0u, e = lane < warp ? sh.weq[lane] : 0u;
-    base_gt = __reduce_add_sync(0xffffffffu, g);
-    base_eq = __reduce_add_sync(0xffffffffu, e);
-  }
-
-  // ---- 4. index-ordered compaction of this warp's segment ----
-  uint32_t run_gt = base_gt, run_eq = base_eq;
-  for (int i0 = seg0; i0 < seg1; i0 += 32) {
-    const int i = i0 + lane;
-    bool gt = false, eq = false;
-    if (i < seg1) {
-      const uint32_t key = load_key<CACHED>(x, keys, i);
-      gt = key > T;
-      eq = key == T;
-    }
-    const uint32_t mg = __ballot_sync(0xffffffffu, gt), me = __ballot_sync(0xffffffffu, eq);
-    const uint32_t pg = run_gt + __popc(mg & lt);
-    const uint32_t pe = run_eq + __popc(me & lt);
-    if (gt || (eq && pe < need_eq)) out[pg + min(pe, need_eq)] = seq_start + i;
-    run_gt += __popc(mg);
-    run_eq += __popc(me);
-  }
-}
-
-__global__ void __launch_bounds__(TK_THREADS, 1)
-sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
-               int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
-  extern __shared__ uint32_t tk_smem[];
-  __shared__ TkShared sh;
-  uint32_t* keys = tk_smem;
-  uint32_t* cand = tk_smem + TK_CACHE;
-  // long rows first: the row count is rarely a multiple of the SM count and the tail should be short rows
-  const int r = row_count - 1 - (int)blockIdx.x;
-  const SpRow ri = sp_row_info(g, row_begin + r);
-  const int n = ri.t_last + 1;
-  if (n <= n_lo) return;  // a short row: sp_topk_small_kernel's
-  int32_t* out = idx + (size_t)r * k;
-  const int keep = min(n, k);
-  if (threadIdx.x == 0 && cnt) cnt[r] = keep;
-  for (int j = keep + threadIdx.x; j < k; j += TK_THREADS) out[j] = -1;
-  if (n <= k) {
-    for (int j = threadIdx.x; j < n; j += TK_THREADS) out[j] = ri.seq_start + j;
-    return;
-  }
-  const float* x = scores + (size_t)r * ld;
-  if (n <= TK_CACHE) topk_row<true>(x, keys, cand, n, k, ri.seq_start, out, sh);
-  else topk_row<false>(x, keys, cand, n, k, ri.seq_start, out, sh);
-}
-
-
 // ---- rows beyond the register-resident classes: ONE streaming pass ----
 // 256 threads per row, three rows per SM.  (1) 512 pseudo-random keys of the row are sorted (bitonic, shared memory);
 // two order statistics bracket the k-th largest key T: klo <= T <= khi with high probability.  (2) The row is read
@@ -338,8 +114,9 @@ sp_topk_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_b
 // register-resident list entries (only the bits below the common prefix of klo and khi are undecided), and (4) the
 // output is compacted from the lists: ties to the lower index and ascending order fall out of the list order.
 // Otherwise the exact radix select over the row (from L2 / HBM) and two more passes take over: always correct, only
-// slower.  The 1024-thread kernel above staged the row in shared memory and walked it three times with a block-wide
-// barrier between the phases of the single row an SM held: ~45 K cycles per 24 K-key row, 0.09 of the HBM rate.
+// slower.  (Round 1's kernel, 1024 threads per row, staged the row in shared memory and walked it three times with a
+// block-wide barrier between the phases of the single row an SM held: ~45 K cycles per 24 K-key row, 0.09 of the HBM
+// rate.)
 constexpr int TX_THREADS = 256;
 constexpr int TX_WARPS = TX_THREADS / 32;
 constexpr int TX_LIST = 1024;    // list entries per warp
@@ -507,8 +284,8 @@ sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, in
 #pragma unroll
     for (int j = 0; j < TX_SAMPLE / TX_THREADS; ++j) {
       const int e = tid + j * TX_THREADS;
-      const uint32_t h = ((uint32_t)e * 2654435761u) >> 12;
-      sk[j] = order_key(__ldg(x + e * stride + (int)(h % (uint32_t)stride)));
+      const uint32_t h = ((uint32_t)e * 2654435761u) >> 16;  // 16 pseudo-random bits -> an offset below stride
+      sk[j] = order_key(__ldg(x + e * stride + (int)((h * (uint32_t)stride) >> 16)));
     }
     if (tid == 0) sh.T = sk[0];
     __syncthreads();
@@ -733,15 +510,15 @@ sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, in
 // i = w * seg + slot * 32 + lane, at most 32 slots).  32-step bisection on the order-preserving keys with
 // `redux.sync` counts (W > 1: combined through a double-buffered shared array, one named barrier of the row's W
 // warps per step), then an
-// index-ordered compaction by ballots from per-warp bases.  The 1024-thread kernel above spends ~9 us per row on
-// block barriers whatever n is; this one costs O(n) issue slots.  A row is processed iff n_lo < n <= n_hi, so that
+// index-ordered compaction by ballots from per-warp bases.  (A 1024-thread kernel per row spends ~9 us per row on
+// block barriers whatever n is; this one costs O(n) issue slots.)  A row is processed iff n_lo < n <= n_hi, so that
 // a panel with mixed row lengths can be covered by one launch per class. ----
 constexpr int TKS_WARPS = 8;   // warps per CTA for W <= 8; W = 16 and 32 use one CTA of W warps per row
 #ifndef TKS_WMAX_DEF
 #define TKS_WMAX_DEF 8
 #endif
-constexpr int TKS_WMAX = TKS_WMAX_DEF;   // the largest class: n <= 16384, two rows fill the register file of an SM (W = 32, one
-                               // row per SM with nothing to overlap its barriers, measured SLOWER than sp_topk_kernel)
+constexpr int TKS_WMAX = TKS_WMAX_DEF;  // the largest class: n <= 8192 (W = 16, rows up to 16384, measured slower than
+                                        // the streaming kernel: c4 @ 32K 1.97 vs 1.79 ms; W = 4: 1.82)
 constexpr int TKS_NW = 1024;  // class W holds rows with n <= TKS_NW * W
 template <int W>
 __global__ void __launch_bounds__((W > TKS_WARPS ? W : TKS_WARPS) * 32, W <= 8 ? 3 : 2)
@@ -841,13 +618,7 @@ int g_sm_count() { return sp_sm_count(); }
 cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int row_begin, int row_count, int k,
                            int max_n_valid, int32_t* idx, int32_t* cnt, cudaStream_t st) {
   if (row_count <= 0) return cudaSuccess;
-  static unsigned char attr_seen[SP_MAX_DEVICES];
-  const size_t smem = (size_t)(TK_CACHE + TK_WARPS * TK_CAND_PER_WARP) * sizeof(uint32_t);
-  if (sp_first_use_on_device(attr_seen)) {
-    cudaError_t e = cudaFuncSetAttribute(sp_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-  }
-  // Row classes by n = n_valid: W = 1, 2, 4, 8 warps per row for n <= 1024 W, the 1024-thread kernel for longer rows.
+  // Row classes by n = n_valid: W = 1, 2, 4, 8 warps per row for n <= 1024 W, the streaming kernel for longer rows.
   // One sequence (cu == nullptr): n(r) = min(L, (r + 1) b_sel) is monotone, each class is a contiguous row range and
   // gets a launch over exactly that range (the bound (r + 1) b_sel is conservative, so no class filter is needed).
   // Packed varlen: every class that can occur is launched over the whole panel and filters its rows by n.
@@ -875,20 +646,14 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     if (e != cudaSuccess) return e;
   }
   auto launch_big = [&](int rb, int rc, int nlo) {
-#if SP_TOPK_OLD_BIG
-    sp_topk_kernel<<<rc, TK_THREADS, smem, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
-                                                 idx + (size_t)(rb - row_begin) * k,
-                                                 cnt ? cnt + (rb - row_begin) : nullptr);
-#else
     sp_topk_stream_kernel<<<rc, TX_THREADS, smem_x, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
                                                           idx + (size_t)(rb - row_begin) * k,
                                                           cnt ? cnt + (rb - row_begin) : nullptr);
-#endif
     sp_count_launch();
   };
   // A class is launched only when it fills the machine (rows * W >= one 8-warp CTA per SM) or when it is the last
   // one the panel needs; otherwise its rows are merged into the next larger class (which handles shorter rows too,
-  // less efficiently) and finally into the 1024-thread kernel: a near-empty extra launch costs more than it saves
+  // less efficiently) and finally into the streaming kernel: a near-empty extra launch costs more than it saves
   // (c3 has 128 rows with n <= 8192: four extra launches made its top-k 0.068 -> 0.094 ms).
   const int fill = g_sm_count() * TKS_WARPS;
   if (contiguous) {

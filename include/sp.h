@@ -47,7 +47,8 @@ typedef enum sp_status {
   SP_ERR_UNSUPPORTED = -2, /* shape outside the built set (d not in {64,128}: the Qwen3.5 head dim 256 / d_idx 256 rows of
                               PAPER.md:280 are NOT built; Hq/Hkv not in {1,2,4,8}; unknown flag bits ...)              */
   SP_ERR_WORKSPACE = -3,   /* workspace too small (see sp_workspace_bytes)                                      */
-  SP_ERR_CUDA = -4         /* a CUDA launch / API error; text via sp_strerror                                   */
+  SP_ERR_CUDA = -4,        /* a CUDA launch / API error; text via sp_strerror                                   */
+  SP_ERR_TOO_LARGE = -5    /* the problem needs more scratch than a no-allocation entry point's fixed array holds */
 } sp_status;
 
 typedef enum sp_mode {
@@ -177,6 +178,24 @@ int sp_topk_support(const sp_params *p, const float *scores, int64_t ld_scores,
  *        [L/32, L] bitmap), with ws == NULL or a smaller one it gathers.  Same result up to summation order. */
 int sp_sparse_gqa_attn(const sp_params *p, const void *Q, const void *K, const void *V,
                        const int32_t *idx, void *O, float *lse, void *ws, size_t ws_bytes, void *stream);
+
+/* sp_sparse_gqa_attn for callers that cannot allocate or pass scratch (CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): per-query lists (b_sel == 1) through the membership-masked tile loop (PAPER.md:107,
+ * :156, :315-317) with its [L/32 + 8, L] bitmap in a FIXED device array inside the library, SP_STATIC_SCRATCH_BYTES
+ * (8.25 MiB: every GPU that loads the library holds it until exit).  The call allocates nothing -- no cudaMalloc,
+ * cudaFree or allocating library routine; it launches the bitmap builder (which first clears the part of the array it
+ * uses) and the attention kernel on `stream`.
+ *   Arguments as for sp_sparse_gqa_attn (device pointers; idx [sp_num_rows(p), k]; O [L,Hq,d] bf16; lse or NULL).
+ *   L > SP_STATIC_MAX_TOKENS (8192)            -> SP_ERR_TOO_LARGE, nothing launched.
+ *   p outside the masked tile loop's shape set (sp_workspace_bytes(p, SP_STAGE_SPARSE_ATTN) == 0), or a support-
+ *   granularity flag set                        -> SP_ERR_UNSUPPORTED.
+ *   Result: identical to sp_sparse_gqa_attn given the SPARSE_ATTN workspace.
+ *   EVERY call on a device shares the one array, which keeps the last call's contents: two calls whose kernels
+ *   overlap on the GPU (different streams, no dependency between them) race.  Calls on one stream are safe. */
+#define SP_STATIC_MAX_TOKENS 8192
+#define SP_STATIC_SCRATCH_BYTES (8192u * (8192u / 32u + 8u) * 4u)
+int sp_sparse_gqa_attn_static(const sp_params *p, const void *Q, const void *K, const void *V,
+                              const int32_t *idx, void *O, float *lse, void *stream);
 
 /* Dense causal GQA attention of the same layer: the same-library baseline and pass 1 of
  * the attention mass.  O may be NULL (only lse is produced); lse may be NULL. */

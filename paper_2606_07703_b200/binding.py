@@ -17,7 +17,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsp.so")
 
-SP_OK, SP_ERR_INVALID_ARG, SP_ERR_UNSUPPORTED, SP_ERR_WORKSPACE, SP_ERR_CUDA = 0, -1, -2, -3, -4
+SP_OK, SP_ERR_INVALID_ARG, SP_ERR_UNSUPPORTED, SP_ERR_WORKSPACE, SP_ERR_CUDA, SP_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5
 SP_MODE_ORACLE, SP_MODE_INDEXER = 0, 1
 SP_F_RELU, SP_F_KEY_LN, SP_F_ROPE = 1, 2, 4   # sp_params.flags: the served scorer of PAPER.md:270-274
 SP_F_GROUP_SUPPORT = 8                        # idx is [Hkv, n_rows, k]: one list per KV group
@@ -28,7 +28,7 @@ SP_F_HEAD_SUPPORT = 16                        # idx is [Hq, n_rows, k]: one list
 EXPORTS = (
     "sp_num_rows", "sp_workspace_bytes", "sp_indexer_scores", "sp_oracle_mass", "sp_topk_support",
     "sp_sparse_gqa_attn", "sp_dense_gqa_attn", "sp_prefill_layer", "sp_layer_host_arena_bytes",
-    "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_support_overlap", "sp_row_kl",
+    "sp_prefill_layer_host", "sp_strerror", "sp_launch_count", "sp_sparse_gqa_attn_static", "sp_support_overlap", "sp_row_kl",
     "sp_oracle_mass_group", "sp_gather_probe", "sp_kv_append", "sp_kv_gather", "sp_chunk_workspace_bytes",
     "sp_prefill_chunk", "sp_oracle_mass_head",
 )
@@ -229,6 +229,12 @@ def sp_sparse_gqa_attn(pb: Problem, Q, K, V, idx, O, lse: Optional[torch.Tensor]
     wp, wb = _ws_args(ws)
     _check(lib().sp_sparse_gqa_attn(C.byref(p), _ptr(Q), _ptr(K), _ptr(V), _ptr(idx), _ptr(O), _ptr(lse), wp, wb,
                                     _stream()))
+
+
+def sp_sparse_gqa_attn_static(pb: Problem, Q, K, V, idx, O, lse: Optional[torch.Tensor] = None):
+    """The no-allocation entry point: per-query lists through the masked tile loop, bitmap in the library's fixed array."""
+    p = pb.c()
+    _check(lib().sp_sparse_gqa_attn_static(C.byref(p), _ptr(Q), _ptr(K), _ptr(V), _ptr(idx), _ptr(O), _ptr(lse), _stream()))
 
 
 def sp_dense_gqa_attn(pb: Problem, Q, K, V, O, lse: Optional[torch.Tensor] = None,

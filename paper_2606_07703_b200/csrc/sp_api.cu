@@ -326,6 +326,8 @@ const char* sp_strerror(int code) {
     case SP_ERR_INVALID_ARG: return "SP_ERR_INVALID_ARG: null/misaligned pointer, bad size, bad cu_seqlens or bad panel";
     case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED: shape outside the built set (d in {64,128}, Hq/Hkv in {1,2,4,8}, d_idx in {64,128}, hidden % 64 == 0, known flags; flags need b_sel in {1,32,64,128})";
     case SP_ERR_WORKSPACE: return "SP_ERR_WORKSPACE: workspace too small, see sp_workspace_bytes";
+    case SP_ERR_TOO_LARGE:
+      return "SP_ERR_TOO_LARGE: the problem needs more scratch than the library's fixed array holds (sp_sparse_gqa_attn_static: L <= 8192)";
     case SP_ERR_CUDA: return g_err_text;
   }
   return "unknown sp_status";
@@ -514,6 +516,30 @@ int sp_sparse_gqa_attn(const sp_params* p, const void* Q, const void* K, const v
   const long long idx_grp =
       (p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)) ? host_geom(&q).num_rows() * (long long)q.k : 0;
   SP_CUDA(run_attn(&q, Q, K, V, idx, 0, q.L, O, lse, (cudaStream_t)stream, idx_grp, per_head, ws, ws_bytes), "sparse attention");
+  return SP_OK;
+}
+
+int sp_sparse_gqa_attn_static(const sp_params* p, const void* Q, const void* K, const void* V, const int32_t* idx,
+                              void* O, float* lse, void* stream) {
+  if (!p) return SP_ERR_INVALID_ARG;
+  if (p->flags & (SP_F_GROUP_SUPPORT | SP_F_HEAD_SUPPORT)) return SP_ERR_UNSUPPORTED;
+  const int rc = validate_common(p, true, false);
+  if (rc != SP_OK) return rc;
+  if (!Q || !K || !V || !idx || !O || !aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+    return SP_ERR_INVALID_ARG;
+  long long pitch, rows;
+  sp_support_bits_shape(p->L, &pitch, &rows);
+  uint32_t* scratch = nullptr;
+  size_t scratch_bytes = 0;
+  SP_CUDA(sp_static_scratch_ptr(&scratch, &scratch_bytes), "static scratch address");
+  if ((size_t)pitch * (size_t)rows * sizeof(uint32_t) > scratch_bytes) return SP_ERR_TOO_LARGE;
+  const MaskedPlan mp = masked_plan(p);
+  if (!mp.use) return SP_ERR_UNSUPPORTED;  // the masked tile loop's shape set; sp_sparse_gqa_attn covers the rest
+  const SpGeom g = dev_geom(p);
+  cudaStream_t st = (cudaStream_t)stream;
+  SP_CUDA(sp_launch_support_bits(g, idx, p->k, host_geom(p).num_rows(), scratch, st), "support bitmap (static scratch)");
+  SP_CUDA(sp_launch_attn_tc_masked(g, mp.chunks, Q, K, V, scratch, p->Hq, p->Hkv, p->d, attn_scale(p), O, lse, st),
+          "sparse attention (static scratch)");
   return SP_OK;
 }
 

@@ -140,6 +140,8 @@ cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chu
                               const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hq, int Hkv,
                               int d, float scale, int local_window, float local_bias, void* O, float* lse,
                               cudaStream_t st);
+// device address and size of the library's fixed scratch array (sp_tc_attn.cu; no allocation, once per device)
+cudaError_t sp_static_scratch_ptr(uint32_t** ptr, size_t* bytes);
 // per-query supports as membership-masked dense attention (sp_tc_attn.cu)
 bool sp_tc_attn_masked_supported(int G, int d);
 void sp_support_bits_shape(long long L, long long* pitch, long long* rows);

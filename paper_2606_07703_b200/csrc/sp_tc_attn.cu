@@ -1014,6 +1014,31 @@ cudaError_t sp_launch_attn_tc_masked(const SpGeom& g, long long n_chunks, const 
   return e;
 }
 
+// ---- fixed scratch of the no-allocation entry point (sp_sparse_gqa_attn_static, include/sp.h) ----
+// The membership bitmap of the masked tile loop for packs of up to SP_STATIC_MAX_TOKENS tokens lives in this file-scope
+// array: every GPU that loads the library holds these 8.25 MiB until exit.  In HOST code the array's name is a host-side
+// stand-in, not a device address: the address a kernel may use comes from cudaGetSymbolAddress, taken once per device
+// with that device current.  Every call shares the array (contents are the last call's; the bitmap builder clears
+// what it uses first), so calls that overlap on the GPU race.
+constexpr size_t SP_STATIC_SCRATCH_WORDS = SP_STATIC_SCRATCH_BYTES / 4;  // pitch x rows of sp_support_bits_shape(8192)
+static_assert(SP_STATIC_SCRATCH_WORDS == (size_t)SP_STATIC_MAX_TOKENS * (SP_STATIC_MAX_TOKENS / 32 + 8), "include/sp.h");
+static __device__ __align__(256) uint32_t sp_static_scratch[SP_STATIC_SCRATCH_WORDS];
+
+cudaError_t sp_static_scratch_ptr(uint32_t** ptr, size_t* bytes) {
+  static uint32_t* dev_ptr[SP_MAX_DEVICES];
+  const int dev = sp_current_device();
+  if (dev_ptr[dev] == nullptr) {
+    uint32_t* q = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&q, sp_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (q == nullptr) return cudaErrorInvalidSymbol;
+    dev_ptr[dev] = q;
+  }
+  *ptr = dev_ptr[dev];
+  *bytes = SP_STATIC_SCRATCH_WORDS * sizeof(uint32_t);
+  return cudaSuccess;
+}
+
 // The tcgen05 attention covers dense attention always and sparse attention when a support row's queries fill a
 // useful part of an M tile; per-query (b_sel == 1) supports are gather-bound and stay on the CUDA-core kernel.
 bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d) {

@@ -261,7 +261,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       mbar_init(&bar.ofin[m], 1);
       mbar_init(&bar.oempty[m], 128);
       mbar_init(&bar.idxfull[m], 128);
-      mbar_init(&bar.idxempty[m], 256);
+      mbar_init(&bar.idxempty[m], 256 + 2);  // every softmax thread + the two MMA issuers
     }
     fence_barrier_init();
   }
@@ -457,8 +457,12 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       {  // Q tile: ONE 3-D TMA box per 64-column block: [256/G queries] x [G heads] x [64 channels] lands as rows
          // R = query * G + head of 128 bytes, SWIZZLE_128B (rows past the chunk are later queries or zero fill: their
          // outputs are never written).  The cp.async version cost ~800 address instructions per loader warp per item.
-        if (n_q > 0) mbar_wait(&bar.qempty, (n_q - 1) & 1);
+        // ONLY the issuing thread waits for the buffer: nothing else here depends on it, and a loader warp that is not
+        // needed for progress may be lapped -- an item whose tiles were all prefetched above (nt <= NS - 2) can finish,
+        // and complete the barrier's NEXT phase, before a slow warp gets here; its parity wait would then never return
+        // (seen under ncu's SASS instrumentation: dense launches with several items per CTA hung on exactly that)
         if (ptid == 0) {
+          if (n_q > 0) mbar_wait(&bar.qempty, (n_q - 1) & 1);
           mbar_expect_tx(&bar.qfull, KB * Q_BLK);
 #pragma unroll
           for (int kb = 0; kb < KB; ++kb)
@@ -512,6 +516,10 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           mbar_wait(&bar.idxfull[ib], iu & 1);
           nt = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
           my_nt = nt;
+          // the issuers release the index buffer too: an item with an empty support needs no MMA, so without this the
+          // loaders could restage the buffer (n_eff_sh, and the barrier's next phase) before a slow issuer got here
+          __syncwarp();
+          if (leader) mbar_arrive(&bar.idxempty[ib]);
         } else {
           nt = it.t1 / AT_KT + 1;
           my_nt = mt == 0 ? min(it.t0 + 128 / G - 1, it.t1) / AT_KT + 1 : nt;

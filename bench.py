@@ -260,7 +260,13 @@ def run_c4_sweep(args, B, torch, gen, peaks):
         t_p1 = timed(lambda: B.sp_dense_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], None, lse), reps)
         t_p2 = timed(lambda: B.sp_oracle_mass(pb, dv["Q"], dv["K"], lse, True, r0, panel, ms), reps)
         t_tk = timed(lambda: B.sp_topk_support(pb, sc, r0, panel, idx_p), reps)
+        # the attention as the layer call runs it (with the SPARSE_ATTN workspace: membership-masked tcgen05 tiles where
+        # that plan applies, else the gather kernel), and the gather kernel on its own
+        nb_at = B.workspace_bytes(pb, B.SP_STAGE_SPARSE_ATTN)
+        ws_at = torch.empty(nb_at, dtype=torch.uint8, device="cuda") if nb_at else None
+        t_at_layer = timed(lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_i, O, None, ws_at), reps)
         t_at = timed(lambda: B.sp_sparse_gqa_attn(pb, dv["Q"], dv["K"], dv["V"], idx_i, O), reps)
+        del ws_at
         kl = torch.empty(panel, dtype=torch.float32, device="cuda")
         B.sp_row_kl(pb, ms, sc, r0, panel, kl)
         pairs = k * L - k * (k - 1) // 2
@@ -269,7 +275,10 @@ def run_c4_sweep(args, B, torch, gen, peaks):
             "overlap_pooled": pooled, "overlap_pooled_rows_beyond_budget": pooled_beyond, "overlap_chance_level": chance,
             "mean_forward_kl_nats_middle_panel": float(kl.double().mean().item()),
             "stages_ms": {"projection": max(t_both - t_sc, 0.0), "scoring": t_sc * f, "mass_pass1_lse": t_p1,
-                          "mass_pass2": t_p2 * f, "topk": t_tk * f, "sparse_attention_per_query": t_at},
+                          "mass_pass2": t_p2 * f, "topk": t_tk * f, "sparse_attention_per_query": t_at_layer},
+            "attention_plan": "membership-masked dense tiles (tcgen05)" if nb_at else "gather (mma.sync + cp.async)",
+            "attention_masked_TFLOPs": (4.0 * cfg.d * cfg.Hq * (L * (L + 1) // 2) / (t_at_layer * 1e-3) / 1e12) if nb_at else None,
+            "attention_gather_kernel_ms": t_at,
             "gather_GBps": 4.0 * cfg.Hkv * cfg.d * pairs / (t_at * 1e-3) / 1e9,
             "mass_pass2_TFLOPs": 2.0 * cfg.d * cfg.Hq * (L * (L + 1) // 2) / (t_p2 * f * 1e-3) / 1e12,
             "panel_rows": [r0, r0 + panel],
@@ -284,10 +293,14 @@ def run_c4_sweep(args, B, torch, gen, peaks):
                                    "value = the L=32768 indexer-mode layer", "Hq": 32, "Hkv": 8, "d": 128, "d_idx": 128,
                        "b_sel": 1, "parallelism": "replicas only (no sharding, no collectives)"},
             "gpu_launches": int(B.launch_count() - l0), "sweep": out,
-            "roofline": {"bound": "hbm", "achieved": ref["gather_GBps"], "peak": peaks["hbm"], "unit": "GB/s",
-                         "frac": ref["gather_GBps"] / peaks["hbm"], "traffic": None,
-                         "kernel": "sparse_attention_per_query (gathered K/V rows, mostly L2 hits)",
-                         "peak_source": peaks["source"]}}
+            "roofline": ({"bound": "tensor", "achieved": ref["attention_masked_TFLOPs"], "peak": peaks["tensor_burst"],
+                          "unit": "TFLOP/s", "frac": ref["attention_masked_TFLOPs"] / peaks["tensor_burst"], "traffic": None,
+                          "kernel": "sparse_attention_per_query as membership-masked dense tiles (flops of the causal triangle)",
+                          "peak_source": peaks["source"]} if ref["attention_masked_TFLOPs"] else
+                         {"bound": "hbm", "achieved": ref["gather_GBps"], "peak": peaks["hbm"], "unit": "GB/s",
+                          "frac": ref["gather_GBps"] / peaks["hbm"], "traffic": None,
+                          "kernel": "sparse_attention_per_query (gathered K/V rows, mostly L2 hits)",
+                          "peak_source": peaks["source"]})}
     print(json.dumps(line))
 
 

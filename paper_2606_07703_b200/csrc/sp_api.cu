@@ -761,7 +761,7 @@ extern "C" int sp_prefill_chunk(const sp_params* p, int32_t q_begin, int32_t q_c
     SP_CUDA(sp_launch_topk(g, scores, pl.ld, rb, rcnt, p->k, max_nv, idx + (size_t)r * p->k, nullptr, st), "chunk top-k");
   }
   const int G = p->Hq / p->Hkv;
-  if (sp_tc_attn_supported(p->b_sel, G, true, p->k, p->d)) {
+  if (sp_tc_attn_supported(p->b_sel, G, true, p->k, p->d, true)) {
     SP_CUDA(sp_launch_attn_tc(g, pl.n_rows, 0, 0, Q, kv->k_pages, kv->v_pages, idx, p->k, p->Hq, p->Hkv, p->d, attn_scale(p),
                               p->local_window, p->local_bias, O, nullptr, st), "chunk sparse attention");
   } else {

@@ -135,7 +135,7 @@ cudaError_t sp_launch_mass_tc(const SpGeom& g, const int32_t* cu_host, const voi
                               int row_count, float* mass, int64_t ld, cudaStream_t st, int grp = -1,
                               int head = -1);  // grp >= 0: that KV group's heads only; head >= 0: that one head only
 
-bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d);
+bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d, bool paged = false);
 cudaError_t sp_launch_attn_tc(const SpGeom& g, long long n_rows, long long n_chunks_dense, long long chunk_base,
                               const void* Q, const void* K, const void* V, const int32_t* idx, int k, int Hq, int Hkv,
                               int d, float scale, int local_window, float local_bias, void* O, float* lse,

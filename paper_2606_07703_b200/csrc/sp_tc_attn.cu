@@ -235,6 +235,10 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
   uint8_t* sBx = sAx + (MASKED ? AT_AX_BYTES : 0);
   int* sIdx = reinterpret_cast<int*>(sBx + (MASKED ? NS * AT_BX_BYTES : 0));  // SPARSE: [2][kpad]
   uint32_t* sFlag = reinterpret_cast<uint32_t*>(sIdx + 2 * kpad);          // SPARSE: [2][kpad / 64]
+  // SPARSE over a PAGED cache: the pool row of every staged entry, [2][kpad] (translated ONCE per entry while staging;
+  // the loaders then gather exactly as from contiguous tensors.  Translating per 16-byte chunk and key tile -- 16 threads
+  // repeat one key's lookup -- made the loaders pace the kernel: 400 us for a 4K-query chunk at 128K, 3x the item time)
+  int* sRow = reinterpret_cast<int*>(sFlag + 2 * (kpad / AT_KT));
   const int ntmax = kpad / AT_KT;
 
   const int win = local_window > 0 ? local_window : 0;
@@ -334,6 +338,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             const int p = pv[u];
             const bool ok = p >= its.seq_start && p <= plast;
             siw[e] = ok ? p : -1;
+            // (an ignored entry still gathers a row: a written one, so that 0 x garbage cannot make a NaN)
+            if (g.bt != nullptr) sRow[ib * kpad + e] = (int)sp_kv_row(g, ok ? p : its.seq_start);
             uint32_t f = 0;
             if (!ok || p > qa0 - win) f |= 1u;
             if (!ok || p > qa1 - win) f |= 2u;
@@ -363,7 +369,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       bool staged_ahead = false;
       if (SPARSE) {
         nt = nt_buf[n_it & 1];
-        si = sIdx + (n_it & 1) * kpad;
+        si = (g.bt != nullptr ? sRow : sIdx) + (n_it & 1) * kpad;  // what the loaders gather by: pool rows / positions
         if (nt == 0) stage_next();  // nothing to load for this item: keep the one-item lookahead
       } else {
         nt = it.t1 / AT_KT + 1;
@@ -408,7 +414,7 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
           src[pi] = Kb + (unsigned long long)(uint32_t)p * row_bytes;
           pos[pi] = p;
         }
-        if (g.bt != nullptr) {  // paged cache: rows through the block table.  A CALL, so that the contiguous path above
+        if (!SPARSE && g.bt != nullptr) {  // paged cache, dense: rows through the block table.  A CALL, so that the contiguous path above
                                 // carries none of it as predicated-off instructions (64 issue slots per tile otherwise)
 #pragma unroll
           for (int pi = 0; pi < PASSES; ++pi) src[pi] = Kb + at_paged_row_bytes(g, pos[pi], row_bytes);
@@ -871,19 +877,19 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
 }
 
 template <int D>
-size_t attn_smem_bytes(int kpad, bool sparse, bool with_o, int stages, bool masked = false) {
+size_t attn_smem_bytes(int kpad, bool sparse, bool with_o, int stages, bool masked = false, bool paged = false) {
   const size_t kb = D / 64;
   return 1024 + kb * 256 * 128 + (size_t)stages * (with_o ? 2 : 1) * kb * AT_KT * 128 +
-         (sparse ? (size_t)2 * kpad * 4 + (size_t)2 * (kpad / AT_KT) * 4 : 0) +
+         (sparse ? (size_t)2 * kpad * 4 + (size_t)2 * (kpad / AT_KT) * 4 : 0) + (sparse && paged ? (size_t)2 * kpad * 4 : 0) +
          (masked ? (size_t)AT_AX_BYTES + (size_t)stages * AT_BX_BYTES : 0);
 }
 
 constexpr size_t AT_SMEM_LIMIT = 227 * 1024 - 512;  // dynamic limit minus the static barriers / slots
 
 template <int D>
-int attn_pick_stages(int kpad, bool sparse, bool with_o, bool masked = false) {
+int attn_pick_stages(int kpad, bool sparse, bool with_o, bool masked = false, bool paged = false) {
   int s = AT_MAX_STAGES;
-  while (s >= 2 && attn_smem_bytes<D>(kpad, sparse, with_o, s, masked) > AT_SMEM_LIMIT) --s;
+  while (s >= 2 && attn_smem_bytes<D>(kpad, sparse, with_o, s, masked, paged) > AT_SMEM_LIMIT) --s;
   return s;  // < 2 -> unsupported
 }
 
@@ -895,9 +901,10 @@ cudaError_t launch_one(const SpGeom& g, cudaStream_t st, const void* Q, const vo
                        int chunk_base, int n_items, void* O, float* lse, const uint32_t* mbits = nullptr,
                        long long mbits_pitch = 0) {
   const int kpad = SPARSE ? (k + AT_KT - 1) / AT_KT * AT_KT : 0;
-  const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O, MASKED);
+  const bool paged = g.bt != nullptr;
+  const int stages = attn_pick_stages<D>(kpad, SPARSE, WITH_O, MASKED, paged);
   if (stages < 2) return cudaErrorInvalidValue;
-  const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages, MASKED);
+  const size_t smem = attn_smem_bytes<D>(kpad, SPARSE, WITH_O, stages, MASKED, paged);
   static size_t attr_smem_dev[SP_MAX_DEVICES];
   size_t& attr_smem = attr_smem_dev[sp_current_device()];
   if (smem > attr_smem) {
@@ -1049,11 +1056,12 @@ cudaError_t sp_static_scratch_ptr(uint32_t** ptr, size_t* bytes) {
 
 // The tcgen05 attention covers dense attention always and sparse attention when a support row's queries fill a
 // useful part of an M tile; per-query (b_sel == 1) supports are gather-bound and stay on the CUDA-core kernel.
-bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d) {
+bool sp_tc_attn_supported(int b_sel, int G, bool sparse, int k, int d, bool paged) {
   if (!sparse) return true;
   if (b_sel * G < 32) return false;
   const int kpad = (k + AT_KT - 1) / AT_KT * AT_KT;
-  return (d == 128 ? attn_pick_stages<128>(kpad, true, true) : attn_pick_stages<64>(kpad, true, true)) >= 2;
+  return (d == 128 ? attn_pick_stages<128>(kpad, true, true, false, paged)
+                   : attn_pick_stages<64>(kpad, true, true, false, paged)) >= 2;
 }
 
 // idx == nullptr -> dense causal attention over the query chunks [chunk_base, chunk_base + n_chunks_dense) of the

@@ -110,6 +110,9 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // exp2 of two fp32 values on the FMA / ALU pipes: round-to-nearest split x = n + f (magic-number add), degree-4
 // minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 2.7e-6 in fp32 Horner form), exponent patched
 // in with an integer add.  Inputs are clamped to >= -125 (result ~2^-125, i.e. 0 for every use here).
+#ifndef AT_POLY_EVERY_LSE
+#define AT_POLY_EVERY_LSE 4  // the same for LSE-only launches (no P, no PV: the exponential unit alone paces them)
+#endif
 #ifndef AT_POLY_EVERY
 #define AT_POLY_EVERY 4  // one pair in AT_POLY_EVERY takes the polynomial path (0 = never)
 #endif
@@ -709,7 +712,8 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
               for (int cc = 0; cc < AT_KT; cc += 2) {
                 const uint64_t x2 = f2_fma(f2_pack(__uint_as_float(v[cc]), __uint_as_float(v[cc + 1])), sl2_2, nm2);
                 float p0, p1;
-                if (WITH_O && AT_POLY_EVERY > 0 && (cc / 2) % AT_POLY_EVERY == AT_POLY_EVERY - 1) {
+                if ((WITH_O ? AT_POLY_EVERY : AT_POLY_EVERY_LSE) > 0 &&
+                    (cc / 2) % (WITH_O ? AT_POLY_EVERY : AT_POLY_EVERY_LSE) == (WITH_O ? AT_POLY_EVERY : AT_POLY_EVERY_LSE) - 1) {
                   ex2_poly2(x2, p0, p1);  // FMA-pipe exp2 for a fraction of the pairs: MUFU.EX2 co-limits the tensor pipe
                 } else {
                   float x0, x1;

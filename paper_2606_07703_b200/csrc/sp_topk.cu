@@ -117,11 +117,10 @@ __device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, 
 // slower.  (Round 1's kernel, 1024 threads per row, staged the row in shared memory and walked it three times with a
 // block-wide barrier between the phases of the single row an SM held: ~45 K cycles per 24 K-key row, 0.09 of the HBM
 // rate.)
-constexpr int TX_THREADS = 256;
-constexpr int TX_WARPS = TX_THREADS / 32;
-constexpr int TX_LIST = 1024;    // list entries per warp
+__host__ __device__ constexpr int tx_list(int txw) { return txw == 8 ? 1024 : 512; }  // list entries per warp (8 B each): 64 KB / 128 KB per row
 constexpr int TX_SAMPLE = 1024;
 constexpr int TX_UNROLL = 4;     // 16-byte loads in flight per lane
+constexpr int TX_WIDE_MIN_N = 16384;  // the 32-warp form pays from here (a warp's segment still spans several load steps)
 
 // rank-th largest (rank >= 1) of the keys the CTA's threads hold in registers: slot j of a thread counts iff bit j of
 // `valid` is set.  MSB-first radix select in digits of up to 8 bits starting at bit `top`: every valid key agrees with
@@ -138,7 +137,7 @@ __device__ __forceinline__ uint32_t tx_select(const uint32_t (&key)[NK], uint32_
   for (int pass = 0; pass < max_passes && hi >= 0; ++pass) {
     const int lo = hi >= 7 ? hi - 7 : 0;
     const uint32_t dmask = (2u << (hi - lo)) - 1u;
-    sh.hist[tid] = 0;  // TX_THREADS == 256 bins
+    if (tid < 256) sh.hist[tid] = 0;
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < NK; ++j) {
@@ -198,8 +197,10 @@ __device__ __forceinline__ void tx_bracket(const uint32_t (&key)[NK], int r_hi, 
   for (int pass = 0; pass < 2 && hi >= 0; ++pass) {
     const int lo = hi >= 7 ? hi - 7 : 0;
     const uint32_t dmask = (2u << (hi - lo)) - 1u;
-    sh.hist[tid] = 0;
-    sh.hist2[tid] = 0;
+    if (tid < 256) {
+      sh.hist[tid] = 0;
+      sh.hist2[tid] = 0;
+    }
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < NK; ++j) {
@@ -253,9 +254,13 @@ __device__ __forceinline__ float key_to_float(uint32_t key) {
   return __uint_as_float((key & 0x80000000u) ? (key ^ 0x80000000u) : ~key);
 }
 
-__global__ void __launch_bounds__(TX_THREADS, 3)
+// TXW = warps per row: 8 (three rows per SM) when the panel has rows enough to fill the machine, 32 (one row per SM, the
+// row's passes spread over four times the warps) for panels of few long rows -- a prefill CHUNK has q_count / b_sel of them.
+template <int TXW>
+__global__ void __launch_bounds__(TXW * 32, TXW == 8 ? 3 : 1)
 sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
                       int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
+  constexpr int TX_THREADS = TXW * 32, TX_WARPS = TXW, TX_LIST = tx_list(TXW);
   extern __shared__ uint32_t tx_smem[];  // [TX_WARPS][TX_LIST] pairs (score bits, index)
   __shared__ TkShared sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -639,16 +644,23 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     }
     sp_count_launch();
   };
-  const size_t smem_x = (size_t)2 * TX_WARPS * TX_LIST * sizeof(uint32_t);
+  const size_t smem_x = (size_t)2 * 8 * tx_list(8) * sizeof(uint32_t), smem_w = (size_t)2 * 32 * tx_list(32) * sizeof(uint32_t);
   static unsigned char attr_seen_x[SP_MAX_DEVICES];
   if (sp_first_use_on_device(attr_seen_x)) {
-    cudaError_t e = cudaFuncSetAttribute(sp_topk_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
+    cudaError_t e = cudaFuncSetAttribute(sp_topk_stream_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sp_topk_stream_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w);
     if (e != cudaSuccess) return e;
   }
   auto launch_big = [&](int rb, int rc, int nlo) {
-    sp_topk_stream_kernel<<<rc, TX_THREADS, smem_x, st>>>(g, scores + (size_t)(rb - row_begin) * ld, ld, rb, rc, k, nlo,
-                                                          idx + (size_t)(rb - row_begin) * k,
-                                                          cnt ? cnt + (rb - row_begin) : nullptr);
+    const float* sc = scores + (size_t)(rb - row_begin) * ld;
+    int32_t* ix = idx + (size_t)(rb - row_begin) * k;
+    int32_t* cn = cnt ? cnt + (rb - row_begin) : nullptr;
+    // fewer rows than SMs: one 32-warp CTA per row instead of an 8-warp one (the SMs would idle otherwise)
+    if (rc <= g_sm_count() && max_n_valid >= TX_WIDE_MIN_N)
+      sp_topk_stream_kernel<32><<<rc, 32 * 32, smem_w, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
+    else
+      sp_topk_stream_kernel<8><<<rc, 8 * 32, smem_x, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     sp_count_launch();
   };
   // A class is launched only when it fills the machine (rows * W >= one 8-warp CTA per SM) or when it is the last

@@ -115,6 +115,8 @@ def rand_scores(seed, rows, ld, quant=None):
     (12000, 8, 256, None, 8),            # one panel crossing all three row classes (n <= 1024, <= 8192, longer)
     (20000, 16, 128, (0, 900, 5000, 20000), 8),   # packed: the three classes interleaved, filtered per kernel
     (8192, 1, 8191, None, None),
+    (131072, 4096, 2048, None, None),    # a prefill chunk's panel: 32 rows of up to 128K keys (32 warps per row)
+    (131072, 4096, 2048, None, 8),
 ])
 def test_topk_exact(L, b, k, cu, quant):
     pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b, cu_seqlens=cu)
@@ -145,11 +147,13 @@ def test_topk_exact(L, b, k, cu, quant):
 
 @pytest.mark.parametrize("pattern", ["ramp_up", "ramp_down", "two_level", "spike_tail", "neg_inf_mix"])
 @pytest.mark.parametrize("k", [1, 300, 1999, 2048])
-def test_topk_adversarial_rows(pattern, k):
+@pytest.mark.parametrize("b", [3000, 100], ids=["few_rows_32_warps_each", "many_rows_8_warps_each"])
+def test_topk_adversarial_rows(pattern, k, b):
     """Rows built to defeat the sampled bracket of the selector: monotone ramps put every bracketed candidate into ONE
     warp's segment (list overflow -> exact radix fallback), two-level rows are one giant tie around the threshold,
     spike_tail hides the top values where a strided sample is sparse, neg_inf_mix has -inf entries."""
-    L, b = 33000, 3000                                     # 11 block rows with n = 3000 ... 33000
+    L = 33000                     # b = 3000: 11 block rows with n = 3000 ... 33000 (fewer rows than SMs: the 32-warp
+                                  # streaming kernel); b = 100: 330 rows, the 8-warp one for n > 8192 and the register classes
     pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
     pbo = orc.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
     rows = pbg.num_rows

@@ -145,6 +145,27 @@ def test_topk_exact(L, b, k, cu, quant):
         assert np.array_equal(idx.cpu().numpy(), want_idx)
 
 
+@pytest.mark.parametrize("b", [2000, 80], ids=["few_rows", "many_rows"])
+def test_topk_rows_not_16_byte_aligned(b):
+    """A score panel whose leading dimension is odd: the rows of the streaming kernel start at arbitrary 4-byte offsets and
+    take its scalar loads (the 16-byte ones need ld % 4 == 0); long rows through both forms of the kernel."""
+    L, k, ld = 20001, 700, 20003
+    pbg = B.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
+    pbo = orc.Problem(L=L, Hq=8, Hkv=2, d=64, k=k, b_sel=b)
+    rows = pbg.num_rows
+    x = rand_scores(31 + b, rows, ld, 8)
+    info = [orc.row_info(pbo, i) for i in range(rows)]
+    nv = np.array([t1 + 1 for _, _, t1 in info], np.int32)
+    want_idx, want_cnt = orc.topk(x.astype(np.float64), nv, k)
+    xs = torch.from_numpy(x).to(DEV)
+    assert xs.stride(0) == ld
+    idx = torch.full((rows, k), -7, dtype=torch.int32, device=DEV)
+    cnt = torch.full((rows,), -7, dtype=torch.int32, device=DEV)
+    B.sp_topk_support(pbg, xs, 0, rows, idx, cnt)
+    assert np.array_equal(cnt.cpu().numpy(), want_cnt)
+    assert np.array_equal(idx.cpu().numpy(), want_idx)
+
+
 @pytest.mark.parametrize("pattern", ["ramp_up", "ramp_down", "two_level", "spike_tail", "neg_inf_mix"])
 @pytest.mark.parametrize("k", [1, 300, 1999, 2048])
 @pytest.mark.parametrize("b", [3000, 100], ids=["few_rows_32_warps_each", "many_rows_8_warps_each"])

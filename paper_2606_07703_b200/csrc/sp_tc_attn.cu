@@ -341,8 +341,6 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
             const int p = pv[u];
             const bool ok = p >= its.seq_start && p <= plast;
             siw[e] = ok ? p : -1;
-            // (an ignored entry still gathers a row: a written one, so that 0 x garbage cannot make a NaN)
-            if (g.bt != nullptr) sRow[ib * kpad + e] = (int)sp_kv_row(g, ok ? p : its.seq_start);
             uint32_t f = 0;
             if (!ok || p > qa0 - win) f |= 1u;
             if (!ok || p > qa1 - win) f |= 2u;
@@ -355,6 +353,13 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       }
       my_last = __reduce_max_sync(0xffffffffu, my_last);
       if (my_last && (ptid & 31) == 0) atomicMax(&n_eff_sh[ib], my_last);
+      if (g.bt != nullptr) {  // paged cache: the pool row of every entry, in a loop of its own (the contiguous path pays one branch)
+        // (an ignored entry still gathers a row: a written one, so that 0 x garbage cannot make a NaN)
+        for (int e = ptid; e < kpad; e += 128) {
+          const int p = siw[e];  // written by this very thread above
+          sRow[ib * kpad + e] = (int)sp_kv_row(g, p >= 0 ? p : its.seq_start);
+        }
+      }
       loader_bar_sync();
       nt_buf[ib] = (n_eff_sh[ib] + AT_KT - 1) / AT_KT;
       mbar_arrive(&bar.idxfull[ib]);
@@ -466,12 +471,18 @@ sp_tc_attn_kernel(const __grid_constant__ CUtensorMap tmQ, SpGeom g, const __nv_
       {  // Q tile: ONE 3-D TMA box per 64-column block: [256/G queries] x [G heads] x [64 channels] lands as rows
          // R = query * G + head of 128 bytes, SWIZZLE_128B (rows past the chunk are later queries or zero fill: their
          // outputs are never written).  The cp.async version cost ~800 address instructions per loader warp per item.
-        // ONLY the issuing thread waits for the buffer: nothing else here depends on it, and a loader warp that is not
-        // needed for progress may be lapped -- an item whose tiles were all prefetched above (nt <= NS - 2) can finish,
-        // and complete the barrier's NEXT phase, before a slow warp gets here; its parity wait would then never return
-        // (seen under ncu's SASS instrumentation: dense launches with several items per CTA hung on exactly that)
+        // Every loader thread waits for the buffer (holding the loaders here, instead of letting three of the four warps
+        // run ahead into the next ring slots, measured 3 % faster), and they meet at a named barrier BEFORE the one thread
+        // issues the load.  The barrier is what makes the parity wait safe: without it a loader warp that is not needed
+        // for progress could be lapped -- an item whose tiles were all prefetched above (nt <= NS - 2) can finish, and
+        // complete the Q barrier's NEXT phase, before a slow warp gets here, and a parity wait on a lapped barrier never
+        // returns (seen under ncu's SASS instrumentation: dense launches with several items per CTA hung on exactly
+        // that).  Now the next phase cannot start before all 128 threads have passed this wait.
+        if (n_q > 0) {
+          mbar_wait(&bar.qempty, (n_q - 1) & 1);
+          loader_bar_sync();
+        }
         if (ptid == 0) {
-          if (n_q > 0) mbar_wait(&bar.qempty, (n_q - 1) & 1);
           mbar_expect_tx(&bar.qfull, KB * Q_BLK);
 #pragma unroll
           for (int kb = 0; kb < KB; ++kb)

@@ -176,6 +176,29 @@ __device__ __forceinline__ void sc_epilogue(uint32_t trow, int warp_q, int lane,
       uint32_t v[32];
       tmem_ld_x32(trow + c0, v);
       tmem_ld_wait();
+      // interior chunk (the bulk of a per-query panel): all 32 x 32 pairs are causal, inside the sequence, inside the row
+      // panel and outside the local window -> multiply, store, step the pointer: no per-element tests (the kernel is
+      // bound by the instructions of this loop, not by the 2 GB it writes: ncu has ALU at 62 %, DRAM at 0.4 of the
+      // write rate a plain fill reaches)
+      const int rowc = hrow0 + c0;
+      if (s_hi <= t0 && t0 + 31 <= q_last && rowc >= row_begin && rowc + 31 < row_begin + row_count &&
+          (local_window <= 0 || t0 - s_hi >= local_window)) {
+        float* dst = scores + (size_t)(rowc - row_begin) * ld + s;
+        if (relu) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            *dst = fmaxf(__uint_as_float(v[j]) * idx_scale, 0.f);
+            dst += ld;
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            *dst = __uint_as_float(v[j]) * idx_scale;
+            dst += ld;
+          }
+        }
+        continue;
+      }
 #pragma unroll
       for (int j = 0; j < 32; ++j) {
         const int t = t0 + j;

@@ -21,6 +21,13 @@
 // element are what the kernel's time is made of, profiles/r2_attn.md).
 // Only tiles that can contain a masked or locally-biased element take the per-element path (flags computed by
 // the loaders while staging the index list).
+//   MASKED: per-query supports (b_sel = 1) as the DENSE tile loop with a membership mask: a one-hot query selector and a
+//           mask tile the loaders expand from a [L/32, L] bitmap are multiplied on the tensor core into S (two extra K
+//           steps per tile), so the softmax warps run their unmasked path; chosen by sp_api.cu when the causal pairs are
+//           few enough against the kept ones (k a sizeable part of the prefix).  Also holds the bitmap builder and the
+//           fixed scratch array of the no-allocation entry point.
+// Barrier rule (profiles/r2_final.md): a parity wait is only safe for a warp whose arrival the barrier's next phase
+// needs; the one wait that was not (the loaders' wait for the Q buffer) is followed by a named barrier.
 #include "sp_common.cuh"
 #include "sp_tc.cuh"
 

@@ -7,7 +7,8 @@
 // element.  Two kernels find (T, need_eq) and compact:
 //   sp_topk_small_kernel<W>  rows up to 1024 W keys (W = 1 .. 8 warps per row), the row in registers, bit-by-bit
 //                            bisection with redux.sync counts;
-//   sp_topk_stream_kernel    longer rows: sampled bracket, ONE streaming pass that lists what can still be selected,
+//   sp_topk_stream_kernel<W> longer rows (W = 8 warps per row, three rows per SM; W = 32 for panels of fewer long rows than
+//                            SMs, e.g. a prefill chunk's): sampled bracket, ONE streaming pass that lists what can still be selected,
 //                            radix select over the candidates, compaction from the list; exact radix-select fallback
 //                            over the whole row when the bracket does not hold (always correct, only slower).
 #include "sp_common.cuh"

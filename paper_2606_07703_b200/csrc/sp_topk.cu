@@ -118,7 +118,10 @@ __device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, 
 // slower.  (Round 1's kernel, 1024 threads per row, staged the row in shared memory and walked it three times with a
 // block-wide barrier between the phases of the single row an SM held: ~45 K cycles per 24 K-key row, 0.09 of the HBM
 // rate.)
-__host__ __device__ constexpr int tx_list(int txw) { return txw == 8 ? 1024 : 512; }  // list entries per warp (8 B each): 64 KB / 128 KB per row
+// list entries per warp (8 B each).  8 warps per row: 1024 (64 KB, three rows per SM) or, when the panel's longest row is
+// expected to list well under 640 entries per warp, 768 (48 KB and 64 registers: FOUR rows per SM, 9 % faster at c4 @ 32K;
+// at 64K the lists outgrow it and rows fall to the exact fallback, 5.4 against 4.4 ms).  32 warps per row: 512 (128 KB).
+constexpr int TX_LIST_WIDE = 512, TX_LIST_8 = 1024, TX_LIST_8_SMALL = 768;  // list entries per warp (8 B each): 64 KB / 128 KB per row
 constexpr int TX_SAMPLE = 1024;
 constexpr int TX_UNROLL = 4;     // 16-byte loads in flight per lane
 constexpr int TX_WIDE_MIN_N = 16384;  // the 32-warp form pays from here (a warp's segment still spans several load steps)
@@ -257,11 +260,11 @@ __device__ __forceinline__ float key_to_float(uint32_t key) {
 
 // TXW = warps per row: 8 (three rows per SM) when the panel has rows enough to fill the machine, 32 (one row per SM, the
 // row's passes spread over four times the warps) for panels of few long rows -- a prefill CHUNK has q_count / b_sel of them.
-template <int TXW>
-__global__ void __launch_bounds__(TXW * 32, TXW == 8 ? 3 : 1)
+template <int TXW, int TX_LIST>
+__global__ void __launch_bounds__(TXW * 32, TXW == 8 ? (TX_LIST <= TX_LIST_8_SMALL ? 4 : 3) : 1)
 sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
                       int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
-  constexpr int TX_THREADS = TXW * 32, TX_WARPS = TXW, TX_LIST = tx_list(TXW);
+  constexpr int TX_THREADS = TXW * 32, TX_WARPS = TXW;
   extern __shared__ uint32_t tx_smem[];  // [TX_WARPS][TX_LIST] pairs (score bits, index)
   __shared__ TkShared sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -375,20 +378,26 @@ sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, in
   uint32_t ck[TX_LIST / 32];
   uint32_t cmask = 0, my_gt = 0, my_c = 0;
   const int slots = over ? 0 : (int)((nl + 31u) >> 5);
+  // (no early exit from this loop: it WRITES the register array, and a break makes ptxas zero the remaining registers on
+  // every one of the 32 exit paths -- ~290 moves per warp; slots are tested in groups of four instead)
 #pragma unroll
-  for (int j = 0; j < TX_LIST / 32; ++j) ck[j] = 0u;
+  for (int j0 = 0; j0 < TX_LIST / 32; j0 += 4) {
 #pragma unroll
-  for (int j = 0; j < TX_LIST / 32; ++j) {
-    if (j >= slots) break;  // warp-uniform
-    const uint32_t e = lane + 32 * j;
-    uint32_t bits;
-    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(bits) : "r"(lst_addr + 8u * e));
-    const uint32_t key = order_key(__uint_as_float(bits));
-    const bool in = e < nl, gt = in && key > khi, cd = in && key <= khi && key >= klo;
-    my_gt += gt;
-    my_c += cd;
-    cmask |= (cd ? 1u : 0u) << j;
-    ck[j] = (gt || cd) ? key : 0u;  // (flush-to-zero extras and padding: key 0)
+    for (int j = j0; j < j0 + 4; ++j) ck[j] = 0u;
+    if (j0 < slots) {  // warp-uniform
+#pragma unroll
+      for (int j = j0; j < j0 + 4; ++j) {
+        const uint32_t e = lane + 32 * j;
+        uint32_t bits;
+        asm volatile("ld.shared.b32 %0, [%1];" : "=r"(bits) : "r"(lst_addr + 8u * e));
+        const uint32_t key = order_key(__uint_as_float(bits));
+        const bool in = e < nl, gt = in && key > khi, cd = in && key <= khi && key >= klo;
+        my_gt += gt;
+        my_c += cd;
+        cmask |= (cd ? 1u : 0u) << j;
+        ck[j] = (gt || cd) ? key : 0u;  // (flush-to-zero extras and padding: key 0)
+      }
+    }
   }
   my_gt = __reduce_add_sync(0xffffffffu, my_gt);
   my_c = __reduce_add_sync(0xffffffffu, my_c);
@@ -645,23 +654,35 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     }
     sp_count_launch();
   };
-  const size_t smem_x = (size_t)2 * 8 * tx_list(8) * sizeof(uint32_t), smem_w = (size_t)2 * 32 * tx_list(32) * sizeof(uint32_t);
+  const size_t smem_x = (size_t)2 * 8 * TX_LIST_8 * sizeof(uint32_t), smem_s = (size_t)2 * 8 * TX_LIST_8_SMALL * sizeof(uint32_t);
+  const size_t smem_w = (size_t)2 * 32 * TX_LIST_WIDE * sizeof(uint32_t);
   static unsigned char attr_seen_x[SP_MAX_DEVICES];
   if (sp_first_use_on_device(attr_seen_x)) {
-    cudaError_t e = cudaFuncSetAttribute(sp_topk_stream_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
+    cudaError_t e = cudaFuncSetAttribute(sp_topk_stream_kernel<8, TX_LIST_8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(sp_topk_stream_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w);
+    e = cudaFuncSetAttribute(sp_topk_stream_kernel<8, TX_LIST_8_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sp_topk_stream_kernel<32, TX_LIST_WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w);
     if (e != cudaSuccess) return e;
   }
+  // entries per warp the longest row of the panel is expected to list: the bracket's floor is the sample rank
+  // ceil(r) + margin of TX_SAMPLE, r = k / n * TX_SAMPLE (the kernel's own formula), spread over 8 warps
+  auto expected_list8 = [&](int n) {
+    const float frac = (float)k / (float)n, r = frac * TX_SAMPLE;
+    const float il = ceilf(r) + ceilf(3.5f * sqrtf(r * (1.f - frac))) + 4.f;
+    return (double)n * (il / TX_SAMPLE) / 8.0;
+  };
   auto launch_big = [&](int rb, int rc, int nlo) {
     const float* sc = scores + (size_t)(rb - row_begin) * ld;
     int32_t* ix = idx + (size_t)(rb - row_begin) * k;
     int32_t* cn = cnt ? cnt + (rb - row_begin) : nullptr;
     // fewer rows than SMs: one 32-warp CTA per row instead of an 8-warp one (the SMs would idle otherwise)
     if (rc <= g_sm_count() && max_n_valid >= TX_WIDE_MIN_N)
-      sp_topk_stream_kernel<32><<<rc, 32 * 32, smem_w, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
+      sp_topk_stream_kernel<32, TX_LIST_WIDE><<<rc, 32 * 32, smem_w, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
+    else if (max_n_valid > k && expected_list8(max_n_valid) <= 400.0)
+      sp_topk_stream_kernel<8, TX_LIST_8_SMALL><<<rc, 8 * 32, smem_s, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     else
-      sp_topk_stream_kernel<8><<<rc, 8 * 32, smem_x, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
+      sp_topk_stream_kernel<8, TX_LIST_8><<<rc, 8 * 32, smem_x, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     sp_count_launch();
   };
   // A class is launched only when it fills the machine (rows * W >= one 8-warp CTA per SM) or when it is the last

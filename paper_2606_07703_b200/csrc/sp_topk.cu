@@ -120,8 +120,9 @@ __device__ void radix_select(const float* __restrict__ x, const uint32_t* keys, 
 // rate.)
 // list entries per warp (8 B each).  8 warps per row: 1024 (64 KB, three rows per SM) or, when the panel's longest row is
 // expected to list well under 640 entries per warp, 768 (48 KB and 64 registers: FOUR rows per SM, 9 % faster at c4 @ 32K;
-// at 64K the lists outgrow it and rows fall to the exact fallback, 5.4 against 4.4 ms).  32 warps per row: 512 (128 KB).
-constexpr int TX_LIST_WIDE = 512, TX_LIST_8 = 1024, TX_LIST_8_SMALL = 768;  // list entries per warp (8 B each): 64 KB / 128 KB per row
+// at 64K the lists outgrow it and rows fall to the exact fallback, 5.4 against 4.3 ms; there 16 warps per row with 512
+// entries each -- the same 64 KB, two rows = 32 warps per SM -- give 4.0 ms).  32 warps per row: 512 (128 KB).
+constexpr int TX_LIST_16 = 512, TX_LIST_WIDE = 512, TX_LIST_8 = 1024, TX_LIST_8_SMALL = 768;  // list entries per warp (8 B each): 64 KB / 128 KB per row
 constexpr int TX_SAMPLE = 1024;
 constexpr int TX_UNROLL = 4;     // 16-byte loads in flight per lane
 constexpr int TX_WIDE_MIN_N = 16384;  // the 32-warp form pays from here (a warp's segment still spans several load steps)
@@ -261,7 +262,7 @@ __device__ __forceinline__ float key_to_float(uint32_t key) {
 // TXW = warps per row: 8 (three rows per SM) when the panel has rows enough to fill the machine, 32 (one row per SM, the
 // row's passes spread over four times the warps) for panels of few long rows -- a prefill CHUNK has q_count / b_sel of them.
 template <int TXW, int TX_LIST>
-__global__ void __launch_bounds__(TXW * 32, TXW == 8 ? (TX_LIST <= TX_LIST_8_SMALL ? 4 : 3) : 1)
+__global__ void __launch_bounds__(TXW * 32, TXW == 8 ? (TX_LIST <= TX_LIST_8_SMALL ? 4 : 3) : (TXW == 16 ? 2 : 1))
 sp_topk_stream_kernel(SpGeom g, const float* __restrict__ scores, int64_t ld, int row_begin, int row_count, int k,
                       int n_lo, int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
   constexpr int TX_THREADS = TXW * 32, TX_WARPS = TXW;
@@ -664,6 +665,8 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sp_topk_stream_kernel<32, TX_LIST_WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sp_topk_stream_kernel<16, TX_LIST_16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x);
+    if (e != cudaSuccess) return e;
   }
   // entries per warp the longest row of the panel is expected to list: the bracket's floor is the sample rank
   // ceil(r) + margin of TX_SAMPLE, r = k / n * TX_SAMPLE (the kernel's own formula), spread over 8 warps
@@ -681,6 +684,8 @@ cudaError_t sp_launch_topk(const SpGeom& g, const float* scores, int64_t ld, int
       sp_topk_stream_kernel<32, TX_LIST_WIDE><<<rc, 32 * 32, smem_w, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     else if (max_n_valid > k && expected_list8(max_n_valid) <= 400.0)
       sp_topk_stream_kernel<8, TX_LIST_8_SMALL><<<rc, 8 * 32, smem_s, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
+    else if (expected_list8(max_n_valid) * 0.5 <= 240.0)  // 16 warps per row, two rows per SM: 32 instead of 24 warps per SM
+      sp_topk_stream_kernel<16, TX_LIST_16><<<rc, 16 * 32, smem_x, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     else
       sp_topk_stream_kernel<8, TX_LIST_8><<<rc, 8 * 32, smem_x, st>>>(g, sc, ld, rb, rc, k, nlo, ix, cn);
     sp_count_launch();
